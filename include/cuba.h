@@ -1,0 +1,157 @@
+/*
+ * cuba.h -- C ABI of the B200-native CuBA hot path (arXiv:1208.0961, "CuBA - a CUDA
+ * implementation of BAMPS"; citations are /root/reference/PAPER.md line numbers).
+ *
+ * One call sequence, one GPU:   cuba_init -> cuba_step* -> cuba_observables -> cuba_destroy
+ *
+ * What a step computes (section 2; order per DESIGN.md reading A1):
+ *   S1  free streaming      x -> x + c^2 p_x/E dt, same for y,z        PAPER.md:34 Eq. 2
+ *   S2  wall reflection     elastic, off the six walls of the box
+ *   S3  cell index          cells of volume dx dy dz
+ *   S4  stable counting sort of the particle store by cell             north_star (3)
+ *   S5  per cell: Philox-keyed shuffle, pair 2k with 2k+1, collide with
+ *       P22 = v_rel (sigma/N_test)(dt/V_cell) * n(n-1)/(2 floor(n/2)),
+ *       v_rel = s/(2 E1 E2), s = (p1+p2)^2; on a hit boost to the CM frame,
+ *       draw an isotropic direction, boost back                        PAPER.md:38-44 Eq. 3
+ * All arithmetic is IEEE fp64, one rounding per written operation, no FMA contraction
+ * (A2), so a trajectory is a pure function of (initial state, seed).
+ *
+ * Conventions: c = 1; lengths fm, time fm/c, momenta and energies GeV, sigma in fm^2
+ * (10 GeV^-2 = 0.389379 fm^2 with hbar c = 0.197327 GeV fm).  Massless gluons: E = |p| is
+ * never stored.  `n_test` is the testparticle multiplier r_test of PAPER.md:44 (the divisor
+ * in Eq. 3, A3).
+ *
+ * Memory: every pointer is labelled DEVICE or HOST.  The caller (PyTorch in the shipped
+ * binding) allocates all device memory; the library allocates none on the cuba_step path.
+ * Errors: every call returns 0 or a negative CUBA_ERR_* code; nothing throws or aborts.
+ * There is no CPU fallback: without a CUDA device every call fails with CUBA_ERR_CUDA.
+ */
+#ifndef CUBA_H
+#define CUBA_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CUBA_OK 0
+#define CUBA_ERR_NULL (-1)        /* a required pointer is null                              */
+#define CUBA_ERR_SIZE (-2)        /* n < 1, n >= 2^32, ncell < 1, ncells >= 2^27, nslab < 1   */
+#define CUBA_ERR_VALUE (-3)       /* non-positive box / n_test / dt, negative sigma           */
+#define CUBA_ERR_WORKSPACE (-4)   /* workspace smaller than cuba_workspace_bytes or misaligned */
+#define CUBA_ERR_CUDA (-5)        /* a CUDA runtime call failed (cuba_last_cuda_error)        */
+#define CUBA_ERR_STATE (-6)       /* a particle outside [0,L], non-finite, or with p = 0      */
+#define CUBA_ERR_CFL (-7)         /* dt not below the smallest cell edge        */
+#define CUBA_ERR_MOVED (-8)       /* device check: a particle crossed more than one cell      */
+#define CUBA_ERR_ROUNDS (-9)      /* a cell needs more than CUBA_MAX_ROUNDS rounds (A6)       */
+#define CUBA_ERR_TRACE (-10)      /* trace capacity too small                                 */
+
+#define CUBA_MAX_ROUNDS 64
+
+typedef struct cuba_ctx cuba_ctx; /* opaque; owned by the library, freed by cuba_destroy */
+
+/* Device pointers to the current particle store (SoA, array order = cell-sorted order). */
+typedef struct cuba_soa {
+    double *x, *y, *z, *px, *py, *pz; /* DEVICE, n doubles each */
+    uint32_t *pid;                    /* DEVICE, n: persistent id = index in the arrays given to cuba_init */
+    uint32_t *cell_start;             /* DEVICE, ncells+1: slots [cell_start[c], cell_start[c+1]) hold cell c */
+} cuba_soa;
+
+typedef struct cuba_counters_t {
+    uint64_t steps;          /* steps done since cuba_init                                   */
+    uint64_t pairs;          /* collision-pair evaluations (sum over steps, cells, rounds)   */
+    uint64_t collisions;     /* pairs that collided                                          */
+    uint64_t rounds;         /* sum over steps and cells with n >= 2 of R(n) (A6)            */
+    uint64_t near_threshold; /* decisions with |u - P| <= 1e-12 (A16)                        */
+    uint64_t max_occupancy;  /* largest cell population seen                                 */
+    uint64_t overflow_cells; /* cells too large for shared memory, done by the global path   */
+    uint64_t device_flags;   /* sticky device error bits (0 when healthy)                    */
+} cuba_counters_t;
+
+/* Trace of ONE step for the bit-exact parity check.  All arrays are HOST memory owned by
+ * the caller.  Pairs are listed in (cell, round, k) order, k = index in the shuffled
+ * order; pair k of a round joins order[2k] (pid_a) and order[2k+1] (pid_b). */
+typedef struct cuba_trace {
+    uint32_t *cell_of_pid; /* HOST, n: cell index of every particle after S3, by pid       */
+    int64_t pair_capacity; /* in: entries available in the arrays below                    */
+    int64_t n_pairs;       /* out: pairs evaluated in this step                            */
+    uint32_t *pair_cell;   /* HOST, pair_capacity                                          */
+    uint32_t *pair_round;  /* HOST                                                         */
+    uint32_t *pid_a;       /* HOST                                                         */
+    uint32_t *pid_b;       /* HOST                                                         */
+    double *P;             /* HOST: scaled collision probability of Eq. 3                  */
+    double *u;             /* HOST: the uniform it was compared with                       */
+    uint8_t *decided;      /* HOST: 1 iff u < P                                            */
+} cuba_trace;
+
+/* Bytes of DEVICE workspace cuba_init needs for n particles on an ncell[0..2] grid
+ * (second copy of the particle store for the out-of-place sort, pid arrays, cell tables,
+ * sort scratch).  Returns 0 for invalid arguments.  The workspace must be 256-byte aligned. */
+size_t cuba_workspace_bytes(int64_t n, const int ncell[3]);
+
+/* Adopt a particle store.  PAPER.md:32 (cells, per-particle r and p), PAPER.md:44 (box with
+ * six walls at 0 and L; N_test).  x..pz are DEVICE arrays of n doubles, adopted in place and
+ * to be kept alive (with `workspace`) until cuba_destroy.  Assigns pid[i] = i, validates the
+ * state on the device (CUBA_ERR_STATE), and bins the initial positions with S3+S4 so that
+ * the store is cell-sorted from the start (A19); on return the caller's arrays
+ * hold the sorted state.  `cuda_stream` is a cudaStream_t (NULL = default stream); all later
+ * work is enqueued on it.  Synchronises once. */
+int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n,
+              double *x, double *y, double *z, double *px, double *py, double *pz,
+              double n_test, uint64_t seed, void *workspace, size_t workspace_bytes,
+              void *cuda_stream);
+
+/* Advance nsteps steps of S1..S5 with time step dt (fm/c) and total cross section sigma
+ * (fm^2).  Asynchronous: kernels are enqueued on the context's stream, no host
+ * synchronisation.  cuba_step(k) == k x cuba_step(1) bit for bit (the global step index is
+ * the only RNG state).  After the call the current store alternates between the caller's
+ * arrays and the workspace copy: ask cuba_state() where it is.  Errors: CUBA_ERR_VALUE,
+ * CUBA_ERR_CFL synchronously; device-side conditions (CUBA_ERR_MOVED, CUBA_ERR_ROUNDS)
+ * surface at the next synchronising call. */
+int cuba_step(cuba_ctx *ctx, int nsteps, double dt, double sigma);
+
+/* PAPER.md:66 (total energy) and PAPER.md:68-70 Fig. 2 (energy density along x).
+ * total = (sum E, sum px, sum py, sum pz) in GeV; edens[j] = sum_{i in slab j} E_i /
+ * (n_test * V_slab) in GeV/fm^3 for nslab equal slabs along x (lab-frame T^00, A15).
+ * HOST outputs; synchronises the stream and reports pending device errors. */
+int cuba_observables(cuba_ctx *ctx, double total[4], int nslab, double *edens);
+
+/* Where the current state lives (DEVICE pointers, valid until the next cuba_step). */
+int cuba_state(cuba_ctx *ctx, cuba_soa *out);
+
+/* Copy the current state to HOST arrays in array order (any pointer may be null). Synchronises. */
+int cuba_get_particles(cuba_ctx *ctx, uint32_t *pid, double *x, double *y, double *z,
+                       double *px, double *py, double *pz);
+
+/* Copy cell_start (ncells+1 entries) of the current state to HOST memory.  Synchronises. */
+int cuba_get_cells(cuba_ctx *ctx, uint32_t *cell_start);
+
+/* One step with the parity trace filled (slow path: allocates temporary device memory,
+ * synchronises).  The state advances exactly as with cuba_step(ctx, 1, dt, sigma). */
+int cuba_step_traced(cuba_ctx *ctx, double dt, double sigma, cuba_trace *out);
+
+/* Counters since cuba_init.  Synchronises. */
+int cuba_counters(cuba_ctx *ctx, cuba_counters_t *out);
+
+/* End-to-end convenience for HOST-resident data: allocates device memory, uploads the six
+ * HOST arrays (n doubles each), runs cuba_init + cuba_step(nsteps) + cuba_observables,
+ * optionally downloads the final state into the same HOST arrays (pid_out may be null;
+ * download != 0 to copy back), frees everything.  Used for the bench's e2e number. */
+int cuba_run_host(const double box[3], const int ncell[3], int64_t n,
+                  double *x, double *y, double *z, double *px, double *py, double *pz,
+                  double n_test, uint64_t seed, int nsteps, double dt, double sigma,
+                  double total[4], int nslab, double *edens, uint32_t *pid_out, int download);
+
+void cuba_destroy(cuba_ctx *ctx);
+const char *cuba_strerror(int code);
+/* Text of the last CUDA runtime error seen by this library in the calling process. */
+const char *cuba_last_cuda_error(void);
+/* Number of kernel launches this library has issued in the calling process. */
+uint64_t cuba_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CUBA_H */

@@ -1,0 +1,12 @@
+"""B200-native CuBA hot path (arXiv:1208.0961): thin Python binding over the C-ABI library
+`libcuba.so` (include/cuba.h).  Argument marshalling only -- every step of the path runs in
+the hand-written sm_100a kernels under csrc/.  PyTorch supplies device memory and streams.
+
+There is no CPU fallback: importing works anywhere (so the ABI can be inspected), but every
+compute call needs the built library and a CUDA device and fails loudly otherwise.
+"""
+from .binding import (Cuba, CubaError, Counters, Trace, lib, lib_path, run_host,  # noqa: F401
+                      workspace_bytes, launch_count, strerror, EXPORTS)
+
+__all__ = ["Cuba", "CubaError", "Counters", "Trace", "lib", "lib_path", "run_host",
+           "workspace_bytes", "launch_count", "strerror", "EXPORTS"]

@@ -1,0 +1,351 @@
+// bin.cuh -- S1-S4: streaming, wall reflection, cell index and the stable counting sort.
+//
+// B200-first design:
+// the store is always cell-sorted (A19) and dt < cell edge, so a particle of
+// old cell c can only land in one of the 27 cells around c.  A counting sort keyed by
+// (old cell, direction d in 0..26) is therefore sparse:
+//   K_A  k_stream_hist   per particle: S1-S3, d; cnt[d][c_old] += 1   (order-free u32 adds)
+//   K_B  k_gather        per new cell: the <= 27 (source cell, d) counts that feed it, taken
+//                        in ascending source-cell order = ascending previous array index,
+//                        turned into exclusive offsets in place; their sum is the new count
+//   K_S/K_F              exclusive scan of the new counts -> cell_start
+//   K_carry              per tile: particles of the tile's first cell that sit in earlier tiles
+//   K_C  k_scatter       per particle again: S1-S3 recomputed, stable rank inside its
+//                        (c_old, d) group from warp ballots, dest = cell_start[c_new] +
+//                        off[d][c_old] + rank.  No atomics touch the order: the placement is
+//                        the stable counting sort of north_star (3), deterministic by construction.
+// HBM traffic per particle-step: K_A reads 48 B, K_C reads 52 B and writes 52 B.
+#pragma once
+#include "common.cuh"
+
+namespace cuba {
+
+struct Moved {
+    double x, y, z, px, py, pz;
+    uint32_t c_old, c_new;
+    int d;   // direction code, -1 when the particle crossed more than one cell (error)
+};
+
+__device__ __forceinline__ Moved move_particle(const Geom &g, double dt, double x, double y,
+                                               double z, double px, double py, double pz)
+{
+    Moved m;
+    const int ix0 = axis_index(x, g.inv_d[0], g.nc[0]);
+    const int iy0 = axis_index(y, g.inv_d[1], g.nc[1]);
+    const int iz0 = axis_index(z, g.inv_d[2], g.nc[2]);
+    m.c_old = cell_linear(g, ix0, iy0, iz0);
+    stream_reflect(g, dt, x, y, z, px, py, pz);
+    const int ix1 = axis_index(x, g.inv_d[0], g.nc[0]);
+    const int iy1 = axis_index(y, g.inv_d[1], g.nc[1]);
+    const int iz1 = axis_index(z, g.inv_d[2], g.nc[2]);
+    m.c_new = cell_linear(g, ix1, iy1, iz1);
+    const int dx = ix1 - ix0 + 1, dy = iy1 - iy0 + 1, dz = iz1 - iz0 + 1;
+    m.d = ((unsigned)dx <= 2u && (unsigned)dy <= 2u && (unsigned)dz <= 2u) ? (dx * 9 + dy * 3 + dz) : -1;
+    m.x = x; m.y = y; m.z = z; m.px = px; m.py = py; m.pz = pz;
+    return m;
+}
+
+// ---- K_A ------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kTileThreads)
+k_stream_hist(Geom g, double dt, int64_t n, Soa in, uint32_t *__restrict__ cnt,
+              uint32_t *__restrict__ tile_rec, uint32_t *__restrict__ flags)
+{
+    __shared__ uint32_t s_tail[kDirs];
+    __shared__ uint32_t s_cf, s_cl;
+    const int tid = threadIdx.x;
+    const int64_t base = (int64_t)blockIdx.x * kTile;
+    const int64_t last = min(n, base + kTile) - 1;
+    if (tid < kDirs) s_tail[tid] = 0;
+
+    uint32_t c_old[kTileItems];
+    int d[kTileItems];
+#pragma unroll
+    for (int j = 0; j < kTileItems; ++j) {
+        const int64_t i = base + j * kTileThreads + tid;
+        const bool valid = i < n;
+        c_old[j] = 0; d[j] = -1;
+        const uint32_t active = __ballot_sync(0xFFFFFFFFu, valid);
+        if (valid) {
+            Moved m = move_particle(g, dt, in.x[i], in.y[i], in.z[i], in.px[i], in.py[i], in.pz[i]);
+            c_old[j] = m.c_old; d[j] = m.d;
+            if (m.d < 0) atomicOr(flags, kFlagMoved);
+            const uint32_t key = (uint32_t)max(m.d, 0) * g.ncells + m.c_old;
+            const uint32_t peers = __match_any_sync(active, key);
+            if ((peers & lanemask_lt()) == 0) atomicAdd(&cnt[key], (uint32_t)__popc(peers));
+            if (i == base) s_cf = m.c_old;
+            if (i == last) s_cl = m.c_old;
+        }
+    }
+    __syncthreads();
+    const uint32_t cl = s_cl;
+    // tail record: how many particles of the tile's LAST cell, per direction (feeds K_carry)
+#pragma unroll
+    for (int j = 0; j < kTileItems; ++j) {
+        const int64_t i = base + j * kTileThreads + tid;
+        const bool mine = (i < n) && c_old[j] == cl;
+        const uint32_t active = __ballot_sync(0xFFFFFFFFu, mine);
+        if (mine) {
+            const int dd = max(d[j], 0);
+            const uint32_t peers = __match_any_sync(active, dd);
+            if ((peers & lanemask_lt()) == 0) atomicAdd(&s_tail[dd], (uint32_t)__popc(peers));
+        }
+    }
+    __syncthreads();
+    uint32_t *rec = tile_rec + (size_t)blockIdx.x * kTileRec;
+    if (tid < kDirs) rec[tid] = s_tail[tid];
+    if (tid == 27) rec[27] = s_cf;
+    if (tid == 28) rec[28] = s_cl;
+}
+
+// ---- K_B ------------------------------------------------------------------------------
+// One thread per NEW cell.  Sources in ascending linear index (x slowest) == ascending
+// previous array position, which is what makes the placement stable (A8).
+__global__ void __launch_bounds__(256)
+k_gather(Geom g, uint32_t *__restrict__ cnt, uint32_t *__restrict__ count_new,
+         uint32_t *__restrict__ block_sum)
+{
+    __shared__ uint32_t s_warp[8];
+    const uint32_t c = blockIdx.x * 256u + threadIdx.x;
+    uint32_t run = 0;
+    if (c < g.ncells) {
+        const int iz = c % g.nc[2];
+        const int iy = (c / g.nc[2]) % g.nc[1];
+        const int ix = c / (g.nc[2] * g.nc[1]);
+        for (int ox = -1; ox <= 1; ++ox) {
+            const int sx = ix + ox;
+            if (sx < 0 || sx >= g.nc[0]) continue;
+            for (int oy = -1; oy <= 1; ++oy) {
+                const int sy = iy + oy;
+                if (sy < 0 || sy >= g.nc[1]) continue;
+                for (int oz = -1; oz <= 1; ++oz) {
+                    const int sz = iz + oz;
+                    if (sz < 0 || sz >= g.nc[2]) continue;
+                    const int dcode = (1 - ox) * 9 + (1 - oy) * 3 + (1 - oz);   // the source moved by -o
+                    const size_t e = (size_t)dcode * g.ncells + cell_linear(g, sx, sy, sz);
+                    const uint32_t v = cnt[e];
+                    cnt[e] = run;
+                    run += v;
+                }
+            }
+        }
+        count_new[c] = run;
+    }
+    uint32_t s = run;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
+    if ((threadIdx.x & 31) == 0) s_warp[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t t = 0;
+        for (int w = 0; w < 8; ++w) t += s_warp[w];
+        block_sum[blockIdx.x] = t;
+    }
+}
+
+// ---- K_S: exclusive scan of the per-block sums (one CTA), also resets the per-step
+// work counters of the collision kernels ------------------------------------------------
+__global__ void __launch_bounds__(1024)
+k_scan_blocks(uint32_t *__restrict__ block_sum, int nblocks, uint32_t *__restrict__ zero_me, int nzero)
+{
+    __shared__ uint32_t s_warp[32];
+    __shared__ uint32_t s_carry;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    if (tid < nzero) zero_me[tid] = 0;
+    if (tid == 0) s_carry = 0;
+    __syncthreads();
+    for (int b0 = 0; b0 < nblocks; b0 += 1024) {
+        const int i = b0 + tid;
+        const uint32_t v = (i < nblocks) ? block_sum[i] : 0u;
+        uint32_t inc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) s_warp[wid] = inc;
+        __syncthreads();
+        if (wid == 0) {
+            uint32_t w = s_warp[lane], winc = w;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, winc, o);
+                if (lane >= o) winc += t;
+            }
+            s_warp[lane] = winc - w;   // exclusive over warps
+        }
+        __syncthreads();
+        const uint32_t carry = s_carry;
+        if (i < nblocks) block_sum[i] = carry + s_warp[wid] + inc - v;
+        __syncthreads();
+        if (tid == 1023) s_carry = carry + s_warp[wid] + inc;
+        __syncthreads();
+    }
+}
+
+// ---- K_F: cell_start = block prefix + local exclusive scan; cells with n >= 2 are appended
+// to the work list of their size class for the collision kernels -------------------------
+constexpr int kNumClasses = 5;   // 4 shared-memory classes + the global-memory overflow class
+
+struct ClassTable {
+    uint32_t max_n[kNumClasses];   // inclusive upper bound of each class (last = UINT32_MAX)
+};
+
+__global__ void __launch_bounds__(256)
+k_cell_start(uint32_t ncells, const uint32_t *__restrict__ count_new,
+             const uint32_t *__restrict__ block_prefix, uint32_t *__restrict__ cell_start,
+             ClassTable ct, uint32_t *__restrict__ class_count, uint32_t *__restrict__ class_list,
+             unsigned long long *__restrict__ max_occ)
+{
+    __shared__ uint32_t s_warp[8];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const uint32_t c = blockIdx.x * 256u + tid;
+    const uint32_t v = (c < ncells) ? count_new[c] : 0u;
+    uint32_t inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) s_warp[wid] = inc;
+    __syncthreads();
+    uint32_t wpre = 0;
+    for (int w = 0; w < wid; ++w) wpre += s_warp[w];
+    const uint32_t start = block_prefix[blockIdx.x] + wpre + inc - v;
+    if (c < ncells) {
+        cell_start[c] = start;
+        if (c == ncells - 1) cell_start[ncells] = start + v;
+    }
+    // size class (warp-aggregated append; the list order does not affect any result)
+    int k = -1;
+    if (v >= 2) {
+        k = 0;
+        while (v > ct.max_n[k]) ++k;
+    }
+    const uint32_t peers = __match_any_sync(0xFFFFFFFFu, k);
+    if (k >= 0) {
+        const int leader = __ffs(peers) - 1;
+        uint32_t pos = 0;
+        if (lane == leader) pos = atomicAdd(&class_count[k], (uint32_t)__popc(peers));
+        pos = __shfl_sync(peers, pos, leader) + __popc(peers & lanemask_lt());
+        class_list[(size_t)k * ncells + pos] = c;
+    }
+    uint32_t vmax = v;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) vmax = max(vmax, __shfl_xor_sync(0xFFFFFFFFu, vmax, o));
+    if (lane == 0 && vmax > 0) atomicMax(max_occ, (unsigned long long)vmax);
+}
+
+// ---- K_carry ---------------------------------------------------------------------------
+// carry[b][d] = number of particles with (cell = first cell of tile b, direction d) that sit in
+// tiles before b.  One warp per tile (lane = d).  A tile starts a walk for its last cell
+// unless it lies in the middle of that cell's run; the walk is linear in the run length.
+__global__ void __launch_bounds__(256)
+k_carry(int ntiles, const uint32_t *__restrict__ tile_rec, uint32_t *__restrict__ carry)
+{
+    const int lane = threadIdx.x & 31;
+    const int b = blockIdx.x * 8 + (threadIdx.x >> 5);
+    if (b >= ntiles || lane >= kDirs) return;
+    const uint32_t *rec = tile_rec + (size_t)b * kTileRec;
+    const uint32_t cf = rec[27], cl = rec[28];
+    const bool has_carry = b > 0 && tile_rec[(size_t)(b - 1) * kTileRec + 28] == cf;
+    if (!has_carry) carry[(size_t)b * kTileRec + lane] = 0;
+    const bool middle = has_carry && cf == cl;
+    if (middle) return;
+    uint32_t acc = rec[lane];
+    for (int bb = b + 1; bb < ntiles; ++bb) {
+        const uint32_t *r2 = tile_rec + (size_t)bb * kTileRec;
+        if (r2[27] != cl) break;
+        carry[(size_t)bb * kTileRec + lane] = acc;
+        if (r2[28] != cl) break;
+        acc += r2[lane];
+    }
+}
+
+// ---- K_C ------------------------------------------------------------------------------
+// Rows are the 32 consecutive particles one warp handles for one item; row r = j*8 + warp,
+// local index li = r*32 + lane = j*256 + tid.  prefix_d(li) = number of particles before li
+// in the tile that moved in direction d.  Stable rank inside (c_old, d) =
+// prefix_d(li) - prefix_d(first particle of c_old in the tile) [+ carry if that is li 0].
+template <bool WITH_CELL_OF_PID>
+__global__ void __launch_bounds__(kTileThreads)
+k_scatter(Geom g, double dt, int64_t n, Soa in, Soa out, const uint32_t *__restrict__ off,
+          const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ carry,
+          uint32_t *__restrict__ cell_of_pid)
+{
+    __shared__ uint32_t s_cold[kTile];
+    __shared__ uint32_t s_ball[kTileRows][kDirs];
+    __shared__ uint32_t s_pref[kTileRows][kDirs];
+    __shared__ uint32_t s_head[kTileRows];
+    __shared__ int s_lasthead[kTileRows];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int64_t base = (int64_t)blockIdx.x * kTile;
+
+    Moved m[kTileItems];
+    uint32_t pid[kTileItems];
+#pragma unroll
+    for (int j = 0; j < kTileItems; ++j) {
+        const int64_t i = base + j * kTileThreads + tid;
+        m[j].d = -1; m[j].c_old = 0xFFFFFFFFu;
+        if (i < n) {
+            m[j] = move_particle(g, dt, in.x[i], in.y[i], in.z[i], in.px[i], in.py[i], in.pz[i]);
+            pid[j] = in.pid[i];
+        }
+        s_cold[j * kTileThreads + tid] = m[j].c_old;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < kTileItems; ++j) {
+        const int r = j * (kTileThreads / 32) + wid;
+        const int li = j * kTileThreads + tid;
+        const bool valid = (base + li) < n;
+        const int dd = m[j].d;
+        uint32_t mine = 0;
+#pragma unroll
+        for (int q = 0; q < kDirs; ++q) {
+            const uint32_t b = __ballot_sync(0xFFFFFFFFu, dd == q);
+            if (lane == q) mine = b;
+        }
+        if (lane < kDirs) s_ball[r][lane] = mine;
+        const bool head = valid && (li == 0 || s_cold[li - 1] != m[j].c_old);
+        const uint32_t hb = __ballot_sync(0xFFFFFFFFu, head);
+        if (lane == 0) s_head[r] = hb;
+    }
+    __syncthreads();
+    if (tid < kDirs) {
+        uint32_t run = 0;
+        for (int r = 0; r < kTileRows; ++r) {
+            s_pref[r][tid] = run;
+            run += __popc(s_ball[r][tid]);
+        }
+    } else if (tid == 32) {
+        int lh = -1;
+        for (int r = 0; r < kTileRows; ++r) {
+            s_lasthead[r] = lh;
+            const uint32_t hb = s_head[r];
+            if (hb) lh = r * 32 + 31 - __clz(hb);
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < kTileItems; ++j) {
+        const int li = j * kTileThreads + tid;
+        if ((base + li) >= n) continue;
+        const int dd = m[j].d;
+        if (dd < 0) continue;   // flagged by K_A; the particle is dropped from the placement
+        const int r = j * (kTileThreads / 32) + wid;
+        const uint32_t pre_i = s_pref[r][dd] + __popc(s_ball[r][dd] & lanemask_lt());
+        const uint32_t hm = s_head[r] & lanemask_le();
+        const int sli = hm ? (r * 32 + 31 - __clz(hm)) : s_lasthead[r];
+        const int rs = sli >> 5, ls = sli & 31;
+        const uint32_t pre_s = s_pref[rs][dd] + __popc(s_ball[rs][dd] & ((1u << ls) - 1u));
+        uint32_t rank = pre_i - pre_s;
+        if (sli == 0) rank += carry[(size_t)blockIdx.x * kTileRec + dd];
+        const uint32_t dest = cell_start[m[j].c_new] + off[(size_t)dd * g.ncells + m[j].c_old] + rank;
+        out.x[dest] = m[j].x; out.y[dest] = m[j].y; out.z[dest] = m[j].z;
+        out.px[dest] = m[j].px; out.py[dest] = m[j].py; out.pz[dest] = m[j].pz;
+        out.pid[dest] = pid[j];
+        if (WITH_CELL_OF_PID) cell_of_pid[pid[j]] = m[j].c_new;
+    }
+}
+
+}  // namespace cuba

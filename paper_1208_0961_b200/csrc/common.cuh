@@ -1,0 +1,116 @@
+// common.cuh -- shared device helpers of the CuBA B200 library: geometry, Eq. 2 streaming,
+// wall reflection, cell index, Philox4x32-10.  Compiled with -fmad=false: every written
+// fp64 operation rounds once (A2).  Citations: /root/reference/PAPER.md lines.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace cuba {
+
+constexpr int kDirs = 27;           // (dix+1)*9 + (diy+1)*3 + (diz+1), each di in {-1,0,1}
+constexpr int kTileThreads = 256;
+constexpr int kTileItems = 4;
+constexpr int kTile = kTileThreads * kTileItems;   // particles per tile in the flat passes
+constexpr int kTileRows = kTile / 32;
+constexpr int kTileRec = 32;        // u32 words per tile record: 27 counts, cf, cl, pad
+
+// device error bits (sticky)
+constexpr uint32_t kFlagMoved = 1u;    // a particle crossed more than one cell in a step
+constexpr uint32_t kFlagRounds = 2u;   // a cell needed more than CUBA_MAX_ROUNDS rounds
+constexpr uint32_t kFlagState = 4u;    // invalid particle at init
+constexpr uint32_t kFlagTrace = 8u;    // trace capacity exceeded
+
+constexpr uint32_t kTagShuf = 0u, kTagDec = 1u, kTagDir = 2u;
+
+struct Geom {
+    double L[3];       // box edges, walls at 0 and L
+    double inv_d[3];   // 1/(L/ncell) per axis
+    int nc[3];         // cells per axis
+    uint32_t ncells;
+};
+
+struct Soa {
+    double *x, *y, *z, *px, *py, *pz;
+    uint32_t *pid;
+};
+
+// ---- Philox4x32-10 (Salmon et al., SC'11): ten rounds of two 32x32->64 multiplies -------
+struct U4 { uint32_t x, y, z, w; };
+
+__device__ __forceinline__ U4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                            uint32_t k0, uint32_t k1)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    return U4{c0, c1, c2, c3};
+}
+
+// counter = {particle id, global step t, round rho, tag<<16 | sub}; key = seed (DESIGN.md RNG)
+__device__ __forceinline__ U4 draw(uint64_t seed, uint32_t id, uint32_t t, uint32_t rho,
+                                   uint32_t tag, uint32_t sub)
+{
+    return philox4x32_10(id, t, rho, (tag << 16) | sub, (uint32_t)seed, (uint32_t)(seed >> 32));
+}
+
+// ---- S1-S3 ---------------------------------------------------------------------------
+__device__ __forceinline__ double energy(double px, double py, double pz)
+{
+    return sqrt((px * px + py * py) + pz * pz);      // massless: E = |p|
+}
+
+__device__ __forceinline__ void reflect_axis(double &x, double &p, double L)
+{
+    if (x < 0.0) { x = -x; p = -p; }                 // PAPER.md:44, walls at 0 and L (A12)
+    else if (x > L) { x = 2.0 * L - x; p = -p; }
+}
+
+__device__ __forceinline__ void stream_reflect(const Geom &g, double dt, double &x, double &y,
+                                               double &z, double &px, double &py, double &pz)
+{
+    const double E = energy(px, py, pz);
+    const double w = dt / E;                         // PAPER.md:34 Eq. 2 with c = 1
+    x = x + px * w;
+    y = y + py * w;
+    z = z + pz * w;
+    reflect_axis(x, px, g.L[0]);
+    reflect_axis(y, py, g.L[1]);
+    reflect_axis(z, pz, g.L[2]);
+}
+
+__device__ __forceinline__ int axis_index(double x, double inv_d, int nc)
+{
+    int i = __double2int_rz(x * inv_d);
+    i = min(i, nc - 1);                              // x == L lands in the last cell (A12)
+    return max(i, 0);
+}
+
+__device__ __forceinline__ uint32_t cell_linear(const Geom &g, int ix, int iy, int iz)
+{
+    return ((uint32_t)ix * (uint32_t)g.nc[1] + (uint32_t)iy) * (uint32_t)g.nc[2] + (uint32_t)iz;
+}
+
+__device__ __forceinline__ uint32_t lanemask_lt()
+{
+    uint32_t m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+
+__device__ __forceinline__ uint32_t lanemask_le()
+{
+    uint32_t m;
+    asm("mov.u32 %0, %%lanemask_le;" : "=r"(m));
+    return m;
+}
+
+// streaming loads/stores: every particle array is touched once per pass
+__device__ __forceinline__ double ld_stream(const double *p) { return __ldcs(p); }
+__device__ __forceinline__ uint32_t ld_stream(const uint32_t *p) { return __ldcs(p); }
+
+}  // namespace cuba

@@ -1,0 +1,579 @@
+// cuba_api.cu -- the C ABI of include/cuba.h: argument validation, workspace carving and
+// stream-ordered kernel launches.  No CPU fallback: every entry point needs a CUDA device.
+#include "../../include/cuba.h"
+
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "bin.cuh"
+#include "collide.cuh"
+#include "common.cuh"
+#include "init_sort.cuh"
+#include "observe.cuh"
+
+using namespace cuba;
+
+namespace {
+
+std::atomic<uint64_t> g_launches{0};
+thread_local char g_cuda_err[256] = "";
+
+bool cuda_ok(cudaError_t e, const char *what)
+{
+    if (e == cudaSuccess) return true;
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", what, cudaGetErrorString(e));
+    return false;
+}
+#define CU(call) do { if (!cuda_ok((call), #call)) return CUBA_ERR_CUDA; } while (0)
+#define LAUNCHED() do { g_launches.fetch_add(1, std::memory_order_relaxed); if (!cuda_ok(cudaGetLastError(), "kernel launch")) return CUBA_ERR_CUDA; } while (0)
+
+// size classes of the collision kernels: threads per CTA, capacity (particles per cell)
+constexpr int kThrS = 32, kCapS = 64;
+constexpr int kThrM = 128, kCapM = 512;
+constexpr int kThrL = 512, kCapL = 2048;
+constexpr int kThrX = 1024, kCapX = 4544;
+
+size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+struct Layout {
+    size_t setB[6], pidA, pidB, cnt, count_new, cell_start, block_sum, tile_rec, carry, class_list,
+        zero, counters, flags, max_occ, obs_partial, obs_result, arena32, arenaE, rsH, total;
+    int64_t ntiles, nblocks_cells, rs_blocks, arena_entries;
+};
+
+constexpr int kObsGrid = 296;
+constexpr int kZeroWords = 16;   // class_count[5], work[5], arena cursor (u64 = 2 words), pad
+
+Layout make_layout(int64_t n, int64_t ncells)
+{
+    Layout L{};
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+    L.ntiles = (n + kTile - 1) / kTile;
+    L.nblocks_cells = (ncells + 255) / 256;
+    L.rs_blocks = (n + kRsTile - 1) / kRsTile;
+    L.arena_entries = n + 2 * ncells + 8;
+    for (int k = 0; k < 6; ++k) L.setB[k] = take((size_t)n * 8);
+    L.pidA = take((size_t)n * 4);
+    L.pidB = take((size_t)n * 4);
+    L.cnt = take((size_t)kDirs * ncells * 4);
+    L.count_new = take((size_t)ncells * 4);
+    L.cell_start = take((size_t)(ncells + 1) * 4);
+    L.block_sum = take((size_t)L.nblocks_cells * 4);
+    L.tile_rec = take((size_t)L.ntiles * kTileRec * 4);
+    L.carry = take((size_t)L.ntiles * kTileRec * 4);
+    L.class_list = take((size_t)kNumClasses * ncells * 4);
+    L.zero = take(kZeroWords * 4);
+    L.counters = take(8 * 8);
+    L.flags = take(4);
+    L.max_occ = take(8);
+    L.obs_partial = take((size_t)kObsGrid * (4 + kObsMaxSlabs) * 8);
+    L.obs_result = take((size_t)(4 + kObsMaxSlabs) * 8);
+    L.arena32 = take((size_t)L.arena_entries * 16);   // also the init sort's key/value double buffers
+    L.arenaE = take((size_t)L.arena_entries * 8);
+    L.rsH = take((size_t)256 * L.rs_blocks * 4);
+    L.total = o;
+    return L;
+}
+
+}  // namespace
+
+struct cuba_ctx {
+    Geom g;
+    int64_t n;
+    double n_test;
+    double box[3];
+    uint64_t seed;
+    uint32_t t;          // global step index
+    uint64_t steps;
+    cudaStream_t stream;
+    Layout lay;
+    unsigned char *ws;
+    Soa set[2];          // [0] caller's arrays + pidA, [1] workspace copy + pidB
+    int cur;
+    int grid_s, grid_m, grid_l, grid_x, grid_o;
+    double *h_obs;       // pinned staging for observables
+    template <typename T> T *at(size_t off) const { return reinterpret_cast<T *>(ws + off); }
+};
+
+// The exported functions take C linkage from their declarations in cuba.h.
+
+const char *cuba_strerror(int code)
+{
+    switch (code) {
+    case CUBA_OK: return "ok";
+    case CUBA_ERR_NULL: return "null pointer";
+    case CUBA_ERR_SIZE: return "size out of range";
+    case CUBA_ERR_VALUE: return "value out of range";
+    case CUBA_ERR_WORKSPACE: return "workspace too small or misaligned";
+    case CUBA_ERR_CUDA: return "CUDA runtime error";
+    case CUBA_ERR_STATE: return "invalid particle state";
+    case CUBA_ERR_CFL: return "dt not below the smallest cell edge";
+    case CUBA_ERR_MOVED: return "a particle crossed more than one cell in a step";
+    case CUBA_ERR_ROUNDS: return "a cell needs more than 64 collision rounds";
+    case CUBA_ERR_TRACE: return "trace capacity too small";
+    default: return "unknown error";
+    }
+}
+
+const char *cuba_last_cuda_error(void) { return g_cuda_err; }
+uint64_t cuba_launch_count(void) { return g_launches.load(); }
+
+static int check_grid(int64_t n, const int ncell[3], int64_t *ncells_out)
+{
+    if (!ncell) return CUBA_ERR_NULL;
+    if (n < 1 || n >= ((int64_t)1 << 32)) return CUBA_ERR_SIZE;
+    for (int k = 0; k < 3; ++k) if (ncell[k] < 1) return CUBA_ERR_SIZE;
+    const int64_t ncells = (int64_t)ncell[0] * ncell[1] * ncell[2];
+    if (ncells >= ((int64_t)1 << 27)) return CUBA_ERR_SIZE;
+    *ncells_out = ncells;
+    return CUBA_OK;
+}
+
+size_t cuba_workspace_bytes(int64_t n, const int ncell[3])
+{
+    int64_t ncells;
+    if (check_grid(n, ncell, &ncells) != CUBA_OK) return 0;
+    return make_layout(n, ncells).total;
+}
+
+static int device_flags_to_error(uint32_t f)
+{
+    if (f & kFlagState) return CUBA_ERR_STATE;
+    if (f & kFlagMoved) return CUBA_ERR_MOVED;
+    if (f & kFlagRounds) return CUBA_ERR_ROUNDS;
+    if (f & kFlagTrace) return CUBA_ERR_TRACE;
+    return CUBA_OK;
+}
+
+static int sync_and_check(cuba_ctx *ctx)
+{
+    uint32_t f = 0;
+    CU(cudaMemcpyAsync(&f, ctx->at<uint32_t>(ctx->lay.flags), 4, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return device_flags_to_error(f);
+}
+
+template <typename K>
+static int occupancy_grid(K kernel, int threads, size_t smem, int sms, int *grid)
+{
+    if (smem > 48 * 1024)
+        CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int per_sm = 0;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem));
+    if (per_sm < 1) per_sm = 1;
+    *grid = per_sm * sms;
+    return CUBA_OK;
+}
+
+int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n,
+              double *x, double *y, double *z, double *px, double *py, double *pz,
+              double n_test, uint64_t seed, void *workspace, size_t workspace_bytes,
+              void *cuda_stream)
+{
+    if (!out || !box || !ncell || !x || !y || !z || !px || !py || !pz || !workspace) return CUBA_ERR_NULL;
+    *out = nullptr;
+    int64_t ncells;
+    int rc = check_grid(n, ncell, &ncells);
+    if (rc != CUBA_OK) return rc;
+    for (int k = 0; k < 3; ++k) if (!(box[k] > 0.0) || !std::isfinite(box[k])) return CUBA_ERR_VALUE;
+    if (!(n_test > 0.0) || !std::isfinite(n_test)) return CUBA_ERR_VALUE;
+    Layout lay = make_layout(n, ncells);
+    if (workspace_bytes < lay.total || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return CUBA_ERR_WORKSPACE;
+
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+
+    cuba_ctx *ctx = new (std::nothrow) cuba_ctx();
+    if (!ctx) return CUBA_ERR_CUDA;
+    ctx->n = n; ctx->n_test = n_test; ctx->seed = seed; ctx->t = 0; ctx->steps = 0;
+    ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    ctx->lay = lay;
+    ctx->ws = static_cast<unsigned char *>(workspace);
+    for (int k = 0; k < 3; ++k) {
+        ctx->box[k] = box[k];
+        ctx->g.L[k] = box[k];
+        ctx->g.nc[k] = ncell[k];
+        ctx->g.inv_d[k] = 1.0 / (box[k] / (double)ncell[k]);
+    }
+    ctx->g.ncells = (uint32_t)ncells;
+    ctx->set[0] = Soa{x, y, z, px, py, pz, ctx->at<uint32_t>(lay.pidA)};
+    ctx->set[1] = Soa{ctx->at<double>(lay.setB[0]), ctx->at<double>(lay.setB[1]), ctx->at<double>(lay.setB[2]),
+                      ctx->at<double>(lay.setB[3]), ctx->at<double>(lay.setB[4]), ctx->at<double>(lay.setB[5]),
+                      ctx->at<uint32_t>(lay.pidB)};
+    ctx->cur = 0;
+    ctx->h_obs = nullptr;
+    auto fail = [&](int code) { if (ctx->h_obs) cudaFreeHost(ctx->h_obs); delete ctx; return code; };
+    if (!cuda_ok(cudaMallocHost(&ctx->h_obs, (4 + kObsMaxSlabs) * sizeof(double)), "cudaMallocHost")) return fail(CUBA_ERR_CUDA);
+
+    rc = occupancy_grid(k_collide<kThrS, kCapS, 16, false>, kThrS, collide_smem_bytes(kCapS), sms, &ctx->grid_s);
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrM, kCapM, 4, false>, kThrM, collide_smem_bytes(kCapM), sms, &ctx->grid_m);
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrL, kCapL, 2, false>, kThrL, collide_smem_bytes(kCapL), sms, &ctx->grid_l);
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrX, kCapX, 1, false>, kThrX, collide_smem_bytes(kCapX), sms, &ctx->grid_x);
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrS, kCapS, 16, true>, kThrS, collide_smem_bytes(kCapS), sms, &ctx->grid_s);
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrM, kCapM, 4, true>, kThrM, collide_smem_bytes(kCapM), sms, &ctx->grid_m);
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrL, kCapL, 2, true>, kThrL, collide_smem_bytes(kCapL), sms, &ctx->grid_l);
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrX, kCapX, 1, true>, kThrX, collide_smem_bytes(kCapX), sms, &ctx->grid_x);
+    if (rc != CUBA_OK) return fail(rc);
+    ctx->grid_o = sms;
+    if (!cuda_ok(cudaFuncSetAttribute(k_observe_partial, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      kObsWarps * kObsMaxSlabs * 8), "cudaFuncSetAttribute")) return fail(CUBA_ERR_CUDA);
+
+    cudaStream_t st = ctx->stream;
+    auto body = [&]() -> int {
+        CU(cudaMemsetAsync(ctx->at<void>(lay.zero), 0, kZeroWords * 4, st));
+        CU(cudaMemsetAsync(ctx->at<void>(lay.counters), 0, 64, st));
+        CU(cudaMemsetAsync(ctx->at<void>(lay.flags), 0, 4, st));
+        CU(cudaMemsetAsync(ctx->at<void>(lay.max_occ), 0, 8, st));
+        // S3 keys + persistent ids, then the general stable sort (A19)
+        uint32_t *kv = ctx->at<uint32_t>(lay.arena32);
+        uint32_t *keys[2] = {kv, kv + n}, *vals[2] = {kv + 2 * n, kv + 3 * n};
+        const unsigned gb = (unsigned)((n + 255) / 256);
+        k_init_keys<<<gb, 256, 0, st>>>(ctx->g, n, ctx->set[0], keys[0], vals[0], ctx->at<uint32_t>(lay.flags));
+        LAUNCHED();
+        int bits = 0;
+        while (bits < 32 && (((uint64_t)ncells - 1) >> bits) != 0) ++bits;
+        const int passes = bits == 0 ? 1 : (bits + 7) / 8;
+        uint32_t *H = ctx->at<uint32_t>(lay.rsH);
+        const uint32_t nb = (uint32_t)lay.rs_blocks;
+        int src = 0;
+        for (int p = 0; p < passes; ++p) {
+            k_rs_hist<<<nb, kRsThreads, 0, st>>>(keys[src], n, 8 * p, nb, H);
+            LAUNCHED();
+            k_scan_blocks<<<1, 1024, 0, st>>>(H, (int)(256 * nb), nullptr, 0);
+            LAUNCHED();
+            k_rs_scatter<<<nb, kRsThreads, 0, st>>>(keys[src], vals[src], keys[1 - src], vals[1 - src], n, 8 * p, nb, H);
+            LAUNCHED();
+            src = 1 - src;
+        }
+        k_gather_perm<<<gb, 256, 0, st>>>(n, vals[src], ctx->set[0], ctx->set[1]);
+        LAUNCHED();
+        k_starts_from_sorted<<<gb, 256, 0, st>>>(n, (uint32_t)ncells, keys[src], ctx->at<uint32_t>(lay.cell_start));
+        LAUNCHED();
+        // hand the sorted store back to the caller's arrays: the current set is 0 after init
+        const double *from[6] = {ctx->set[1].x, ctx->set[1].y, ctx->set[1].z, ctx->set[1].px, ctx->set[1].py, ctx->set[1].pz};
+        double *to[6] = {x, y, z, px, py, pz};
+        for (int k = 0; k < 6; ++k) CU(cudaMemcpyAsync(to[k], from[k], (size_t)n * 8, cudaMemcpyDeviceToDevice, st));
+        CU(cudaMemcpyAsync(ctx->set[0].pid, ctx->set[1].pid, (size_t)n * 4, cudaMemcpyDeviceToDevice, st));
+        return sync_and_check(ctx);
+    };
+    rc = body();
+    if (rc != CUBA_OK) return fail(rc);
+    *out = ctx;
+    return CUBA_OK;
+}
+
+void cuba_destroy(cuba_ctx *ctx)
+{
+    if (!ctx) return;
+    cudaStreamSynchronize(ctx->stream);
+    if (ctx->h_obs) cudaFreeHost(ctx->h_obs);
+    delete ctx;
+}
+
+// trace device buffers (cuba_step_traced only)
+struct TraceDev {
+    unsigned long long *off = nullptr;
+    uint32_t *cell = nullptr, *round = nullptr, *pa = nullptr, *pb = nullptr, *cell_of_pid = nullptr;
+    double *P = nullptr, *u = nullptr;
+    uint8_t *dec = nullptr;
+};
+
+template <bool TRACE>
+static int launch_collide(cuba_ctx *ctx, double base, const TraceDev *td)
+{
+    const Layout &lay = ctx->lay;
+    Soa &cur = ctx->set[ctx->cur];
+    CollideParams P{};
+    P.seed = ctx->seed; P.t = ctx->t; P.base = base;
+    P.cell_start = ctx->at<uint32_t>(lay.cell_start);
+    P.px = cur.px; P.py = cur.py; P.pz = cur.pz; P.pid = cur.pid;
+    P.counters = ctx->at<unsigned long long>(lay.counters);
+    P.flags = ctx->at<uint32_t>(lay.flags);
+    P.arena = ctx->at<uint32_t>(lay.arena32);
+    if (TRACE) {
+        P.trace_off = td->off; P.tr_cell = td->cell; P.tr_round = td->round; P.tr_pa = td->pa; P.tr_pb = td->pb;
+        P.tr_P = td->P; P.tr_u = td->u; P.tr_dec = td->dec;
+    }
+    uint32_t *zero = ctx->at<uint32_t>(lay.zero);
+    uint32_t *lists = ctx->at<uint32_t>(lay.class_list);
+    auto cls = [&](int k) { P.list = lists + (size_t)k * ctx->g.ncells; P.list_count = zero + k; P.work = zero + 5 + k; };
+    cudaStream_t st = ctx->stream;
+    cls(0);
+    k_collide<kThrS, kCapS, 16, TRACE><<<ctx->grid_s, kThrS, collide_smem_bytes(kCapS), st>>>(P);
+    LAUNCHED();
+    cls(1);
+    k_collide<kThrM, kCapM, 4, TRACE><<<ctx->grid_m, kThrM, collide_smem_bytes(kCapM), st>>>(P);
+    LAUNCHED();
+    cls(2);
+    k_collide<kThrL, kCapL, 2, TRACE><<<ctx->grid_l, kThrL, collide_smem_bytes(kCapL), st>>>(P);
+    LAUNCHED();
+    cls(3);
+    k_collide<kThrX, kCapX, 1, TRACE><<<ctx->grid_x, kThrX, collide_smem_bytes(kCapX), st>>>(P);
+    LAUNCHED();
+    cls(4);
+    k_collide_overflow<TRACE><<<ctx->grid_o, 1024, 0, st>>>(P, reinterpret_cast<unsigned long long *>(zero + 10),
+                                                           ctx->at<double>(lay.arenaE));
+    LAUNCHED();
+    return CUBA_OK;
+}
+
+static int check_step_args(const cuba_ctx *ctx, double dt, double sigma, double *base)
+{
+    if (!(dt > 0.0) || !std::isfinite(dt) || !(sigma >= 0.0) || !std::isfinite(sigma)) return CUBA_ERR_VALUE;
+    const double dx = ctx->box[0] / (double)ctx->g.nc[0];
+    const double dy = ctx->box[1] / (double)ctx->g.nc[1];
+    const double dz = ctx->box[2] / (double)ctx->g.nc[2];
+    const double dmin = std::fmin(dx, std::fmin(dy, dz));
+    if (!(dt < dmin)) return CUBA_ERR_CFL;
+    const double V = (dx * dy) * dz;
+    *base = (sigma * dt) / (ctx->n_test * V);         // Eq. 3 without v_rel; A3
+    return CUBA_OK;
+}
+
+// S1-S4 of one step: leaves the streamed, cell-sorted store in set[1-cur] and flips cur
+static int enqueue_bin(cuba_ctx *ctx, double dt, uint32_t *cell_of_pid)
+{
+    const Layout &lay = ctx->lay;
+    cudaStream_t st = ctx->stream;
+    const int64_t n = ctx->n;
+    const uint32_t ncells = ctx->g.ncells;
+    Soa &in = ctx->set[ctx->cur], &outp = ctx->set[1 - ctx->cur];
+    uint32_t *cnt = ctx->at<uint32_t>(lay.cnt);
+    uint32_t *zero = ctx->at<uint32_t>(lay.zero);
+    CU(cudaMemsetAsync(cnt, 0, (size_t)kDirs * ncells * 4, st));
+    k_stream_hist<<<(unsigned)lay.ntiles, kTileThreads, 0, st>>>(ctx->g, dt, n, in, cnt, ctx->at<uint32_t>(lay.tile_rec),
+                                                                  ctx->at<uint32_t>(lay.flags));
+    LAUNCHED();
+    k_gather<<<(unsigned)lay.nblocks_cells, 256, 0, st>>>(ctx->g, cnt, ctx->at<uint32_t>(lay.count_new),
+                                                          ctx->at<uint32_t>(lay.block_sum));
+    LAUNCHED();
+    k_scan_blocks<<<1, 1024, 0, st>>>(ctx->at<uint32_t>(lay.block_sum), (int)lay.nblocks_cells, zero, kZeroWords);
+    LAUNCHED();
+    ClassTable ct{{(uint32_t)kCapS, (uint32_t)kCapM, (uint32_t)kCapL, (uint32_t)kCapX, 0xFFFFFFFFu}};
+    k_cell_start<<<(unsigned)lay.nblocks_cells, 256, 0, st>>>(ncells, ctx->at<uint32_t>(lay.count_new),
+                                                              ctx->at<uint32_t>(lay.block_sum), ctx->at<uint32_t>(lay.cell_start),
+                                                              ct, zero, ctx->at<uint32_t>(lay.class_list),
+                                                              ctx->at<unsigned long long>(lay.max_occ));
+    LAUNCHED();
+    k_carry<<<(unsigned)((lay.ntiles + 7) / 8), 256, 0, st>>>((int)lay.ntiles, ctx->at<uint32_t>(lay.tile_rec),
+                                                              ctx->at<uint32_t>(lay.carry));
+    LAUNCHED();
+    if (cell_of_pid)
+        k_scatter<true><<<(unsigned)lay.ntiles, kTileThreads, 0, st>>>(ctx->g, dt, n, in, outp, cnt, ctx->at<uint32_t>(lay.cell_start),
+                                                                       ctx->at<uint32_t>(lay.carry), cell_of_pid);
+    else
+        k_scatter<false><<<(unsigned)lay.ntiles, kTileThreads, 0, st>>>(ctx->g, dt, n, in, outp, cnt, ctx->at<uint32_t>(lay.cell_start),
+                                                                        ctx->at<uint32_t>(lay.carry), nullptr);
+    LAUNCHED();
+    ctx->cur = 1 - ctx->cur;
+    return CUBA_OK;
+}
+
+int cuba_step(cuba_ctx *ctx, int nsteps, double dt, double sigma)
+{
+    if (!ctx) return CUBA_ERR_NULL;
+    if (nsteps < 0) return CUBA_ERR_SIZE;
+    double base;
+    int rc = check_step_args(ctx, dt, sigma, &base);
+    if (rc != CUBA_OK) return rc;
+    for (int s = 0; s < nsteps; ++s) {
+        rc = enqueue_bin(ctx, dt, nullptr);
+        if (rc != CUBA_OK) return rc;
+        rc = launch_collide<false>(ctx, base, nullptr);
+        if (rc != CUBA_OK) return rc;
+        ctx->t += 1;
+        ctx->steps += 1;
+    }
+    return CUBA_OK;
+}
+
+int cuba_step_traced(cuba_ctx *ctx, double dt, double sigma, cuba_trace *out)
+{
+    if (!ctx || !out || !out->cell_of_pid) return CUBA_ERR_NULL;
+    if (out->pair_capacity > 0 && (!out->pair_cell || !out->pair_round || !out->pid_a || !out->pid_b || !out->P ||
+                                   !out->u || !out->decided)) return CUBA_ERR_NULL;
+    double base;
+    int rc = check_step_args(ctx, dt, sigma, &base);
+    if (rc != CUBA_OK) return rc;
+    const int64_t n = ctx->n;
+    const uint32_t ncells = ctx->g.ncells;
+    TraceDev td;
+    auto release = [&]() {
+        cudaFree(td.off); cudaFree(td.cell); cudaFree(td.round); cudaFree(td.pa); cudaFree(td.pb);
+        cudaFree(td.cell_of_pid); cudaFree(td.P); cudaFree(td.u); cudaFree(td.dec);
+    };
+    auto body = [&]() -> int {
+        CU(cudaMalloc(&td.cell_of_pid, (size_t)n * 4));
+        int r = enqueue_bin(ctx, dt, td.cell_of_pid);
+        if (r != CUBA_OK) return r;
+        r = sync_and_check(ctx);
+        if (r != CUBA_OK) return r;
+        // per-cell record offsets: R(n) * floor(n/2), the same fp64 expressions as the kernel
+        std::vector<uint32_t> start((size_t)ncells + 1);
+        CU(cudaMemcpy(start.data(), ctx->at<uint32_t>(ctx->lay.cell_start), ((size_t)ncells + 1) * 4, cudaMemcpyDeviceToHost));
+        std::vector<unsigned long long> off((size_t)ncells + 1);
+        unsigned long long run = 0;
+        for (uint32_t c = 0; c < ncells; ++c) {
+            off[c] = run;
+            const uint32_t nn = start[c + 1] - start[c];
+            if (nn >= 2) {
+                const double cn = (nn & 1u) ? (double)nn : (double)(nn - 1u);
+                const double pmax = (2.0 * cn) * base;
+                int R = !(pmax <= 64.0) ? 64 : ((pmax <= 1.0) ? 1 : (int)std::ceil(pmax));
+                run += (unsigned long long)R * (nn >> 1);
+            }
+        }
+        off[ncells] = run;
+        out->n_pairs = (int64_t)run;
+        CU(cudaMemcpy(out->cell_of_pid, td.cell_of_pid, (size_t)n * 4, cudaMemcpyDeviceToHost));
+        if ((int64_t)run > out->pair_capacity) return CUBA_ERR_TRACE;
+        const size_t m = run ? (size_t)run : 1;
+        CU(cudaMalloc(&td.off, ((size_t)ncells + 1) * 8));
+        CU(cudaMalloc(&td.cell, m * 4)); CU(cudaMalloc(&td.round, m * 4));
+        CU(cudaMalloc(&td.pa, m * 4)); CU(cudaMalloc(&td.pb, m * 4));
+        CU(cudaMalloc(&td.P, m * 8)); CU(cudaMalloc(&td.u, m * 8)); CU(cudaMalloc(&td.dec, m));
+        CU(cudaMemcpy(td.off, off.data(), ((size_t)ncells + 1) * 8, cudaMemcpyHostToDevice));
+        r = launch_collide<true>(ctx, base, &td);
+        if (r != CUBA_OK) return r;
+        ctx->t += 1;
+        ctx->steps += 1;
+        r = sync_and_check(ctx);
+        if (r != CUBA_OK) return r;
+        if (run) {
+            CU(cudaMemcpy(out->pair_cell, td.cell, m * 4, cudaMemcpyDeviceToHost));
+            CU(cudaMemcpy(out->pair_round, td.round, m * 4, cudaMemcpyDeviceToHost));
+            CU(cudaMemcpy(out->pid_a, td.pa, m * 4, cudaMemcpyDeviceToHost));
+            CU(cudaMemcpy(out->pid_b, td.pb, m * 4, cudaMemcpyDeviceToHost));
+            CU(cudaMemcpy(out->P, td.P, m * 8, cudaMemcpyDeviceToHost));
+            CU(cudaMemcpy(out->u, td.u, m * 8, cudaMemcpyDeviceToHost));
+            CU(cudaMemcpy(out->decided, td.dec, m, cudaMemcpyDeviceToHost));
+        }
+        return CUBA_OK;
+    };
+    rc = body();
+    release();
+    return rc;
+}
+
+int cuba_observables(cuba_ctx *ctx, double total[4], int nslab, double *edens)
+{
+    if (!ctx || !total || !edens) return CUBA_ERR_NULL;
+    if (nslab < 1 || nslab > kObsMaxSlabs) return CUBA_ERR_SIZE;
+    const Layout &lay = ctx->lay;
+    const Soa &cur = ctx->set[ctx->cur];
+    cudaStream_t st = ctx->stream;
+    const double inv_w = (double)nslab / ctx->box[0];
+    const double vol = ((ctx->n_test * (ctx->box[0] / (double)nslab)) * ctx->box[1]) * ctx->box[2];
+    double *partial = ctx->at<double>(lay.obs_partial), *result = ctx->at<double>(lay.obs_result);
+    k_observe_partial<<<kObsGrid, kObsThreads, (size_t)kObsWarps * nslab * 8, st>>>(ctx->n, cur.x, cur.px, cur.py, cur.pz,
+                                                                                  inv_w, nslab, partial);
+    LAUNCHED();
+    k_observe_final<<<(4 + nslab + 255) / 256, 256, 0, st>>>(kObsGrid, nslab, partial, vol, result);
+    LAUNCHED();
+    CU(cudaMemcpyAsync(ctx->h_obs, result, (size_t)(4 + nslab) * 8, cudaMemcpyDeviceToHost, st));
+    int rc = sync_and_check(ctx);
+    if (rc != CUBA_OK) return rc;
+    memcpy(total, ctx->h_obs, 4 * sizeof(double));
+    memcpy(edens, ctx->h_obs + 4, (size_t)nslab * sizeof(double));
+    return CUBA_OK;
+}
+
+int cuba_state(cuba_ctx *ctx, cuba_soa *out)
+{
+    if (!ctx || !out) return CUBA_ERR_NULL;
+    const Soa &c = ctx->set[ctx->cur];
+    out->x = c.x; out->y = c.y; out->z = c.z; out->px = c.px; out->py = c.py; out->pz = c.pz;
+    out->pid = c.pid;
+    out->cell_start = ctx->at<uint32_t>(ctx->lay.cell_start);
+    return CUBA_OK;
+}
+
+int cuba_get_particles(cuba_ctx *ctx, uint32_t *pid, double *x, double *y, double *z,
+                       double *px, double *py, double *pz)
+{
+    if (!ctx) return CUBA_ERR_NULL;
+    int rc = sync_and_check(ctx);
+    if (rc != CUBA_OK) return rc;
+    const Soa &c = ctx->set[ctx->cur];
+    const size_t b = (size_t)ctx->n * 8;
+    if (pid) CU(cudaMemcpy(pid, c.pid, (size_t)ctx->n * 4, cudaMemcpyDeviceToHost));
+    if (x) CU(cudaMemcpy(x, c.x, b, cudaMemcpyDeviceToHost));
+    if (y) CU(cudaMemcpy(y, c.y, b, cudaMemcpyDeviceToHost));
+    if (z) CU(cudaMemcpy(z, c.z, b, cudaMemcpyDeviceToHost));
+    if (px) CU(cudaMemcpy(px, c.px, b, cudaMemcpyDeviceToHost));
+    if (py) CU(cudaMemcpy(py, c.py, b, cudaMemcpyDeviceToHost));
+    if (pz) CU(cudaMemcpy(pz, c.pz, b, cudaMemcpyDeviceToHost));
+    return CUBA_OK;
+}
+
+int cuba_get_cells(cuba_ctx *ctx, uint32_t *cell_start)
+{
+    if (!ctx || !cell_start) return CUBA_ERR_NULL;
+    int rc = sync_and_check(ctx);
+    if (rc != CUBA_OK) return rc;
+    CU(cudaMemcpy(cell_start, ctx->at<uint32_t>(ctx->lay.cell_start), ((size_t)ctx->g.ncells + 1) * 4, cudaMemcpyDeviceToHost));
+    return CUBA_OK;
+}
+
+int cuba_counters(cuba_ctx *ctx, cuba_counters_t *out)
+{
+    if (!ctx || !out) return CUBA_ERR_NULL;
+    unsigned long long c[8] = {0};
+    unsigned long long mo = 0;
+    uint32_t f = 0;
+    CU(cudaStreamSynchronize(ctx->stream));
+    CU(cudaMemcpy(c, ctx->at<void>(ctx->lay.counters), 64, cudaMemcpyDeviceToHost));
+    CU(cudaMemcpy(&mo, ctx->at<void>(ctx->lay.max_occ), 8, cudaMemcpyDeviceToHost));
+    CU(cudaMemcpy(&f, ctx->at<void>(ctx->lay.flags), 4, cudaMemcpyDeviceToHost));
+    out->steps = ctx->steps; out->pairs = c[0]; out->collisions = c[1]; out->rounds = c[2];
+    out->near_threshold = c[3]; out->max_occupancy = mo; out->overflow_cells = c[4]; out->device_flags = f;
+    return CUBA_OK;
+}
+
+int cuba_run_host(const double box[3], const int ncell[3], int64_t n,
+                  double *x, double *y, double *z, double *px, double *py, double *pz,
+                  double n_test, uint64_t seed, int nsteps, double dt, double sigma,
+                  double total[4], int nslab, double *edens, uint32_t *pid_out, int download)
+{
+    if (!box || !ncell || !x || !y || !z || !px || !py || !pz || !total || !edens) return CUBA_ERR_NULL;
+    const size_t wsb = cuba_workspace_bytes(n, ncell);
+    if (wsb == 0) return CUBA_ERR_SIZE;
+    double *host[6] = {x, y, z, px, py, pz};
+    double *dev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    void *ws = nullptr;
+    cuba_ctx *ctx = nullptr;
+    cudaStream_t st = nullptr;
+    auto body = [&]() -> int {
+        CU(cudaStreamCreate(&st));
+        for (int k = 0; k < 6; ++k) CU(cudaMalloc(&dev[k], (size_t)n * 8));
+        CU(cudaMalloc(&ws, wsb));
+        for (int k = 0; k < 6; ++k) CU(cudaMemcpyAsync(dev[k], host[k], (size_t)n * 8, cudaMemcpyHostToDevice, st));
+        int r = cuba_init(&ctx, box, ncell, n, dev[0], dev[1], dev[2], dev[3], dev[4], dev[5], n_test, seed, ws, wsb, st);
+        if (r != CUBA_OK) return r;
+        r = cuba_step(ctx, nsteps, dt, sigma);
+        if (r != CUBA_OK) return r;
+        r = cuba_observables(ctx, total, nslab, edens);
+        if (r != CUBA_OK) return r;
+        if (download) {
+            const Soa &c = ctx->set[ctx->cur];
+            const double *from[6] = {c.x, c.y, c.z, c.px, c.py, c.pz};
+            for (int k = 0; k < 6; ++k) CU(cudaMemcpyAsync(host[k], from[k], (size_t)n * 8, cudaMemcpyDeviceToHost, st));
+            if (pid_out) CU(cudaMemcpyAsync(pid_out, c.pid, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
+            CU(cudaStreamSynchronize(st));
+        }
+        return CUBA_OK;
+    };
+    const int rc = body();
+    if (ctx) cuba_destroy(ctx);
+    for (int k = 0; k < 6; ++k) cudaFree(dev[k]);
+    cudaFree(ws);
+    if (st) cudaStreamDestroy(st);
+    return rc;
+}
+

@@ -1,0 +1,122 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (`-m gpu`).
+The oracle cannot run 25M particles in seconds, so the check is on sampled outputs the
+oracle computes one by one, plus properties that hold at any size:
+  * streaming + reflection + cell index of sampled particles (oracle S1-S3) -- exact;
+  * the store is a cell-sorted permutation, stable w.r.t. the previous array order;
+  * whole hot cells re-collided by the oracle from the GPU's own post-binning momenta -- exact;
+  * energy conservation and pair/round counters against the cell counts."""
+import math
+
+import numpy as np
+import pytest
+
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def cuba():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_1208_0961_b200 as c
+    c.lib()
+    return c
+
+
+@pytest.mark.parametrize("config", [1, 2])
+def test_full_size_step_sampled_against_oracle(cuba, oracle_mod, config):
+    w = workloads.make(config)
+    g = cuba.Cuba.from_workload(w)
+    ncells = g.ncells
+    pid0, *s0 = g.particles()
+    start0 = g.cell_start()
+    tot0, _ = g.observables(64)
+    # ---- sigma = 0 step: S1-S4 only, so the oracle's S1-S3 apply particle by particle
+    g.step(1, w.dt, 0.0)
+    pid1, *s1 = g.particles()
+    start1 = g.cell_start()
+    (ox, oy, oz, opx, opy, opz), _ = oracle_mod.stream_reflect(*s0, w.dt, w.box)      # by previous slot
+    slot_prev = np.empty(w.n, dtype=np.int64)
+    slot_prev[pid0] = np.arange(w.n)
+    src = slot_prev[pid1]                                                            # previous slot of each new slot
+    for name, got, ref in zip("x y z px py pz".split(), s1, (ox, oy, oz, opx, opy, opz)):
+        assert np.array_equal(got, ref[src]), name
+    cell1 = oracle_mod.cell_index(s1[0], s1[1], s1[2], w.box, w.ncell)
+    assert np.all(np.diff(cell1.astype(np.int64)) >= 0)
+    assert np.array_equal(start1, np.searchsorted(cell1, np.arange(ncells + 1), side="left").astype(np.uint32))
+    same = cell1[1:] == cell1[:-1]
+    assert np.all(src[1:][same] > src[:-1][same])                                    # stable (A8)
+    assert np.array_equal(np.sort(pid1), np.arange(w.n, dtype=np.uint32))
+    # ---- one real step: re-collide sampled cells with the oracle from the GPU's binned state
+    g.step(1, w.dt, 0.0)              # bin once more so that "before" below is post-binning data
+    pidb, *sb = g.particles()
+    startb = g.cell_start()
+    t_index = g.counters().steps      # global step index of the next step
+    # a zero-dt-like probe is impossible (dt > 0), so the check uses a sub-box handed to the oracle:
+    # particles of one cell, placed in a 1-cell box, stepped with a dt small enough to keep them there
+    g.step(1, w.dt, w.sigma)
+    pida, *sa = g.particles()
+    starta = g.cell_start()
+    c2 = g.counters()
+    counts = np.diff(starta.astype(np.int64))
+    d = np.array(w.box) / np.array(w.ncell)
+    V = float(np.prod(d))
+    base = (w.sigma * w.dt) / (w.n_test * V)
+    cn = np.where(counts % 2 == 1, counts, counts - 1).astype(np.float64)
+    R = np.where(counts >= 2, np.maximum(1, np.ceil(2.0 * cn * base)), 0).astype(np.int64)
+    assert c2.rounds == int(R.sum())
+    assert c2.pairs == int((R * (counts // 2)).sum())
+    assert c2.max_occupancy >= counts.max() and c2.device_flags == 0 and c2.near_threshold == 0
+    # collisions happened at the closed-form rate sum_cells n(n-1)/2 * base (<v_rel> = 1 in each
+    # thermal half; the mixing layer is thin) within 1 %
+    expect = float((counts * (counts - 1) / 2.0).sum() * base)
+    assert c2.collisions == pytest.approx(expect, rel=0.01)
+    # energy conservation over the three steps
+    tot1, _ = g.observables(64)
+    assert abs(tot1[0] - tot0[0]) / tot0[0] < 1e-10
+    # sampled cells: the oracle collides the same particles (same pids, same seed, same t)
+    # when fed the post-binning momenta; positions there are irrelevant to S5
+    rng = np.random.default_rng(5)
+    slot_b = np.empty(w.n, dtype=np.int64)
+    slot_b[pidb] = np.arange(w.n)
+    hot = np.argsort(counts)[-3:]
+    sample = np.concatenate([hot, rng.integers(0, ncells, 12)])
+    for c in sample:
+        lo, hi = int(starta[c]), int(starta[c + 1])
+        if hi - lo < 2:
+            continue
+        ids = pida[lo:hi]
+        before = slot_b[ids]
+        got = np.stack([sa[3][lo:hi], sa[4][lo:hi], sa[5][lo:hi]])
+        # momenta before S5 of this step = post-binning momenta reflected by this step's walls:
+        # take them from a replay of S1-S2 on the "before" state
+        (rx, ry, rz, rpx, rpy, rpz), _ = oracle_mod.stream_reflect(*[a[before] for a in sb], w.dt, w.box)
+        ref = oracle_collide_cell(oracle_mod, w, ids, np.stack([rpx, rpy, rpz]), t_index, base)
+        assert np.array_equal(got, ref), "cell %d" % c
+
+
+def oracle_collide_cell(oracle_mod, w, ids, p, t, base):
+    """S5 of one cell done with the oracle's own pieces (shuffle_order, pair_kinematics, the
+    DEC uniform via philox + u53, direction, scatter), in the order of oracle/cuba_oracle.c."""
+    n = ids.shape[0]
+    cn = float(n if n % 2 else n - 1)
+    pmax = (2.0 * cn) * base
+    R = 1 if pmax <= 1.0 else int(math.ceil(pmax))
+    scale = (cn * base) / float(R)
+    p = p.copy()
+    index_of = {int(v): k for k, v in enumerate(ids)}
+    key = [w.seed & 0xFFFFFFFF, w.seed >> 32]
+    for rho in range(R):
+        order = oracle_mod.shuffle_order(w.seed, t, rho, ids)
+        for k in range(n // 2):
+            a, b = index_of[int(order[2 * k])], index_of[int(order[2 * k + 1])]
+            Ea, Eb, s, vrel = oracle_mod.pair_kinematics(p[:, a], p[:, b])
+            P = vrel * scale
+            wds = oracle_mod.philox4x32_10([int(ids[a]), t, rho, 1 << 16], key)
+            u = oracle_mod.u53(wds[0], wds[1])
+            if u < P:
+                nhat, _ = oracle_mod.direction(w.seed, int(ids[a]), t, rho)
+                qa, qb = oracle_mod.scatter(p[:, a], p[:, b], Ea, Eb, s, nhat)
+                p[:, a], p[:, b] = qa, qb
+    return p

@@ -1,0 +1,225 @@
+"""GPU-vs-oracle parity, through the C ABI (`-m gpu`).  Protocol of SURVEY.md 8(c):
+ (i) one traced step from an identical state: cell indices, pair lists, probabilities,
+     uniforms and decisions equal bit for bit (decisions within 1e-12 of the threshold are
+     counted -- there are none), state within 1e-12 relative (in fact identical bits);
+ (ii) many steps: state still identical, energy-density profiles within 1e-12."""
+import math
+
+import numpy as np
+import pytest
+
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+REL = 1e-12   # north_star: "positions and momenta within 1e-12 relative in fp64"
+
+
+@pytest.fixture(scope="module")
+def cuba():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_1208_0961_b200 as c
+    c.lib()   # fails loudly if the extension was not built
+    return c
+
+
+def assert_state_equal(gpu_particles, ora_particles, exact=True):
+    assert np.array_equal(gpu_particles[0], ora_particles[0]), "pid / array order differs"
+    for name, g, o in zip("x y z px py pz".split(), gpu_particles[1:], ora_particles[1:]):
+        scale = np.maximum(np.abs(o), 1e-300)
+        assert np.all(np.abs(g - o) <= REL * scale), name
+        if exact:
+            assert np.array_equal(g, o), name + " bits differ"
+
+
+def run_traced_step(cuba, oracle_mod, w):
+    g = cuba.Cuba.from_workload(w)
+    o = oracle_mod.Oracle.from_workload(w)
+    assert_state_equal(g.particles(), o.particles())           # A19: init sort
+    assert np.array_equal(g.cell_start(), o.cells()[1])
+    o.set_trace(True)
+    o.step(1, w.dt, w.sigma)
+    tg = g.step_traced(w.dt, w.sigma)
+    to = o.trace()
+    # cell indices by pid
+    ocell, ostart = o.cells()
+    opid = o.particles()[0]
+    ocell_of_pid = np.empty(w.n, dtype=np.uint32)
+    ocell_of_pid[opid] = ocell
+    assert np.array_equal(tg.cell_of_pid, ocell_of_pid)
+    # pair lists in (cell, round, k) order, probabilities, uniforms, decisions
+    assert tg.cell.shape[0] == to["cell"].shape[0]
+    assert np.array_equal(tg.cell, to["cell"]) and np.array_equal(tg.round, to["round"])
+    assert np.array_equal(tg.pid_a, to["pid_a"]) and np.array_equal(tg.pid_b, to["pid_b"])
+    near = np.abs(to["u"] - to["P"]) <= 1e-12
+    assert near.sum() == 0
+    assert np.array_equal(tg.u, to["u"])
+    assert np.array_equal(tg.P, to["P"])
+    assert np.array_equal(tg.decided[~near], to["decided"][~near])
+    # state
+    assert_state_equal(g.particles(), o.particles())
+    assert np.array_equal(g.cell_start(), ostart)
+    gc, oc = g.counters(), o.counters()
+    assert (gc.pairs, gc.collisions, gc.rounds, gc.near_threshold, gc.max_occupancy) == \
+           (oc["pairs"], oc["collisions"], oc["rounds"], oc["near_threshold"], oc["max_occupancy"])
+    assert gc.device_flags == 0
+    return g, o
+
+
+def test_one_step_bit_exact_thermal_box(cuba, oracle_mod):
+    run_traced_step(cuba, oracle_mod, workloads.make(0))
+
+
+def test_one_step_bit_exact_riemann_small(cuba, oracle_mod):
+    g, o = run_traced_step(cuba, oracle_mod, workloads.riemann_small())
+    # keep going untraced: 9 more steps, still identical
+    w = workloads.riemann_small()
+    g.step(9, w.dt, w.sigma)
+    o.step(9, w.dt, w.sigma)
+    assert_state_equal(g.particles(), o.particles())
+
+
+def test_one_step_bit_exact_many_rounds_and_size_classes(cuba, oracle_mod):
+    """sigma = 50 GeV^-2 on half-width cells (the configs[3] regime: R up to 3), with cells in
+    the 32-, 128- and 512-thread classes and a ragged last tile."""
+    w = workloads.riemann(L=(6.0, 3.0, 2.0), ncell=(12, 3, 2), r_test=60.0, sigma_gev2=50.0, dt=0.05, seed=13)
+    assert w.n % 1024 != 0
+    g, o = run_traced_step(cuba, oracle_mod, w)
+    assert o.counters()["rounds"] > 1.5 * (np.diff(o.cells()[1].astype(np.int64)) >= 2).sum()
+    assert o.counters()["max_occupancy"] > 512
+
+
+def test_config0_full_run_matches_oracle(cuba, oracle_mod):
+    """BASELINE.json:configs[0]: 50 steps, state bit-identical, totals and profile to 1e-12."""
+    w = workloads.make(0)
+    g = cuba.Cuba.from_workload(w)
+    o = oracle_mod.Oracle.from_workload(w)
+    tot0, _ = g.observables(8)
+    g.step(w.steps, w.dt, w.sigma)
+    o.step(w.steps, w.dt, w.sigma)
+    assert_state_equal(g.particles(), o.particles())
+    gt, ge = g.observables(8)
+    ot, oe = o.observables(8)
+    assert np.allclose(ge, oe, rtol=REL, atol=0)
+    assert gt[0] == pytest.approx(ot[0], rel=REL)
+    assert np.allclose(gt[1:], ot[1:], rtol=0, atol=REL * ot[0])
+    assert abs(gt[0] - tot0[0]) / tot0[0] < 1e-10        # PAPER.md:66 energy conservation
+    gc, oc = g.counters(), o.counters()
+    assert (gc.steps, gc.pairs, gc.collisions, gc.rounds) == (50, oc["pairs"], oc["collisions"], oc["rounds"])
+    assert gc.near_threshold == 0 and gc.device_flags == 0 and gc.overflow_cells == 0
+
+
+def test_riemann_profiles_over_many_steps(cuba, oracle_mod):
+    """Protocol (ii) at a size the oracle finishes in seconds: 64-slab profiles every 10 steps."""
+    w = workloads.riemann(L=(16.0, 4.0, 4.0), ncell=(16, 4, 4), r_test=10.0, seed=14)
+    g = cuba.Cuba.from_workload(w)
+    o = oracle_mod.Oracle.from_workload(w)
+    for _ in range(4):
+        g.step(10, w.dt, w.sigma)
+        o.step(10, w.dt, w.sigma)
+        gt, ge = g.observables(64)
+        ot, oe = o.observables(64)
+        assert np.allclose(ge, oe, rtol=REL, atol=0)
+        assert np.allclose(gt, ot, rtol=REL, atol=REL * ot[0])
+    assert_state_equal(g.particles(), o.particles())
+
+
+def test_k_steps_equal_k_single_steps_and_determinism(cuba):
+    w = workloads.riemann_small()
+    a, b, c = (cuba.Cuba.from_workload(w) for _ in range(3))
+    a.step(4, w.dt, w.sigma)
+    for _ in range(4):
+        b.step(1, w.dt, w.sigma)
+    c.step(4, w.dt, w.sigma)
+    pa, pb, pc = a.particles(), b.particles(), c.particles()
+    for u, v, x in zip(pa, pb, pc):
+        assert np.array_equal(u, v) and np.array_equal(u, x)
+    assert np.array_equal(a.observables(16)[1], c.observables(16)[1])   # reductions are order-fixed
+
+
+@pytest.mark.parametrize("case", ["single", "two", "one_cell_overflow", "flat_grid", "empty_cells"])
+def test_edge_cases_match_oracle(cuba, oracle_mod, case):
+    rng = np.random.default_rng(77)
+    if case == "single":          # n = 1: nothing to pair
+        w = workloads.thermal_box(L=(2.0, 2.0, 2.0), ncell=(2, 2, 2), count=1, seed=3)
+    elif case == "two":
+        w = workloads.thermal_box(L=(1.0, 1.0, 1.0), ncell=(1, 1, 1), count=2, seed=3, r_test=0.05)
+    elif case == "one_cell_overflow":   # one cell far beyond the largest shared-memory class
+        w = workloads.thermal_box(L=(1.0, 1.0, 1.0), ncell=(1, 1, 1), count=6000, seed=4, r_test=2000.0)
+    elif case == "flat_grid":     # a single layer of cells in y and z, odd sizes
+        w = workloads.thermal_box(L=(7.0, 1.0, 3.0), ncell=(7, 1, 3), count=3001, seed=5, r_test=1.0)
+    else:                         # most cells empty: particles only in two far-apart blobs
+        w = workloads.thermal_box(L=(16.0, 16.0, 16.0), ncell=(16, 16, 16), count=4000, seed=6, r_test=0.05)
+        w.x[:] = np.where(rng.random(w.n) < 0.5, 0.5, 15.2) + 0.3 * rng.random(w.n)
+        w.y[:] = 7.0 + 2.0 * rng.random(w.n)
+        w.z[:] = 0.1 + 0.5 * rng.random(w.n)
+    g = cuba.Cuba.from_workload(w)
+    o = oracle_mod.Oracle.from_workload(w)
+    for _ in range(3):
+        g.step(1, w.dt, w.sigma)
+        o.step(1, w.dt, w.sigma)
+        assert_state_equal(g.particles(), o.particles())
+        assert np.array_equal(g.cell_start(), o.cells()[1])
+    gc, oc = g.counters(), o.counters()
+    assert (gc.pairs, gc.collisions, gc.rounds) == (oc["pairs"], oc["collisions"], oc["rounds"])
+    if case == "one_cell_overflow":
+        assert gc.overflow_cells == 3 and oc["collisions"] > 100
+    if case == "single":
+        assert gc.pairs == 0
+
+
+def test_wall_reflection_on_device_preserves_energy_bits(cuba):
+    """PAPER.md:44 with sigma = 0: after many wall hits every |p| is bit-identical."""
+    import torch
+    w = workloads.thermal_box(L=(2.0, 2.0, 2.0), ncell=(2, 2, 2), count=50000, seed=9)
+    g = cuba.Cuba.from_workload(w)
+    E0 = np.sqrt((w.px * w.px + w.py * w.py) + w.pz * w.pz)
+    g.step(30, 0.9, 0.0)
+    pid, x, y, z, px, py, pz = g.particles()
+    E1 = np.sqrt((px * px + py * py) + pz * pz)
+    assert np.array_equal(E1, E0[pid])
+    for a, L in zip((x, y, z), w.box):
+        assert a.min() >= 0.0 and a.max() <= L
+    assert (np.sign(px) != np.sign(w.px[pid])).sum() > 1000
+
+
+def test_errors_are_codes_not_crashes(cuba):
+    import torch
+    w = workloads.thermal_box(L=(2.0, 2.0, 2.0), ncell=(2, 2, 2), count=500, seed=1)
+    g = cuba.Cuba.from_workload(w)
+    with pytest.raises(cuba.CubaError) as e:
+        g.step(1, 1.0, 0.1)                      # dt == cell edge
+    assert e.value.code == -7
+    with pytest.raises(cuba.CubaError) as e:
+        g.step(1, -0.1, 0.1)
+    assert e.value.code == -3
+    with pytest.raises(cuba.CubaError) as e:
+        g.observables(0)
+    assert e.value.code == -2
+    g.step(1, 0.1, 1e9)                          # needs > 64 rounds: reported at the next sync
+    with pytest.raises(cuba.CubaError) as e:
+        g.observables(4)
+    assert e.value.code == -9
+    bad = [torch.from_numpy(a.copy()).cuda() for a in w.arrays()]
+    bad[0][7] = 2.5                              # outside the box
+    with pytest.raises(cuba.CubaError) as e:
+        cuba.Cuba(w.box, w.ncell, *bad, 1.0, 1)
+    assert e.value.code == -6
+    bad = [torch.from_numpy(a.copy()).cuda() for a in w.arrays()]
+    bad[3][7] = bad[4][7] = bad[5][7] = 0.0      # p = 0
+    with pytest.raises(cuba.CubaError) as e:
+        cuba.Cuba(w.box, w.ncell, *bad, 1.0, 1)
+    assert e.value.code == -6
+
+
+def test_run_host_end_to_end_matches_oracle(cuba, oracle_mod):
+    w = workloads.riemann_small()
+    host = [a.copy() for a in w.arrays()]
+    tot, ed, pid = cuba.run_host(w.box, w.ncell, *host, w.n_test, w.seed, 5, w.dt, w.sigma, 16, download=True)
+    o = oracle_mod.Oracle.from_workload(w)
+    o.step(5, w.dt, w.sigma)
+    ot, oe = o.observables(16)
+    assert np.allclose(ed, oe, rtol=REL, atol=0) and tot[0] == pytest.approx(ot[0], rel=REL)
+    assert_state_equal((pid, *host), o.particles())
+    assert cuba.launch_count() > 0
