@@ -1,0 +1,329 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the CuBA hot path on B200 (one JSON line).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl cuba|reference]
+
+A "step" is one pass of the whole hot path (S1-S5: stream, reflect, bin, pair, collide)
+over the full particle store of BASELINE.json:configs[C] (default C = 2, the ~25M-particle
+Riemann problem north_star's target is quoted on).  `value` = particle-updates/s =
+N * K / t with the state resident in HBM; t from CUDA events on the launching stream,
+max over ranks.  The state (1.3 GB per copy) is far larger than the 126 MB L2, so no
+flush is needed between steps.  N > 1 GPUs run N independent replicas (different seeds),
+no collective on the data path ("replicas only", scaling "weak").
+
+`--impl reference` times the CPU oracle, as it stands, on a bounded sample of the same
+workload (a transverse slice of the box: same densities, cells, dt, sigma).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402
+
+METRIC = "particle_updates_per_s"
+UNIT = "particle-updates/s"
+
+# algorithmic HBM bytes per particle-step of each kernel
+BYTES_STREAM_HIST = 48      # reads x,y,z,px,py,pz
+BYTES_SCATTER = 104         # reads 6 fp64 + pid, writes 6 fp64 + pid
+BYTES_COLLIDE = 52          # reads px,py,pz,pid, writes px,py,pz (cells with n >= 2)
+BYTES_STEP = BYTES_STREAM_HIST + BYTES_SCATTER + BYTES_COLLIDE   # 204, SURVEY.md 8(d)
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML every 10 ms while armed."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.armed, self.stop_flag = index, [], False, False
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception as e:  # pragma: no cover
+            self.err = repr(e)
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        while not self.stop_flag:
+            if self.armed:
+                try:
+                    mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                    reasons = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h) if hasattr(
+                        nv, "nvmlDeviceGetCurrentClocksEventReasons") else nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                    self.samples.append((mhz, int(reasons)))
+                except Exception:
+                    pass
+            time.sleep(0.01)
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": getattr(self, "max_mhz", None), "reasons": ["unsampled"]}
+        names = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+                 0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+                 0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+        bits = 0
+        for _, r in self.samples:
+            bits |= r
+        reasons = [n for b, n in names.items() if bits & b and n != "gpu_idle"]
+        return {"sm_mhz": float(np.median([m for m, _ in self.samples])), "sm_max_mhz": float(self.max_mhz),
+                "reasons": reasons, "samples": len(self.samples)}
+
+
+def oracle_sample_workload(config):
+    """The bounded sample of configs[config] the CPU oracle is timed on: same densities,
+    cell size, dt and sigma, a quarter of the transverse extent in y and z."""
+    if config in (1, 2):
+        r = 10.0 if config == 1 else 100.0
+        w = workloads.riemann(L=(32.0, 8.0, 8.0), ncell=(32, 8, 8), r_test=r, seed=config + 1)
+        return w, "configs[%d] restricted to a 32x8x8 fm^3 transverse slice (same T, r_test, cells, dt, sigma)" % config
+    if config == 3:
+        w = workloads.riemann(L=(32.0, 8.0, 8.0), ncell=(64, 8, 8), r_test=40.0, sigma_gev2=50.0, dt=0.05, seed=4)
+        return w, "configs[3] restricted to a 32x8x8 fm^3 transverse slice"
+    if config == 4:
+        w = workloads.skewed(L=(64.0, 8.0, 8.0), ncell=(64, 8, 8), r_test=100.0, seed=5)
+        return w, "configs[4] restricted to a 64x8x8 fm^3 transverse slice"
+    w = workloads.make(0)
+    return w, "configs[0] whole"
+
+
+def time_oracle(w, steps, warmup):
+    import oracle
+    o = oracle.Oracle.from_workload(w)
+    if warmup:
+        o.step(warmup, w.dt, w.sigma)
+    t0 = time.perf_counter()
+    o.step(steps, w.dt, w.sigma)
+    dt = time.perf_counter() - t0
+    c = o.counters()
+    o.close()
+    return dt, c
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the CPU oracle as it stands, host cores, rank 0 only."""
+    if rank != 0:
+        return
+    w, sample = oracle_sample_workload(args.config)
+    dt, c = time_oracle(w, args.steps, args.warmup)
+    value = w.n * args.steps / dt
+    full = workloads_name(args.config)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": full, "sample": sample, "n_particles": w.n},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workloads_name(config):
+    return {0: "configs[0] thermal box 8^3 fm^3, r_test=2 (13.8k particles)",
+            1: "configs[1] Riemann 32^3 fm^3, r_test=10 (2.49M particles)",
+            2: "configs[2] Riemann 32^3 fm^3, T=0.4/0.2 GeV, r_test=100 (24.9M particles), sigma=10 GeV^-2, dt=0.1 fm/c",
+            3: "configs[3] Riemann fine cells 0.5x1x1 fm, r_test=40 (9.96M particles), sigma=50 GeV^-2, dt=0.05",
+            4: "configs[4] skewed occupancy 64x32x32 fm^3, r_test=100 (53.9M particles)"}[config]
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json:configs")
+    ap.add_argument("--impl", default="cuba", choices=["cuba", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "cuba" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_1208_0961_b200 as cuba
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+    cuba.lib()
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- workload: replica `rank` of configs[C] (independent seed per rank) -------------
+    w = workloads.CONFIGS[args.config]()
+    if rank:
+        w.seed = w.seed + 1000 * rank
+    host = [torch.from_numpy(a).pin_memory() for a in w.arrays()]
+    sim = cuba.Cuba(w.box, w.ncell, *[h.to(dev) for h in host], w.n_test, w.seed)
+    n = w.n
+
+    sampler = ClockSampler(local)
+    sampler.start()
+
+    # ---- warm-up, then the timed region: K steps, CUDA events on the launching stream ---
+    sim.step(args.warmup, w.dt, w.sigma)
+    barrier()
+    c0 = sim.counters()
+    l0 = cuba.launch_count()
+    sim.profile_enable(True)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.armed = True
+    ev0.record()
+    sim.step(args.steps, w.dt, w.sigma)
+    ev1.record()
+    barrier()
+    sampler.armed = False
+    ms = ev0.elapsed_time(ev1)
+    launches = cuba.launch_count() - l0
+    prof = sim.profile_read()
+    sim.profile_enable(False)
+    c1 = sim.counters()
+    pairs = c1.pairs - c0.pairs
+    if c1.device_flags:
+        raise SystemExit("device error flags %d" % c1.device_flags)
+
+    # particles each collide class handled in the last step (for per-launch algorithmic bytes)
+    counts = np.diff(sim.cell_start().astype(np.int64))
+    caps = [64, 512, 2048, 4544]
+    cls = np.searchsorted(caps, counts, side="left")
+    class_particles = [int(counts[(cls == k) & (counts >= 2)].sum()) for k in range(5)]
+
+    # ---- observables timed separately --------------------------------------------------
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    tot, ed = sim.observables(w.nslab)
+    obs_ms = 1e3 * (time.perf_counter() - t0)
+
+    # ---- end to end through the C ABI with HOST buffers --------------------------------
+    e2e = None
+    if not args.no_e2e:
+        e2e_steps = args.steps
+        harr = [h.numpy() for h in host]
+        cuba.run_host(w.box, w.ncell, *harr, w.n_test, w.seed, 1, w.dt, w.sigma, w.nslab)   # warm the allocator
+        barrier()
+        t0 = time.perf_counter()
+        cuba.run_host(w.box, w.ncell, *harr, w.n_test, w.seed, e2e_steps, w.dt, w.sigma, w.nslab)
+        torch.cuda.synchronize()
+        e2e_s = time.perf_counter() - t0
+        e2e = {"s": e2e_s, "steps": e2e_steps}
+    sim.close()
+
+    # ---- reduce over ranks: max time, summed work --------------------------------------
+    if world > 1:
+        t = torch.tensor([ms, e2e["s"] if e2e else 0.0], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t[0])
+        if e2e:
+            e2e["s"] = float(t[1])
+        s = torch.tensor([float(n), float(pairs), float(launches)], device=dev, dtype=torch.float64)
+        dist.all_reduce(s, op=dist.ReduceOp.SUM)
+        n_total, pairs_total, launches = float(s[0]), float(s[1]), int(s[2])
+    else:
+        n_total, pairs_total = float(n), float(pairs)
+    sampler.stop_flag = True
+
+    if rank == 0:
+        peak, peak_src = peaks()
+        sec = ms * 1e-3
+        value = n_total * args.steps / sec
+        # dominant kernel by measured device time
+        per_kernel = {k: {"ms_per_launch": (v[0] / v[1]) if v[1] else 0.0, "launches": v[1], "ms_total": v[0]}
+                      for k, v in prof.items()}
+        alg = {"k_stream_hist": BYTES_STREAM_HIST * n, "k_scatter": BYTES_SCATTER * n,
+               "k_collide<32>": BYTES_COLLIDE * class_particles[0], "k_collide<128>": BYTES_COLLIDE * class_particles[1],
+               "k_collide<512>": BYTES_COLLIDE * class_particles[2], "k_collide<1024>": BYTES_COLLIDE * class_particles[3],
+               "k_collide_overflow": BYTES_COLLIDE * class_particles[4]}
+        dom = max(per_kernel, key=lambda k: per_kernel[k]["ms_total"])
+        dom_ms = per_kernel[dom]["ms_per_launch"]
+        achieved = alg.get(dom, 0) / (dom_ms * 1e-3) / 1e9 if dom_ms else 0.0
+        kernels = {}
+        for k, v in per_kernel.items():
+            if v["launches"]:
+                gbs = alg.get(k, 0) / (v["ms_per_launch"] * 1e-3) / 1e9 if v["ms_per_launch"] else 0.0
+                kernels[k] = {"ms_per_launch": round(v["ms_per_launch"], 5), "share": round(v["ms_total"] / ms, 4),
+                              "alg_GBps": round(gbs, 1), "frac": round(gbs / peak, 4)}
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workloads_name(args.config), "n_particles": n, "ncells": sim.ncells,
+                       "l2": "inputs larger than L2 (%.2f GB state per copy vs 126 MB L2), no flush" % (52 * n / 1e9)
+                       if 52 * n > 4 * 126e6 else "state comparable to L2: cache-resident, not a roofline config",
+                       "parallelism": "replicas x%d" % world if world > 1 else "single GPU"},
+            "pair_evals_per_s": pairs_total / sec,
+            "pairs_per_step": pairs_total / args.steps,
+            "observables_ms": obs_ms,
+            "gpu_launches": int(launches),
+            "clocks": sampler.summary(),
+            "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                         "alg_bytes_per_launch": alg.get(dom, 0),
+                         "step": {"alg_bytes_per_particle": BYTES_STEP, "achieved": BYTES_STEP * value / world / 1e9,
+                                  "frac": BYTES_STEP * value / world / 1e9 / peak, "frac_of_8TBps_nominal": BYTES_STEP * value / world / 8e12},
+                         "kernels": kernels},
+        }
+        if e2e:
+            line["e2e"] = {"value": n_total * e2e["steps"] / e2e["s"], "unit": UNIT,
+                           "h2d_bytes_per_step": 48 * n / e2e["steps"], "d2h_bytes_per_step": 8 * (4 + w.nslab) / e2e["steps"],
+                           "call": "cuba_run_host: pinned HOST arrays -> H2D -> cuba_init -> cuba_step(%d) -> cuba_observables -> D2H"
+                                   % e2e["steps"], "seconds": e2e["s"]}
+        if not args.no_cpu_baseline:
+            ow, sample = oracle_sample_workload(args.config)
+            osteps = max(2, min(10, int(12e6 // max(ow.n, 1)) + 1))
+            odt, oc = time_oracle(ow, osteps, 0)
+            line["cpu_baseline"] = {"value": ow.n * osteps / odt, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                    "sample": "%s, N=%d, %d steps, %.1f s" % (sample, ow.n, osteps, odt),
+                                    "host_cores_available": os.cpu_count()}
+        line["paper_context"] = ("CuBA 58.09 s vs BAMPS 756 s (~13x), GPU and CPU models not named in the paper "
+                                 "(Fermi-era CUDA 4.1), run size not stated (PAPER.md:92)")
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -144,6 +144,17 @@ int cuba_run_host(const double box[3], const int ncell[3], int64_t n,
                   double n_test, uint64_t seed, int nsteps, double dt, double sigma,
                   double total[4], int nslab, double *edens, uint32_t *pid_out, int download);
 
+/* Per-kernel timing for the roofline report.  cuba_profile_enable(ctx, 1) makes cuba_step
+ * record a CUDA event on the context's stream after every kernel it launches (host cost
+ * ~1 us per event, no device-side serialisation beyond the stream's own order);
+ * cuba_profile_read synchronises and returns, for each of the CUBA_PROFILE_GROUPS kernel
+ * groups, the summed device time in milliseconds and the number of launches since the last
+ * enable, then clears the log.  HOST outputs of CUBA_PROFILE_GROUPS entries each. */
+#define CUBA_PROFILE_GROUPS 12
+int cuba_profile_enable(cuba_ctx *ctx, int on);
+int cuba_profile_read(cuba_ctx *ctx, double *ms_sum, uint64_t *launches);
+const char *cuba_profile_name(int group);
+
 void cuba_destroy(cuba_ctx *ctx);
 const char *cuba_strerror(int code);
 /* Text of the last CUDA runtime error seen by this library in the calling process. */

@@ -13,7 +13,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 # every symbol include/cuba.h declares
 EXPORTS = ("cuba_workspace_bytes", "cuba_init", "cuba_step", "cuba_observables", "cuba_state",
            "cuba_get_particles", "cuba_get_cells", "cuba_step_traced", "cuba_counters", "cuba_run_host", "cuba_destroy",
-           "cuba_strerror", "cuba_last_cuda_error", "cuba_launch_count")
+           "cuba_strerror", "cuba_last_cuda_error", "cuba_launch_count", "cuba_profile_enable",
+           "cuba_profile_read", "cuba_profile_name")
 
 
 class CubaError(RuntimeError):
@@ -100,6 +101,10 @@ def lib():
         L.cuba_strerror.restype = c_char_p
         L.cuba_last_cuda_error.restype = c_char_p
         L.cuba_launch_count.restype = c_uint64
+        L.cuba_profile_enable.argtypes = [c_void_p, c_int]
+        L.cuba_profile_read.argtypes = [c_void_p, dp, POINTER(c_uint64)]
+        L.cuba_profile_name.argtypes = [c_int]
+        L.cuba_profile_name.restype = c_char_p
         _lib = L
     return _lib
 
@@ -227,6 +232,17 @@ class Cuba:
         _check(lib().cuba_step_traced(self._h, float(dt), float(sigma), ctypes.byref(tr)))
         m = int(tr.n_pairs)
         return Trace(cell_of_pid, cell[:m], rnd[:m], pa[:m], pb[:m], P[:m], u[:m], dec[:m])
+
+    def profile_enable(self, on=True):
+        _check(lib().cuba_profile_enable(self._h, int(bool(on))))
+
+    def profile_read(self):
+        """{kernel group: (summed device ms, launches)} since profile_enable."""
+        G = 12
+        ms = (c_double * G)()
+        cnt = (c_uint64 * G)()
+        _check(lib().cuba_profile_read(self._h, ms, cnt))
+        return {lib().cuba_profile_name(g).decode(): (float(ms[g]), int(cnt[g])) for g in range(G)}
 
     def counters(self) -> Counters:
         c = _Counters()

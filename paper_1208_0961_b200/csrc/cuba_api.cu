@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <utility>
 #include <vector>
 
 #include "bin.cuh"
@@ -97,6 +98,9 @@ struct cuba_ctx {
     int cur;
     int grid_s, grid_m, grid_l, grid_x, grid_o;
     double *h_obs;       // pinned staging for observables
+    bool prof_on = false;
+    std::vector<cudaEvent_t> prof_pool;          // reused events
+    std::vector<std::pair<cudaEvent_t, int>> prof_log;   // (event, group) in stream order; group -1 = step start
     template <typename T> T *at(size_t off) const { return reinterpret_cast<T *>(ws + off); }
 };
 
@@ -156,6 +160,20 @@ static int sync_and_check(cuba_ctx *ctx)
     CU(cudaMemcpyAsync(&f, ctx->at<uint32_t>(ctx->lay.flags), 4, cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     return device_flags_to_error(f);
+}
+
+enum { G_MEMSET = 0, G_STREAM_HIST, G_GATHER, G_SCAN, G_CELL_START, G_CARRY, G_SCATTER,
+       G_COLLIDE_S, G_COLLIDE_M, G_COLLIDE_L, G_COLLIDE_X, G_COLLIDE_O };
+static_assert(G_COLLIDE_O + 1 == CUBA_PROFILE_GROUPS, "profile groups");
+
+static void prof_mark(cuba_ctx *ctx, int group)
+{
+    if (!ctx->prof_on) return;
+    cudaEvent_t e;
+    if (ctx->prof_pool.empty()) { if (cudaEventCreate(&e) != cudaSuccess) return; }
+    else { e = ctx->prof_pool.back(); ctx->prof_pool.pop_back(); }
+    cudaEventRecord(e, ctx->stream);
+    ctx->prof_log.emplace_back(e, group);
 }
 
 template <typename K>
@@ -273,6 +291,8 @@ void cuba_destroy(cuba_ctx *ctx)
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
     if (ctx->h_obs) cudaFreeHost(ctx->h_obs);
+    for (auto &pe : ctx->prof_log) cudaEventDestroy(pe.first);
+    for (auto e : ctx->prof_pool) cudaEventDestroy(e);
     delete ctx;
 }
 
@@ -307,19 +327,24 @@ static int launch_collide(cuba_ctx *ctx, double base, const TraceDev *td)
     cls(0);
     k_collide<kThrS, kCapS, 16, TRACE><<<ctx->grid_s, kThrS, collide_smem_bytes(kCapS), st>>>(P);
     LAUNCHED();
+    prof_mark(ctx, G_COLLIDE_S);
     cls(1);
     k_collide<kThrM, kCapM, 4, TRACE><<<ctx->grid_m, kThrM, collide_smem_bytes(kCapM), st>>>(P);
     LAUNCHED();
+    prof_mark(ctx, G_COLLIDE_M);
     cls(2);
     k_collide<kThrL, kCapL, 2, TRACE><<<ctx->grid_l, kThrL, collide_smem_bytes(kCapL), st>>>(P);
     LAUNCHED();
+    prof_mark(ctx, G_COLLIDE_L);
     cls(3);
     k_collide<kThrX, kCapX, 1, TRACE><<<ctx->grid_x, kThrX, collide_smem_bytes(kCapX), st>>>(P);
     LAUNCHED();
+    prof_mark(ctx, G_COLLIDE_X);
     cls(4);
     k_collide_overflow<TRACE><<<ctx->grid_o, 1024, 0, st>>>(P, reinterpret_cast<unsigned long long *>(zero + 10),
                                                            ctx->at<double>(lay.arenaE));
     LAUNCHED();
+    prof_mark(ctx, G_COLLIDE_O);
     return CUBA_OK;
 }
 
@@ -346,24 +371,31 @@ static int enqueue_bin(cuba_ctx *ctx, double dt, uint32_t *cell_of_pid)
     Soa &in = ctx->set[ctx->cur], &outp = ctx->set[1 - ctx->cur];
     uint32_t *cnt = ctx->at<uint32_t>(lay.cnt);
     uint32_t *zero = ctx->at<uint32_t>(lay.zero);
+    prof_mark(ctx, -1);
     CU(cudaMemsetAsync(cnt, 0, (size_t)kDirs * ncells * 4, st));
+    prof_mark(ctx, G_MEMSET);
     k_stream_hist<<<(unsigned)lay.ntiles, kTileThreads, 0, st>>>(ctx->g, dt, n, in, cnt, ctx->at<uint32_t>(lay.tile_rec),
                                                                   ctx->at<uint32_t>(lay.flags));
     LAUNCHED();
+    prof_mark(ctx, G_STREAM_HIST);
     k_gather<<<(unsigned)lay.nblocks_cells, 256, 0, st>>>(ctx->g, cnt, ctx->at<uint32_t>(lay.count_new),
                                                           ctx->at<uint32_t>(lay.block_sum));
     LAUNCHED();
+    prof_mark(ctx, G_GATHER);
     k_scan_blocks<<<1, 1024, 0, st>>>(ctx->at<uint32_t>(lay.block_sum), (int)lay.nblocks_cells, zero, kZeroWords);
     LAUNCHED();
+    prof_mark(ctx, G_SCAN);
     ClassTable ct{{(uint32_t)kCapS, (uint32_t)kCapM, (uint32_t)kCapL, (uint32_t)kCapX, 0xFFFFFFFFu}};
     k_cell_start<<<(unsigned)lay.nblocks_cells, 256, 0, st>>>(ncells, ctx->at<uint32_t>(lay.count_new),
                                                               ctx->at<uint32_t>(lay.block_sum), ctx->at<uint32_t>(lay.cell_start),
                                                               ct, zero, ctx->at<uint32_t>(lay.class_list),
                                                               ctx->at<unsigned long long>(lay.max_occ));
     LAUNCHED();
+    prof_mark(ctx, G_CELL_START);
     k_carry<<<(unsigned)((lay.ntiles + 7) / 8), 256, 0, st>>>((int)lay.ntiles, ctx->at<uint32_t>(lay.tile_rec),
                                                               ctx->at<uint32_t>(lay.carry));
     LAUNCHED();
+    prof_mark(ctx, G_CARRY);
     if (cell_of_pid)
         k_scatter<true><<<(unsigned)lay.ntiles, kTileThreads, 0, st>>>(ctx->g, dt, n, in, outp, cnt, ctx->at<uint32_t>(lay.cell_start),
                                                                        ctx->at<uint32_t>(lay.carry), cell_of_pid);
@@ -371,6 +403,7 @@ static int enqueue_bin(cuba_ctx *ctx, double dt, uint32_t *cell_of_pid)
         k_scatter<false><<<(unsigned)lay.ntiles, kTileThreads, 0, st>>>(ctx->g, dt, n, in, outp, cnt, ctx->at<uint32_t>(lay.cell_start),
                                                                         ctx->at<uint32_t>(lay.carry), nullptr);
     LAUNCHED();
+    prof_mark(ctx, G_SCATTER);
     ctx->cur = 1 - ctx->cur;
     return CUBA_OK;
 }
@@ -509,6 +542,42 @@ int cuba_get_particles(cuba_ctx *ctx, uint32_t *pid, double *x, double *y, doubl
     if (px) CU(cudaMemcpy(px, c.px, b, cudaMemcpyDeviceToHost));
     if (py) CU(cudaMemcpy(py, c.py, b, cudaMemcpyDeviceToHost));
     if (pz) CU(cudaMemcpy(pz, c.pz, b, cudaMemcpyDeviceToHost));
+    return CUBA_OK;
+}
+
+const char *cuba_profile_name(int group)
+{
+    static const char *names[CUBA_PROFILE_GROUPS] = {
+        "memset_cnt", "k_stream_hist", "k_gather", "k_scan_blocks", "k_cell_start", "k_carry", "k_scatter",
+        "k_collide<32>", "k_collide<128>", "k_collide<512>", "k_collide<1024>", "k_collide_overflow"};
+    return (group >= 0 && group < CUBA_PROFILE_GROUPS) ? names[group] : "?";
+}
+
+int cuba_profile_enable(cuba_ctx *ctx, int on)
+{
+    if (!ctx) return CUBA_ERR_NULL;
+    CU(cudaStreamSynchronize(ctx->stream));
+    for (auto &pe : ctx->prof_log) ctx->prof_pool.push_back(pe.first);
+    ctx->prof_log.clear();
+    ctx->prof_on = on != 0;
+    return CUBA_OK;
+}
+
+int cuba_profile_read(cuba_ctx *ctx, double *ms_sum, uint64_t *launches)
+{
+    if (!ctx || !ms_sum || !launches) return CUBA_ERR_NULL;
+    CU(cudaStreamSynchronize(ctx->stream));
+    for (int g = 0; g < CUBA_PROFILE_GROUPS; ++g) { ms_sum[g] = 0.0; launches[g] = 0; }
+    for (size_t i = 1; i < ctx->prof_log.size(); ++i) {
+        const int g = ctx->prof_log[i].second;
+        if (g < 0) continue;                          // a step-start marker closes nothing
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, ctx->prof_log[i - 1].first, ctx->prof_log[i].first));
+        ms_sum[g] += (double)ms;
+        launches[g] += 1;
+    }
+    for (auto &pe : ctx->prof_log) ctx->prof_pool.push_back(pe.first);
+    ctx->prof_log.clear();
     return CUBA_OK;
 }
 

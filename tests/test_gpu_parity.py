@@ -82,8 +82,8 @@ def test_one_step_bit_exact_riemann_small(cuba, oracle_mod):
 
 def test_one_step_bit_exact_many_rounds_and_size_classes(cuba, oracle_mod):
     """sigma = 50 GeV^-2 on half-width cells (the configs[3] regime: R up to 3), with cells in
-    the 32-, 128- and 512-thread classes and a ragged last tile."""
-    w = workloads.riemann(L=(6.0, 3.0, 2.0), ncell=(12, 3, 2), r_test=60.0, sigma_gev2=50.0, dt=0.05, seed=13)
+    the 32- and 512-thread classes (riemann_small covers the 128-thread one) and a ragged last tile."""
+    w = workloads.riemann(L=(6.0, 3.0, 2.0), ncell=(12, 3, 2), r_test=90.0, sigma_gev2=50.0, dt=0.05, seed=13)
     assert w.n % 1024 != 0
     g, o = run_traced_step(cuba, oracle_mod, w)
     assert o.counters()["rounds"] > 1.5 * (np.diff(o.cells()[1].astype(np.int64)) >= 2).sum()
@@ -150,7 +150,7 @@ def test_edge_cases_match_oracle(cuba, oracle_mod, case):
     elif case == "flat_grid":     # a single layer of cells in y and z, odd sizes
         w = workloads.thermal_box(L=(7.0, 1.0, 3.0), ncell=(7, 1, 3), count=3001, seed=5, r_test=1.0)
     else:                         # most cells empty: particles only in two far-apart blobs
-        w = workloads.thermal_box(L=(16.0, 16.0, 16.0), ncell=(16, 16, 16), count=4000, seed=6, r_test=0.05)
+        w = workloads.thermal_box(L=(16.0, 16.0, 16.0), ncell=(16, 16, 16), count=4000, seed=6, r_test=2.0)
         w.x[:] = np.where(rng.random(w.n) < 0.5, 0.5, 15.2) + 0.3 * rng.random(w.n)
         w.y[:] = 7.0 + 2.0 * rng.random(w.n)
         w.z[:] = 0.1 + 0.5 * rng.random(w.n)
