@@ -92,7 +92,7 @@ typedef struct cuba_trace {
 size_t cuba_workspace_bytes(int64_t n, const int ncell[3]);
 
 /* Adopt a particle store.  PAPER.md:32 (cells, per-particle r and p), PAPER.md:44 (box with
- * six walls at 0 and L; N_test).  x..pz are DEVICE arrays of n doubles, adopted in place and
+ * six walls at 0 and L; N_test).  x..pz are DEVICE arrays of n doubles (16-byte aligned), adopted in place and
  * to be kept alive (with `workspace`) until cuba_destroy.  Assigns pid[i] = i, validates the
  * state on the device (CUBA_ERR_STATE), and bins the initial positions with S3+S4 so that
  * the store is cell-sorted from the start (A19); on return the caller's arrays

@@ -45,56 +45,118 @@ __device__ __forceinline__ Moved move_particle(const Geom &g, double dt, double 
     return m;
 }
 
+// ---- tile staging shared by K_A and K_C -----------------------------------------------------
+// Persistent CTAs walk the tiles blockIdx.x, blockIdx.x + gridDim.x, ...  Each tile's arrays
+// are contiguous 4 KB (fp64) / 2 KB (pid) chunks, fetched with cp.async.bulk (TMA bulk copy)
+// into one of two shared-memory stages and signalled on an mbarrier, so a whole tile of the
+// next iteration is in flight while the current one is computed -- no registers are tied up
+// by loads, which is what bounded the first version (ncu: long-scoreboard stalls at 24-36 %
+// occupancy, profiles/r01_*).  The last, partial tile is loaded with plain loads.
+template <int NARR>   // 6: x,y,z,px,py,pz   7: + pid
+struct alignas(128) TileStage {
+    double v[6][kTile];
+    uint32_t pid[NARR == 7 ? kTile : 1];
+};
+
+template <int NARR>
+__device__ __forceinline__ void stage_issue(TileStage<NARR> &st, uint64_t *bar, const Soa &in, int64_t n, int64_t tile)
+{
+    const int64_t base = tile * kTile;
+    if (base + kTile <= n) {                      // full tile: one elected thread issues the bulk copies
+        if (threadIdx.x == 0) {
+            mbar_expect_tx(bar, 6 * kTile * 8 + (NARR == 7 ? kTile * 4 : 0));
+            bulk_g2s(st.v[0], in.x + base, kTile * 8, bar);
+            bulk_g2s(st.v[1], in.y + base, kTile * 8, bar);
+            bulk_g2s(st.v[2], in.z + base, kTile * 8, bar);
+            bulk_g2s(st.v[3], in.px + base, kTile * 8, bar);
+            bulk_g2s(st.v[4], in.py + base, kTile * 8, bar);
+            bulk_g2s(st.v[5], in.pz + base, kTile * 8, bar);
+            if (NARR == 7) bulk_g2s(st.pid, in.pid + base, kTile * 4, bar);
+        }
+    } else {                                      // ragged tail: plain loads by everybody
+        for (int li = threadIdx.x; li < kTile; li += kTileThreads) {
+            const int64_t i = base + li;
+            if (i < n) {
+                st.v[0][li] = in.x[i]; st.v[1][li] = in.y[i]; st.v[2][li] = in.z[i];
+                st.v[3][li] = in.px[i]; st.v[4][li] = in.py[i]; st.v[5][li] = in.pz[i];
+                if (NARR == 7) st.pid[li] = in.pid[i];
+            }
+        }
+    }
+}
+
+template <int NARR>
+__device__ __forceinline__ void stage_wait(uint64_t *bar, uint32_t parity, int64_t n, int64_t tile)
+{
+    if (tile * kTile + kTile <= n) mbar_wait(bar, parity);
+    else __syncthreads();
+}
+
 // ---- K_A ------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kTileThreads)
-k_stream_hist(Geom g, double dt, int64_t n, Soa in, uint32_t *__restrict__ cnt,
+__global__ void __launch_bounds__(kTileThreads, 4)
+k_stream_hist(Geom g, double dt, int64_t n, int64_t ntiles, Soa in, uint32_t *__restrict__ cnt,
               uint32_t *__restrict__ tile_rec, uint32_t *__restrict__ flags)
 {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    TileStage<6> *stage = reinterpret_cast<TileStage<6> *>(smem_raw);
+    __shared__ __align__(8) uint64_t s_bar[2];
     __shared__ uint32_t s_tail[kDirs];
     __shared__ uint32_t s_cf, s_cl;
     const int tid = threadIdx.x;
-    const int64_t base = (int64_t)blockIdx.x * kTile;
-    const int64_t last = min(n, base + kTile) - 1;
-    if (tid < kDirs) s_tail[tid] = 0;
-
-    uint32_t c_old[kTileItems];
-    int d[kTileItems];
-#pragma unroll
-    for (int j = 0; j < kTileItems; ++j) {
-        const int64_t i = base + j * kTileThreads + tid;
-        const bool valid = i < n;
-        c_old[j] = 0; d[j] = -1;
-        const uint32_t active = __ballot_sync(0xFFFFFFFFu, valid);
-        if (valid) {
-            Moved m = move_particle(g, dt, in.x[i], in.y[i], in.z[i], in.px[i], in.py[i], in.pz[i]);
-            c_old[j] = m.c_old; d[j] = m.d;
-            if (m.d < 0) atomicOr(flags, kFlagMoved);
-            const uint32_t key = (uint32_t)max(m.d, 0) * g.ncells + m.c_old;
-            const uint32_t peers = __match_any_sync(active, key);
-            if ((peers & lanemask_lt()) == 0) atomicAdd(&cnt[key], (uint32_t)__popc(peers));
-            if (i == base) s_cf = m.c_old;
-            if (i == last) s_cl = m.c_old;
-        }
-    }
+    if (tid == 0) { mbar_init(&s_bar[0], 1); mbar_init(&s_bar[1], 1); mbar_fence_init(); }
     __syncthreads();
-    const uint32_t cl = s_cl;
-    // tail record: how many particles of the tile's LAST cell, per direction (feeds K_carry)
+    int64_t tile = blockIdx.x;
+    if (tile < ntiles) stage_issue<6>(stage[0], &s_bar[0], in, n, tile);
+    for (int it = 0; tile < ntiles; ++it, tile += gridDim.x) {
+        const int b = it & 1;
+        const int64_t next = tile + gridDim.x;
+        if (next < ntiles) stage_issue<6>(stage[b ^ 1], &s_bar[b ^ 1], in, n, next);
+        if (tid < kDirs) s_tail[tid] = 0;
+        stage_wait<6>(&s_bar[b], (uint32_t)((it >> 1) & 1), n, tile);
+        const TileStage<6> &st = stage[b];
+        const int64_t base = tile * kTile;
+        const int64_t last = min(n, base + kTile) - 1;
+        uint32_t c_old[kTileItems];
+        int d[kTileItems];
 #pragma unroll
-    for (int j = 0; j < kTileItems; ++j) {
-        const int64_t i = base + j * kTileThreads + tid;
-        const bool mine = (i < n) && c_old[j] == cl;
-        const uint32_t active = __ballot_sync(0xFFFFFFFFu, mine);
-        if (mine) {
-            const int dd = max(d[j], 0);
-            const uint32_t peers = __match_any_sync(active, dd);
-            if ((peers & lanemask_lt()) == 0) atomicAdd(&s_tail[dd], (uint32_t)__popc(peers));
+        for (int j = 0; j < kTileItems; ++j) {
+            const int li = j * kTileThreads + tid;
+            const int64_t i = base + li;
+            const bool valid = i < n;
+            c_old[j] = 0; d[j] = -1;
+            const uint32_t active = __ballot_sync(0xFFFFFFFFu, valid);
+            if (valid) {
+                Moved m = move_particle(g, dt, st.v[0][li], st.v[1][li], st.v[2][li], st.v[3][li], st.v[4][li], st.v[5][li]);
+                c_old[j] = m.c_old; d[j] = m.d;
+                if (m.d < 0) atomicOr(flags, kFlagMoved);
+                const uint32_t key = (uint32_t)max(m.d, 0) * g.ncells + m.c_old;
+                const uint32_t peers = __match_any_sync(active, key);
+                if ((peers & lanemask_lt()) == 0) atomicAdd(&cnt[key], (uint32_t)__popc(peers));
+                if (i == base) s_cf = m.c_old;
+                if (i == last) s_cl = m.c_old;
+            }
         }
+        __syncthreads();
+        const uint32_t cl = s_cl;
+        // tail record: how many particles of the tile's LAST cell, per direction (feeds K_carry)
+#pragma unroll
+        for (int j = 0; j < kTileItems; ++j) {
+            const int64_t i = base + j * kTileThreads + tid;
+            const bool mine = (i < n) && c_old[j] == cl;
+            const uint32_t active = __ballot_sync(0xFFFFFFFFu, mine);
+            if (mine) {
+                const int dd = max(d[j], 0);
+                const uint32_t peers = __match_any_sync(active, dd);
+                if ((peers & lanemask_lt()) == 0) atomicAdd(&s_tail[dd], (uint32_t)__popc(peers));
+            }
+        }
+        __syncthreads();
+        uint32_t *rec = tile_rec + (size_t)tile * kTileRec;
+        if (tid < kDirs) rec[tid] = s_tail[tid];
+        if (tid == 27) rec[27] = s_cf;
+        if (tid == 28) rec[28] = s_cl;
+        __syncthreads();   // stage b and s_tail are free again
     }
-    __syncthreads();
-    uint32_t *rec = tile_rec + (size_t)blockIdx.x * kTileRec;
-    if (tid < kDirs) rec[tid] = s_tail[tid];
-    if (tid == 27) rec[27] = s_cf;
-    if (tid == 28) rec[28] = s_cl;
 }
 
 // ---- K_B ------------------------------------------------------------------------------
@@ -267,84 +329,99 @@ k_carry(int ntiles, const uint32_t *__restrict__ tile_rec, uint32_t *__restrict_
 // in the tile that moved in direction d.  Stable rank inside (c_old, d) =
 // prefix_d(li) - prefix_d(first particle of c_old in the tile) [+ carry if that is li 0].
 template <bool WITH_CELL_OF_PID>
-__global__ void __launch_bounds__(kTileThreads)
-k_scatter(Geom g, double dt, int64_t n, Soa in, Soa out, const uint32_t *__restrict__ off,
+__global__ void __launch_bounds__(kTileThreads, 3)
+k_scatter(Geom g, double dt, int64_t n, int64_t ntiles, Soa in, Soa out, const uint32_t *__restrict__ off,
           const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ carry,
           uint32_t *__restrict__ cell_of_pid)
 {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    TileStage<7> *stage = reinterpret_cast<TileStage<7> *>(smem_raw);
+    __shared__ __align__(8) uint64_t s_bar[2];
     __shared__ uint32_t s_cold[kTile];
     __shared__ uint32_t s_ball[kTileRows][kDirs];
     __shared__ uint32_t s_pref[kTileRows][kDirs];
     __shared__ uint32_t s_head[kTileRows];
     __shared__ int s_lasthead[kTileRows];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const int64_t base = (int64_t)blockIdx.x * kTile;
+    if (tid == 0) { mbar_init(&s_bar[0], 1); mbar_init(&s_bar[1], 1); mbar_fence_init(); }
+    __syncthreads();
+    int64_t tile = blockIdx.x;
+    if (tile < ntiles) stage_issue<7>(stage[0], &s_bar[0], in, n, tile);
+    for (int it = 0; tile < ntiles; ++it, tile += gridDim.x) {
+        const int b = it & 1;
+        const int64_t next = tile + gridDim.x;
+        if (next < ntiles) stage_issue<7>(stage[b ^ 1], &s_bar[b ^ 1], in, n, next);
+        stage_wait<7>(&s_bar[b], (uint32_t)((it >> 1) & 1), n, tile);
+        const TileStage<7> &st = stage[b];
+        const int64_t base = tile * kTile;
 
-    Moved m[kTileItems];
-    uint32_t pid[kTileItems];
+        Moved m[kTileItems];
 #pragma unroll
-    for (int j = 0; j < kTileItems; ++j) {
-        const int64_t i = base + j * kTileThreads + tid;
-        m[j].d = -1; m[j].c_old = 0xFFFFFFFFu;
-        if (i < n) {
-            m[j] = move_particle(g, dt, in.x[i], in.y[i], in.z[i], in.px[i], in.py[i], in.pz[i]);
-            pid[j] = in.pid[i];
+        for (int j = 0; j < kTileItems; ++j) {
+            const int li = j * kTileThreads + tid;
+            m[j].d = -1; m[j].c_old = 0xFFFFFFFFu;
+            if (base + li < n)
+                m[j] = move_particle(g, dt, st.v[0][li], st.v[1][li], st.v[2][li], st.v[3][li], st.v[4][li], st.v[5][li]);
+            s_cold[li] = m[j].c_old;
         }
-        s_cold[j * kTileThreads + tid] = m[j].c_old;
-    }
-    __syncthreads();
+        __syncthreads();
 #pragma unroll
-    for (int j = 0; j < kTileItems; ++j) {
-        const int r = j * (kTileThreads / 32) + wid;
-        const int li = j * kTileThreads + tid;
-        const bool valid = (base + li) < n;
-        const int dd = m[j].d;
-        uint32_t mine = 0;
+        for (int j = 0; j < kTileItems; ++j) {
+            const int r = j * (kTileThreads / 32) + wid;
+            const int li = j * kTileThreads + tid;
+            const bool valid = (base + li) < n;
+            const int dd = m[j].d;
+            uint32_t mine = 0;
 #pragma unroll
-        for (int q = 0; q < kDirs; ++q) {
-            const uint32_t b = __ballot_sync(0xFFFFFFFFu, dd == q);
-            if (lane == q) mine = b;
+            for (int q = 0; q < kDirs; ++q) {
+                const uint32_t bq = __ballot_sync(0xFFFFFFFFu, dd == q);
+                if (lane == q) mine = bq;
+            }
+            if (lane < kDirs) s_ball[r][lane] = mine;
+            const bool head = valid && (li == 0 || s_cold[li - 1] != m[j].c_old);
+            const uint32_t hb = __ballot_sync(0xFFFFFFFFu, head);
+            if (lane == 0) s_head[r] = hb;
         }
-        if (lane < kDirs) s_ball[r][lane] = mine;
-        const bool head = valid && (li == 0 || s_cold[li - 1] != m[j].c_old);
-        const uint32_t hb = __ballot_sync(0xFFFFFFFFu, head);
-        if (lane == 0) s_head[r] = hb;
-    }
-    __syncthreads();
-    if (tid < kDirs) {
-        uint32_t run = 0;
-        for (int r = 0; r < kTileRows; ++r) {
-            s_pref[r][tid] = run;
-            run += __popc(s_ball[r][tid]);
-        }
-    } else if (tid == 32) {
-        int lh = -1;
-        for (int r = 0; r < kTileRows; ++r) {
-            s_lasthead[r] = lh;
-            const uint32_t hb = s_head[r];
-            if (hb) lh = r * 32 + 31 - __clz(hb);
-        }
-    }
-    __syncthreads();
+        __syncthreads();
+        if (tid < kDirs) {
+            uint32_t run = 0;
 #pragma unroll
-    for (int j = 0; j < kTileItems; ++j) {
-        const int li = j * kTileThreads + tid;
-        if ((base + li) >= n) continue;
-        const int dd = m[j].d;
-        if (dd < 0) continue;   // flagged by K_A; the particle is dropped from the placement
-        const int r = j * (kTileThreads / 32) + wid;
-        const uint32_t pre_i = s_pref[r][dd] + __popc(s_ball[r][dd] & lanemask_lt());
-        const uint32_t hm = s_head[r] & lanemask_le();
-        const int sli = hm ? (r * 32 + 31 - __clz(hm)) : s_lasthead[r];
-        const int rs = sli >> 5, ls = sli & 31;
-        const uint32_t pre_s = s_pref[rs][dd] + __popc(s_ball[rs][dd] & ((1u << ls) - 1u));
-        uint32_t rank = pre_i - pre_s;
-        if (sli == 0) rank += carry[(size_t)blockIdx.x * kTileRec + dd];
-        const uint32_t dest = cell_start[m[j].c_new] + off[(size_t)dd * g.ncells + m[j].c_old] + rank;
-        out.x[dest] = m[j].x; out.y[dest] = m[j].y; out.z[dest] = m[j].z;
-        out.px[dest] = m[j].px; out.py[dest] = m[j].py; out.pz[dest] = m[j].pz;
-        out.pid[dest] = pid[j];
-        if (WITH_CELL_OF_PID) cell_of_pid[pid[j]] = m[j].c_new;
+            for (int r = 0; r < kTileRows; ++r) {
+                s_pref[r][tid] = run;
+                run += __popc(s_ball[r][tid]);
+            }
+        } else if (tid == 32) {
+            int lh = -1;
+#pragma unroll
+            for (int r = 0; r < kTileRows; ++r) {
+                s_lasthead[r] = lh;
+                const uint32_t hb = s_head[r];
+                if (hb) lh = r * 32 + 31 - __clz(hb);
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < kTileItems; ++j) {
+            const int li = j * kTileThreads + tid;
+            if ((base + li) >= n) continue;
+            const int dd = m[j].d;
+            if (dd < 0) continue;   // flagged by K_A; the particle is dropped from the placement
+            const int r = j * (kTileThreads / 32) + wid;
+            const uint32_t pre_i = s_pref[r][dd] + __popc(s_ball[r][dd] & lanemask_lt());
+            const uint32_t hm = s_head[r] & lanemask_le();
+            const int sli = hm ? (r * 32 + 31 - __clz(hm)) : s_lasthead[r];
+            const int rs = sli >> 5, ls = sli & 31;
+            const uint32_t pre_s = s_pref[rs][dd] + __popc(s_ball[rs][dd] & ((1u << ls) - 1u));
+            uint32_t rank = pre_i - pre_s;
+            if (sli == 0) rank += carry[(size_t)tile * kTileRec + dd];
+            const uint32_t dest = cell_start[m[j].c_new] + off[(size_t)dd * g.ncells + m[j].c_old] + rank;
+            const uint32_t id = st.pid[li];
+            out.x[dest] = m[j].x; out.y[dest] = m[j].y; out.z[dest] = m[j].z;
+            out.px[dest] = m[j].px; out.py[dest] = m[j].py; out.pz[dest] = m[j].pz;
+            out.pid[dest] = id;
+            if (WITH_CELL_OF_PID) cell_of_pid[id] = m[j].c_new;
+        }
+        __syncthreads();   // stage b and the ballot tables are free again
     }
 }
 

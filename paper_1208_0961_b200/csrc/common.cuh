@@ -9,7 +9,7 @@ namespace cuba {
 
 constexpr int kDirs = 27;           // (dix+1)*9 + (diy+1)*3 + (diz+1), each di in {-1,0,1}
 constexpr int kTileThreads = 256;
-constexpr int kTileItems = 4;
+constexpr int kTileItems = 2;
 constexpr int kTile = kTileThreads * kTileItems;   // particles per tile in the flat passes
 constexpr int kTileRows = kTile / 32;
 constexpr int kTileRec = 32;        // u32 words per tile record: 27 counts, cf, cl, pad
@@ -109,8 +109,47 @@ __device__ __forceinline__ uint32_t lanemask_le()
     return m;
 }
 
-// streaming loads/stores: every particle array is touched once per pass
-__device__ __forceinline__ double ld_stream(const double *p) { return __ldcs(p); }
-__device__ __forceinline__ uint32_t ld_stream(const uint32_t *p) { return __ldcs(p); }
+// ---- TMA-style bulk staging: cp.async.bulk global -> shared, completion on an mbarrier ---
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
+{
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+
+__device__ __forceinline__ void mbar_fence_init()
+{
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra.uni WAIT_DONE;\n"
+        "bra.uni WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+
+// bytes must be a multiple of 16 and both addresses 16-byte aligned
+__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
 
 }  // namespace cuba

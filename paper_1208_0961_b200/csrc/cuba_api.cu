@@ -96,7 +96,7 @@ struct cuba_ctx {
     unsigned char *ws;
     Soa set[2];          // [0] caller's arrays + pidA, [1] workspace copy + pidB
     int cur;
-    int grid_s, grid_m, grid_l, grid_x, grid_o;
+    int grid_s, grid_m, grid_l, grid_x, grid_o, grid_hist, grid_scat;
     double *h_obs;       // pinned staging for observables
     bool prof_on = false;
     std::vector<cudaEvent_t> prof_pool;          // reused events
@@ -179,7 +179,7 @@ static void prof_mark(cuba_ctx *ctx, int group)
 template <typename K>
 static int occupancy_grid(K kernel, int threads, size_t smem, int sms, int *grid)
 {
-    if (smem > 48 * 1024)
+    if (smem > 32 * 1024)
         CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem));
@@ -202,6 +202,8 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
     if (!(n_test > 0.0) || !std::isfinite(n_test)) return CUBA_ERR_VALUE;
     Layout lay = make_layout(n, ncells);
     if (workspace_bytes < lay.total || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return CUBA_ERR_WORKSPACE;
+    for (const double *a : {x, y, z, px, py, pz})
+        if (reinterpret_cast<uintptr_t>(a) & 15u) return CUBA_ERR_WORKSPACE;   // bulk copies need 16-byte alignment
 
     int dev = 0, sms = 0;
     CU(cudaGetDevice(&dev));
@@ -237,6 +239,9 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
     if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrM, kCapM, 4, true>, kThrM, collide_smem_bytes(kCapM), sms, &ctx->grid_m);
     if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrL, kCapL, 2, true>, kThrL, collide_smem_bytes(kCapL), sms, &ctx->grid_l);
     if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrX, kCapX, 1, true>, kThrX, collide_smem_bytes(kCapX), sms, &ctx->grid_x);
+    if (rc == CUBA_OK) rc = occupancy_grid(k_stream_hist, kTileThreads, 2 * sizeof(TileStage<6>), sms, &ctx->grid_hist);
+    if (rc == CUBA_OK) rc = occupancy_grid(k_scatter<true>, kTileThreads, 2 * sizeof(TileStage<7>), sms, &ctx->grid_scat);
+    if (rc == CUBA_OK) rc = occupancy_grid(k_scatter<false>, kTileThreads, 2 * sizeof(TileStage<7>), sms, &ctx->grid_scat);
     if (rc != CUBA_OK) return fail(rc);
     ctx->grid_o = sms;
     if (!cuda_ok(cudaFuncSetAttribute(k_observe_partial, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -374,7 +379,7 @@ static int enqueue_bin(cuba_ctx *ctx, double dt, uint32_t *cell_of_pid)
     prof_mark(ctx, -1);
     CU(cudaMemsetAsync(cnt, 0, (size_t)kDirs * ncells * 4, st));
     prof_mark(ctx, G_MEMSET);
-    k_stream_hist<<<(unsigned)lay.ntiles, kTileThreads, 0, st>>>(ctx->g, dt, n, in, cnt, ctx->at<uint32_t>(lay.tile_rec),
+    k_stream_hist<<<ctx->grid_hist, kTileThreads, 2 * sizeof(TileStage<6>), st>>>(ctx->g, dt, n, lay.ntiles, in, cnt, ctx->at<uint32_t>(lay.tile_rec),
                                                                   ctx->at<uint32_t>(lay.flags));
     LAUNCHED();
     prof_mark(ctx, G_STREAM_HIST);
@@ -397,10 +402,10 @@ static int enqueue_bin(cuba_ctx *ctx, double dt, uint32_t *cell_of_pid)
     LAUNCHED();
     prof_mark(ctx, G_CARRY);
     if (cell_of_pid)
-        k_scatter<true><<<(unsigned)lay.ntiles, kTileThreads, 0, st>>>(ctx->g, dt, n, in, outp, cnt, ctx->at<uint32_t>(lay.cell_start),
+        k_scatter<true><<<ctx->grid_scat, kTileThreads, 2 * sizeof(TileStage<7>), st>>>(ctx->g, dt, n, lay.ntiles, in, outp, cnt, ctx->at<uint32_t>(lay.cell_start),
                                                                        ctx->at<uint32_t>(lay.carry), cell_of_pid);
     else
-        k_scatter<false><<<(unsigned)lay.ntiles, kTileThreads, 0, st>>>(ctx->g, dt, n, in, outp, cnt, ctx->at<uint32_t>(lay.cell_start),
+        k_scatter<false><<<ctx->grid_scat, kTileThreads, 2 * sizeof(TileStage<7>), st>>>(ctx->g, dt, n, lay.ntiles, in, outp, cnt, ctx->at<uint32_t>(lay.cell_start),
                                                                         ctx->at<uint32_t>(lay.carry), nullptr);
     LAUNCHED();
     prof_mark(ctx, G_SCATTER);
