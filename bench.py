@@ -226,10 +226,12 @@ def main():
         raise SystemExit("device error flags %d" % c1.device_flags)
 
     # particles each collide class handled in the last step (for per-launch algorithmic bytes)
+    import re
     counts = np.diff(sim.cell_start().astype(np.int64))
-    caps = [64, 512, 2048, 4544]
+    collide_names = [k for k in prof if k.startswith("k_collide")]
+    caps = [int(re.search(r"cap=(\d+)", k).group(1)) for k in collide_names if "cap=" in k]
     cls = np.searchsorted(caps, counts, side="left")
-    class_particles = [int(counts[(cls == k) & (counts >= 2)].sum()) for k in range(5)]
+    class_particles = {name: int(counts[(cls == k) & (counts >= 2)].sum()) for k, name in enumerate(collide_names)}
 
     # ---- observables timed separately --------------------------------------------------
     torch.cuda.synchronize()
@@ -272,10 +274,8 @@ def main():
         # dominant kernel by measured device time
         per_kernel = {k: {"ms_per_launch": (v[0] / v[1]) if v[1] else 0.0, "launches": v[1], "ms_total": v[0]}
                       for k, v in prof.items()}
-        alg = {"k_stream_hist": BYTES_STREAM_HIST * n, "k_scatter": BYTES_SCATTER * n,
-               "k_collide<32>": BYTES_COLLIDE * class_particles[0], "k_collide<128>": BYTES_COLLIDE * class_particles[1],
-               "k_collide<512>": BYTES_COLLIDE * class_particles[2], "k_collide<1024>": BYTES_COLLIDE * class_particles[3],
-               "k_collide_overflow": BYTES_COLLIDE * class_particles[4]}
+        alg = {"k_stream_hist": BYTES_STREAM_HIST * n, "k_scatter": BYTES_SCATTER * n}
+        alg.update({name: BYTES_COLLIDE * cnt for name, cnt in class_particles.items()})
         dom = max(per_kernel, key=lambda k: per_kernel[k]["ms_total"])
         dom_ms = per_kernel[dom]["ms_per_launch"]
         achieved = alg.get(dom, 0) / (dom_ms * 1e-3) / 1e9 if dom_ms else 0.0

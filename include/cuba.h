@@ -150,7 +150,7 @@ int cuba_run_host(const double box[3], const int ncell[3], int64_t n,
  * cuba_profile_read synchronises and returns, for each of the CUBA_PROFILE_GROUPS kernel
  * groups, the summed device time in milliseconds and the number of launches since the last
  * enable, then clears the log.  HOST outputs of CUBA_PROFILE_GROUPS entries each. */
-#define CUBA_PROFILE_GROUPS 12
+#define CUBA_PROFILE_GROUPS 15
 int cuba_profile_enable(cuba_ctx *ctx, int on);
 int cuba_profile_read(cuba_ctx *ctx, double *ms_sum, uint64_t *launches);
 const char *cuba_profile_name(int group);

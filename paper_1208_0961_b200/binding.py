@@ -238,7 +238,7 @@ class Cuba:
 
     def profile_read(self):
         """{kernel group: (summed device ms, launches)} since profile_enable."""
-        G = 12
+        G = 15
         ms = (c_double * G)()
         cnt = (c_uint64 * G)()
         _check(lib().cuba_profile_read(self._h, ms, cnt))

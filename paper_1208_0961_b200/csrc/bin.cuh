@@ -246,7 +246,7 @@ k_scan_blocks(uint32_t *__restrict__ block_sum, int nblocks, uint32_t *__restric
 
 // ---- K_F: cell_start = block prefix + local exclusive scan; cells with n >= 2 are appended
 // to the work list of their size class for the collision kernels -------------------------
-constexpr int kNumClasses = 5;   // 4 shared-memory classes + the global-memory overflow class
+constexpr int kNumClasses = 8;   // 7 shared-memory classes + the global-memory overflow class
 
 struct ClassTable {
     uint32_t max_n[kNumClasses];   // inclusive upper bound of each class (last = UINT32_MAX)

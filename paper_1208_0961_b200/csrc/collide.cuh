@@ -93,8 +93,8 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t *s
     return wpre + inc - v;
 }
 
-// THREADS threads work on one cell of n particles whose scratch arrays are given (shared
-// memory for the size classes, global memory for the overflow class).
+// Generic routine (overflow class): THREADS threads work on one cell of n particles of any
+// size, scratch arrays in global memory, n buckets of 32-bit counters, run-time loops.
 template <int THREADS, bool TRACE, typename IdxT>
 __device__ __forceinline__ void collide_cell(const CollideParams &P, uint32_t c, uint32_t lo, uint32_t n,
                                              double *sp0, double *sp1, double *sp2, double *sE,
@@ -212,6 +212,210 @@ __device__ __forceinline__ void collide_cell(const CollideParams &P, uint32_t c,
     if (tid == 0) atomicAdd(&P.counters[2], (unsigned long long)R);
 }
 
+// One pair: Eq. 3 decision.  Returns hit; s (Mandelstam) through s_out.
+__device__ __forceinline__ bool pair_decide(const CollideParams &P, uint32_t ida, uint32_t rho, double scale,
+                                            double pax, double pay, double paz, double Ea,
+                                            double pbx, double pby, double pbz, double Eb,
+                                            double &s_out, double &prob_out, double &u_out)
+{
+    const double ee = Ea * Eb;
+    const double dx = Eb * pax - Ea * pbx;
+    const double dy = Eb * pay - Ea * pby;
+    const double dz = Eb * paz - Ea * pbz;
+    const double s = ((dx * dx + dy * dy) + dz * dz) / ee;   // (p_a+p_b)^2, A9
+    const double vrel = 0.5 * (s / ee);                       // s/(2 E_a E_b)
+    const double prob = vrel * scale;                         // Eq. 3 * cn/R
+    const U4 w = draw(P.seed, ida, P.t, rho, kTagDec, 0);
+    const double u = u53(w.x, w.y);
+    s_out = s; prob_out = prob; u_out = u;
+    return u < prob;
+}
+
+// Boost to the CM frame, isotropic direction, boost back (closed form A10).
+__device__ __forceinline__ void pair_scatter(const CollideParams &P, uint32_t ida, uint32_t rho, double s,
+                                             double pax, double pay, double paz, double Ea,
+                                             double pbx, double pby, double pbz, double Eb,
+                                             double q[6])
+{
+    double nx, ny, nz;
+    draw_direction(P.seed, ida, P.t, rho, nx, ny, nz);
+    const double rs = sqrt(s);
+    const double Pvx = pax + pbx, Pvy = pay + pby, Pvz = paz + pbz;
+    const double Et = Ea + Eb;
+    const double Pn = (Pvx * nx + Pvy * ny) + Pvz * nz;
+    const double al = Pn / (Et + rs);
+    const double f1 = 1.0 + al, f2 = 1.0 - al;
+    q[0] = 0.5 * (rs * nx + Pvx * f1);
+    q[1] = 0.5 * (rs * ny + Pvy * f1);
+    q[2] = 0.5 * (rs * nz + Pvz * f1);
+    q[3] = 0.5 * (Pvx * f2 - rs * nx);
+    q[4] = 0.5 * (Pvy * f2 - rs * ny);
+    q[5] = 0.5 * (Pvz * f2 - rs * nz);
+}
+
+// Shared-memory classes: THREADS threads, at most THREADS*ITEMS particles, compile-time trip
+// counts.  Differences to the generic routine, all invisible in the results:
+//   * 2n buckets with 16-bit counters packed two per word (expected occupancy 1/2);
+//   * pairs that collide are compacted into a list first, so the expensive scatter path runs
+//     on full warps instead of on the ~25 % of lanes that hit in a round.
+template <int THREADS, int ITEMS, bool TRACE>
+__device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32_t c, uint32_t lo, uint32_t n,
+                                                  double *sp0, double *sp1, double *sp2, double *sE,
+                                                  uint32_t *spid, uint32_t *skey, uint32_t *sbkt,
+                                                  uint16_t *sord, uint16_t *stmp, uint32_t *s_warp,
+                                                  uint32_t *s_nhit,
+                                                  unsigned long long &n_pairs, unsigned long long &n_coll,
+                                                  unsigned long long &n_near)
+{
+    const int tid = threadIdx.x, lane = tid & 31;
+    const double cn = (n & 1u) ? (double)n : (double)(n - 1u);
+    const double pmax = (2.0 * cn) * P.base;
+    int R;
+    if (!(pmax <= 64.0)) { if (tid == 0) atomicOr(P.flags, kFlagRounds); R = 64; }
+    else R = (pmax <= 1.0) ? 1 : (int)ceil(pmax);
+    const double scale = (cn * P.base) / (double)R;
+    const uint32_t npairs = n >> 1;
+    const uint32_t nb = 2u * n;
+    uint16_t *sb16 = reinterpret_cast<uint16_t *>(sbkt);
+    double *sS = reinterpret_cast<double *>(skey);   // Mandelstam s of the colliding pairs (skey is dead by then)
+
+#pragma unroll
+    for (int it = 0; it < ITEMS; ++it) {
+        const uint32_t j = tid + it * THREADS;
+        if (j < n) {
+            const double a = P.px[lo + j], b = P.py[lo + j], cc = P.pz[lo + j];
+            sp0[j] = a; sp1[j] = b; sp2[j] = cc;
+            sE[j] = energy(a, b, cc);
+            spid[j] = P.pid[lo + j];
+            sbkt[j] = 0;
+        }
+    }
+    if (tid == 0) { sbkt[n] = 0; *s_nhit = 0; }
+    __syncthreads();
+
+    for (int rho = 0; rho < R; ++rho) {
+        // (a) keys, bucket counts; the arrival slot only serves to park the element
+#pragma unroll
+        for (int it = 0; it < ITEMS; ++it) {
+            const uint32_t j = tid + it * THREADS;
+            if (j < n) {
+                const uint32_t k = draw(P.seed, spid[j], P.t, (uint32_t)rho, kTagShuf, 0).x;
+                skey[j] = k;
+                const uint32_t b = __umulhi(k, nb);
+                const uint32_t sh = (b & 1u) * 16u;
+                const uint32_t old = atomicAdd(&sbkt[b >> 1], 1u << sh);
+                sord[j] = (uint16_t)((old >> sh) & 0xFFFFu);
+            }
+        }
+        __syncthreads();
+        // (b) exclusive scan of the 2n counters (n words), contiguous chunk of words per thread
+        {
+            const uint32_t chunk = (n + THREADS - 1) / THREADS;
+            const uint32_t w0 = min(n, tid * chunk), w1 = min(n, w0 + chunk);
+            uint32_t sum = 0;
+            for (uint32_t w = w0; w < w1; ++w) { const uint32_t v = sbkt[w]; sum += (v & 0xFFFFu) + (v >> 16); }
+            uint32_t total;
+            uint32_t run = block_exclusive_scan<THREADS>(sum, s_warp, total);
+            for (uint32_t w = w0; w < w1; ++w) {
+                const uint32_t v = sbkt[w];
+                const uint32_t mid = run + (v & 0xFFFFu);
+                sbkt[w] = run | (mid << 16);
+                run = mid + (v >> 16);
+            }
+            if (tid == 0) sbkt[n] = n;   // start of the sentinel bucket 2n
+        }
+        __syncthreads();
+        // (c) park element j at its arrival slot inside its bucket
+#pragma unroll
+        for (int it = 0; it < ITEMS; ++it) {
+            const uint32_t j = tid + it * THREADS;
+            if (j < n) stmp[(uint32_t)sb16[__umulhi(skey[j], nb)] + (uint32_t)sord[j]] = (uint16_t)j;
+        }
+        __syncthreads();
+        // (d) final rank = bucket start + number of bucket mates with a smaller (key, pid)
+#pragma unroll
+        for (int it = 0; it < ITEMS; ++it) {
+            const uint32_t j = tid + it * THREADS;
+            if (j < n) {
+                const uint32_t k = skey[j];
+                const uint32_t b = __umulhi(k, nb);
+                const uint32_t beg = sb16[b], end = sb16[b + 1];
+                uint32_t rank = beg;
+                if (end - beg > 1u) {
+                    const uint32_t id = spid[j];
+                    for (uint32_t q = beg; q < end; ++q) {
+                        const uint32_t jj = stmp[q];
+                        const uint32_t k2 = skey[jj];
+                        rank += (k2 < k || (k2 == k && spid[jj] < id)) ? 1u : 0u;
+                    }
+                }
+                sord[rank] = (uint16_t)j;   // arrival slots in sord are dead after (c)
+            }
+        }
+        __syncthreads();
+        // (e1) pair order[2k] with order[2k+1]: Eq. 3 decision; colliding pairs go to a list
+#pragma unroll
+        for (int it = 0; it < (ITEMS + 1) / 2; ++it) {
+            const uint32_t k = tid + it * THREADS;
+            bool hit = false;
+            double s = 0.0;
+            if (k < npairs) {
+                const uint32_t a = sord[2 * k], b = sord[2 * k + 1];
+                const uint32_t ida = spid[a];
+                double prob, u;
+                hit = pair_decide(P, ida, (uint32_t)rho, scale, sp0[a], sp1[a], sp2[a], sE[a],
+                                  sp0[b], sp1[b], sp2[b], sE[b], s, prob, u);
+                n_pairs += 1;
+                if (fabs(u - prob) <= 1e-12) n_near += 1;
+                if (TRACE) {
+                    const unsigned long long e = P.trace_off[c] + (unsigned long long)rho * npairs + k;
+                    P.tr_cell[e] = c; P.tr_round[e] = (uint32_t)rho; P.tr_pa[e] = ida; P.tr_pb[e] = spid[b];
+                    P.tr_P[e] = prob; P.tr_u[e] = u; P.tr_dec[e] = hit ? 1 : 0;
+                }
+            }
+            const uint32_t hm = __ballot_sync(0xFFFFFFFFu, hit);
+            if (hm) {
+                uint32_t basep = 0;
+                if (lane == 0) basep = atomicAdd(s_nhit, (uint32_t)__popc(hm));
+                basep = __shfl_sync(0xFFFFFFFFu, basep, 0);
+                if (hit) {
+                    const uint32_t pos = basep + __popc(hm & lanemask_lt());
+                    stmp[pos] = (uint16_t)k;      // stmp and skey are dead after (d)
+                    sS[k] = s;
+                }
+            }
+        }
+        // the bucket counters are free from here on: clear them for the next round
+#pragma unroll
+        for (int it = 0; it < ITEMS; ++it) {
+            const uint32_t j = tid + it * THREADS;
+            if (j < n) sbkt[j] = 0;
+        }
+        if (tid == 0) sbkt[n] = 0;
+        __syncthreads();
+        // (e2) scatter the colliding pairs, densely
+        const uint32_t nhit = *s_nhit;
+        for (uint32_t h = tid; h < nhit; h += THREADS) {
+            const uint32_t k = stmp[h];
+            const uint32_t a = sord[2 * k], b = sord[2 * k + 1];
+            double q[6];
+            pair_scatter(P, spid[a], (uint32_t)rho, sS[k], sp0[a], sp1[a], sp2[a], sE[a],
+                         sp0[b], sp1[b], sp2[b], sE[b], q);
+            sp0[a] = q[0]; sp1[a] = q[1]; sp2[a] = q[2]; sE[a] = energy(q[0], q[1], q[2]);
+            sp0[b] = q[3]; sp1[b] = q[4]; sp2[b] = q[5]; sE[b] = energy(q[3], q[4], q[5]);
+        }
+        if (tid == 0) n_coll += nhit;
+        __syncthreads();
+        if (tid == 0) *s_nhit = 0;
+    }
+#pragma unroll
+    for (int it = 0; it < ITEMS; ++it) {
+        const uint32_t j = tid + it * THREADS;
+        if (j < n) { P.px[lo + j] = sp0[j]; P.py[lo + j] = sp1[j]; P.pz[lo + j] = sp2[j]; }
+    }
+    if (tid == 0) atomicAdd(&P.counters[2], (unsigned long long)R);
+}
+
 template <int THREADS>
 __device__ __forceinline__ void flush_counters(const CollideParams &P, unsigned long long n_pairs,
                                                unsigned long long n_coll, unsigned long long n_near)
@@ -229,8 +433,15 @@ __device__ __forceinline__ void flush_counters(const CollideParams &P, unsigned 
     }
 }
 
-// Shared-memory classes: CAP particles at most, 48 B of shared memory per particle.
-template <int THREADS, int CAP, int MIN_BLOCKS, bool TRACE>
+__device__ __forceinline__ void prefetch_l2(const void *p)
+{
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+
+// Shared-memory classes: CAP particles at most, 48 B of shared memory per particle.  The next
+// work item is fetched one cell ahead and its momenta / pids are prefetched into L2 while
+// the current cell is processed, so the load phase does not wait on DRAM.
+template <int THREADS, int ITEMS, int CAP, int MIN_BLOCKS, bool TRACE>
 __global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
 k_collide(CollideParams P)
 {
@@ -239,24 +450,37 @@ k_collide(CollideParams P)
     double *sp1 = sp0 + CAP, *sp2 = sp1 + CAP, *sE = sp2 + CAP;
     uint32_t *spid = reinterpret_cast<uint32_t *>(sE + CAP);
     uint32_t *skey = spid + CAP;
-    uint32_t *sbkt = skey + CAP;                 // CAP + 2 entries
+    uint32_t *sbkt = skey + CAP;                 // CAP + 2 words = 2 CAP + 4 packed counters
     uint16_t *sord = reinterpret_cast<uint16_t *>(sbkt + CAP + 2);
     uint16_t *stmp = sord + CAP;
     __shared__ uint32_t s_warp[32];
-    __shared__ uint32_t s_item;
+    __shared__ uint32_t s_item[2];
+    __shared__ uint32_t s_nhit;
 
     const uint32_t nlist = *P.list_count;
     unsigned long long n_pairs = 0, n_coll = 0, n_near = 0;
-    for (;;) {
-        if (threadIdx.x == 0) s_item = atomicAdd(P.work, 1u);
+    if (threadIdx.x == 0) s_item[0] = atomicAdd(P.work, 1u);
+    __syncthreads();
+    uint32_t item = s_item[0];
+    for (int it = 0; item < nlist; ++it) {
+        if (threadIdx.x == 0) s_item[(it + 1) & 1] = atomicAdd(P.work, 1u);
         __syncthreads();
-        const uint32_t item = s_item;
-        if (item >= nlist) break;
+        const uint32_t next = s_item[(it + 1) & 1];
+        if (next < nlist) {
+            const uint32_t c2 = P.list[next];
+            const uint32_t lo2 = P.cell_start[c2], n2 = P.cell_start[c2 + 1] - lo2;
+            for (uint32_t l = threadIdx.x * 16u; l < n2 + 16u; l += THREADS * 16u) {   // one 128 B line per thread
+                const uint32_t e = lo2 + min(l, n2 - 1u);
+                prefetch_l2(P.px + e); prefetch_l2(P.py + e); prefetch_l2(P.pz + e);
+                if ((l & 16u) == 0) prefetch_l2(P.pid + e);
+            }
+        }
         const uint32_t c = P.list[item];
         const uint32_t lo = P.cell_start[c], n = P.cell_start[c + 1] - lo;
-        collide_cell<THREADS, TRACE, uint16_t>(P, c, lo, n, sp0, sp1, sp2, sE, spid, skey, sbkt, sord,
-                                               stmp, s_warp, n_pairs, n_coll, n_near);
+        collide_cell_smem<THREADS, ITEMS, TRACE>(P, c, lo, n, sp0, sp1, sp2, sE, spid, skey, sbkt, sord,
+                                                 stmp, s_warp, &s_nhit, n_pairs, n_coll, n_near);
         __syncthreads();
+        item = next;
     }
     flush_counters<THREADS>(P, n_pairs, n_coll, n_near);
 }

@@ -32,11 +32,20 @@ bool cuda_ok(cudaError_t e, const char *what)
 #define CU(call) do { if (!cuda_ok((call), #call)) return CUBA_ERR_CUDA; } while (0)
 #define LAUNCHED() do { g_launches.fetch_add(1, std::memory_order_relaxed); if (!cuda_ok(cudaGetLastError(), "kernel launch")) return CUBA_ERR_CUDA; } while (0)
 
-// size classes of the collision kernels: threads per CTA, capacity (particles per cell)
-constexpr int kThrS = 32, kCapS = 64;
-constexpr int kThrM = 128, kCapM = 512;
-constexpr int kThrL = 512, kCapL = 2048;
-constexpr int kThrX = 1024, kCapX = 4544;
+// Size classes of the collision kernels: X(index, threads per CTA, items per thread, capacity
+// in particles, min CTAs per SM).  A cell goes to the first class whose capacity holds it; a
+// cell beyond the last capacity goes to the global-memory overflow kernel.  Thread counts are
+// about a quarter of the capacity so that every thread owns <= 4 particles and <= 2 pairs.
+#define CUBA_FOR_EACH_CLASS(X) \
+    X(0, 32, 4, 128, 16)       \
+    X(1, 64, 4, 256, 12)       \
+    X(2, 128, 4, 512, 8)       \
+    X(3, 224, 4, 896, 4)       \
+    X(4, 352, 4, 1408, 3)      \
+    X(5, 512, 4, 2048, 2)      \
+    X(6, 1024, 5, 4544, 1)
+constexpr int kSmemClasses = 7;
+static_assert(kSmemClasses + 1 == kNumClasses, "class table");
 
 size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
@@ -47,7 +56,7 @@ struct Layout {
 };
 
 constexpr int kObsGrid = 296;
-constexpr int kZeroWords = 16;   // class_count[5], work[5], arena cursor (u64 = 2 words), pad
+constexpr int kZeroWords = 32;   // class_count[8], work[8], arena cursor (u64 = 2 words), pad
 
 Layout make_layout(int64_t n, int64_t ncells)
 {
@@ -96,7 +105,7 @@ struct cuba_ctx {
     unsigned char *ws;
     Soa set[2];          // [0] caller's arrays + pidA, [1] workspace copy + pidB
     int cur;
-    int grid_s, grid_m, grid_l, grid_x, grid_o, grid_hist, grid_scat;
+    int grid_cls[kSmemClasses], grid_o, grid_hist, grid_scat;
     double *h_obs;       // pinned staging for observables
     bool prof_on = false;
     std::vector<cudaEvent_t> prof_pool;          // reused events
@@ -162,9 +171,8 @@ static int sync_and_check(cuba_ctx *ctx)
     return device_flags_to_error(f);
 }
 
-enum { G_MEMSET = 0, G_STREAM_HIST, G_GATHER, G_SCAN, G_CELL_START, G_CARRY, G_SCATTER,
-       G_COLLIDE_S, G_COLLIDE_M, G_COLLIDE_L, G_COLLIDE_X, G_COLLIDE_O };
-static_assert(G_COLLIDE_O + 1 == CUBA_PROFILE_GROUPS, "profile groups");
+enum { G_MEMSET = 0, G_STREAM_HIST, G_GATHER, G_SCAN, G_CELL_START, G_CARRY, G_SCATTER, G_COLLIDE0 };
+static_assert(G_COLLIDE0 + kNumClasses == CUBA_PROFILE_GROUPS, "profile groups");
 
 static void prof_mark(cuba_ctx *ctx, int group)
 {
@@ -231,14 +239,12 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
     auto fail = [&](int code) { if (ctx->h_obs) cudaFreeHost(ctx->h_obs); delete ctx; return code; };
     if (!cuda_ok(cudaMallocHost(&ctx->h_obs, (4 + kObsMaxSlabs) * sizeof(double)), "cudaMallocHost")) return fail(CUBA_ERR_CUDA);
 
-    rc = occupancy_grid(k_collide<kThrS, kCapS, 16, false>, kThrS, collide_smem_bytes(kCapS), sms, &ctx->grid_s);
-    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrM, kCapM, 4, false>, kThrM, collide_smem_bytes(kCapM), sms, &ctx->grid_m);
-    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrL, kCapL, 2, false>, kThrL, collide_smem_bytes(kCapL), sms, &ctx->grid_l);
-    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrX, kCapX, 1, false>, kThrX, collide_smem_bytes(kCapX), sms, &ctx->grid_x);
-    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrS, kCapS, 16, true>, kThrS, collide_smem_bytes(kCapS), sms, &ctx->grid_s);
-    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrM, kCapM, 4, true>, kThrM, collide_smem_bytes(kCapM), sms, &ctx->grid_m);
-    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrL, kCapL, 2, true>, kThrL, collide_smem_bytes(kCapL), sms, &ctx->grid_l);
-    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<kThrX, kCapX, 1, true>, kThrX, collide_smem_bytes(kCapX), sms, &ctx->grid_x);
+#define CUBA_OCC(K, T, I, C, MB)                                                                                          \
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, false>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]); \
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, true>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]);
+    rc = CUBA_OK;
+    CUBA_FOR_EACH_CLASS(CUBA_OCC)
+#undef CUBA_OCC
     if (rc == CUBA_OK) rc = occupancy_grid(k_stream_hist, kTileThreads, 2 * sizeof(TileStage<6>), sms, &ctx->grid_hist);
     if (rc == CUBA_OK) rc = occupancy_grid(k_scatter<true>, kTileThreads, 2 * sizeof(TileStage<7>), sms, &ctx->grid_scat);
     if (rc == CUBA_OK) rc = occupancy_grid(k_scatter<false>, kTileThreads, 2 * sizeof(TileStage<7>), sms, &ctx->grid_scat);
@@ -327,29 +333,20 @@ static int launch_collide(cuba_ctx *ctx, double base, const TraceDev *td)
     }
     uint32_t *zero = ctx->at<uint32_t>(lay.zero);
     uint32_t *lists = ctx->at<uint32_t>(lay.class_list);
-    auto cls = [&](int k) { P.list = lists + (size_t)k * ctx->g.ncells; P.list_count = zero + k; P.work = zero + 5 + k; };
+    auto cls = [&](int k) { P.list = lists + (size_t)k * ctx->g.ncells; P.list_count = zero + k; P.work = zero + 8 + k; };
     cudaStream_t st = ctx->stream;
-    cls(0);
-    k_collide<kThrS, kCapS, 16, TRACE><<<ctx->grid_s, kThrS, collide_smem_bytes(kCapS), st>>>(P);
-    LAUNCHED();
-    prof_mark(ctx, G_COLLIDE_S);
-    cls(1);
-    k_collide<kThrM, kCapM, 4, TRACE><<<ctx->grid_m, kThrM, collide_smem_bytes(kCapM), st>>>(P);
-    LAUNCHED();
-    prof_mark(ctx, G_COLLIDE_M);
-    cls(2);
-    k_collide<kThrL, kCapL, 2, TRACE><<<ctx->grid_l, kThrL, collide_smem_bytes(kCapL), st>>>(P);
-    LAUNCHED();
-    prof_mark(ctx, G_COLLIDE_L);
-    cls(3);
-    k_collide<kThrX, kCapX, 1, TRACE><<<ctx->grid_x, kThrX, collide_smem_bytes(kCapX), st>>>(P);
-    LAUNCHED();
-    prof_mark(ctx, G_COLLIDE_X);
-    cls(4);
-    k_collide_overflow<TRACE><<<ctx->grid_o, 1024, 0, st>>>(P, reinterpret_cast<unsigned long long *>(zero + 10),
+#define CUBA_LAUNCH(K, T, I, C, MB)                                                              \
+    cls(K);                                                                                      \
+    k_collide<T, I, C, MB, TRACE><<<ctx->grid_cls[K], T, collide_smem_bytes(C), st>>>(P);        \
+    LAUNCHED();                                                                                  \
+    prof_mark(ctx, G_COLLIDE0 + K);
+    CUBA_FOR_EACH_CLASS(CUBA_LAUNCH)
+#undef CUBA_LAUNCH
+    cls(kSmemClasses);
+    k_collide_overflow<TRACE><<<ctx->grid_o, 1024, 0, st>>>(P, reinterpret_cast<unsigned long long *>(zero + 16),
                                                            ctx->at<double>(lay.arenaE));
     LAUNCHED();
-    prof_mark(ctx, G_COLLIDE_O);
+    prof_mark(ctx, G_COLLIDE0 + kSmemClasses);
     return CUBA_OK;
 }
 
@@ -390,7 +387,11 @@ static int enqueue_bin(cuba_ctx *ctx, double dt, uint32_t *cell_of_pid)
     k_scan_blocks<<<1, 1024, 0, st>>>(ctx->at<uint32_t>(lay.block_sum), (int)lay.nblocks_cells, zero, kZeroWords);
     LAUNCHED();
     prof_mark(ctx, G_SCAN);
-    ClassTable ct{{(uint32_t)kCapS, (uint32_t)kCapM, (uint32_t)kCapL, (uint32_t)kCapX, 0xFFFFFFFFu}};
+    ClassTable ct{};
+#define CUBA_CAP(K, T, I, C, MB) ct.max_n[K] = C;
+    CUBA_FOR_EACH_CLASS(CUBA_CAP)
+#undef CUBA_CAP
+    ct.max_n[kSmemClasses] = 0xFFFFFFFFu;
     k_cell_start<<<(unsigned)lay.nblocks_cells, 256, 0, st>>>(ncells, ctx->at<uint32_t>(lay.count_new),
                                                               ctx->at<uint32_t>(lay.block_sum), ctx->at<uint32_t>(lay.cell_start),
                                                               ct, zero, ctx->at<uint32_t>(lay.class_list),
@@ -554,7 +555,10 @@ const char *cuba_profile_name(int group)
 {
     static const char *names[CUBA_PROFILE_GROUPS] = {
         "memset_cnt", "k_stream_hist", "k_gather", "k_scan_blocks", "k_cell_start", "k_carry", "k_scatter",
-        "k_collide<32>", "k_collide<128>", "k_collide<512>", "k_collide<1024>", "k_collide_overflow"};
+#define CUBA_NAME(K, T, I, C, MB) "k_collide<T=" #T ",cap=" #C ">",
+        CUBA_FOR_EACH_CLASS(CUBA_NAME)
+#undef CUBA_NAME
+        "k_collide_overflow"};
     return (group >= 0 && group < CUBA_PROFILE_GROUPS) ? names[group] : "?";
 }
 
