@@ -163,6 +163,7 @@ def main():
     ap.add_argument("--impl", default="cuba", choices=["cuba", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--profile-mode", type=int, default=1, help="1: normal operation; 2: serialise the collision classes (diagnostic)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuba" else args.warmup
 
@@ -207,7 +208,7 @@ def main():
     barrier()
     c0 = sim.counters()
     l0 = cuba.launch_count()
-    sim.profile_enable(True)
+    sim.profile_enable(args.profile_mode)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     sampler.armed = True
@@ -219,7 +220,7 @@ def main():
     ms = ev0.elapsed_time(ev1)
     launches = cuba.launch_count() - l0
     prof = sim.profile_read()
-    sim.profile_enable(False)
+    sim.profile_enable(0)
     c1 = sim.counters()
     pairs = c1.pairs - c0.pairs
     if c1.device_flags:
@@ -228,7 +229,7 @@ def main():
     # particles each collide class handled in the last step (for per-launch algorithmic bytes)
     import re
     counts = np.diff(sim.cell_start().astype(np.int64))
-    collide_names = [k for k in prof if k.startswith("k_collide")]
+    collide_names = [k for k in prof if k.startswith("k_collide<") or k == "k_collide_overflow"]
     caps = [int(re.search(r"cap=(\d+)", k).group(1)) for k in collide_names if "cap=" in k]
     cls = np.searchsorted(caps, counts, side="left")
     class_particles = {name: int(counts[(cls == k) & (counts >= 2)].sum()) for k, name in enumerate(collide_names)}
@@ -276,6 +277,7 @@ def main():
                       for k, v in prof.items()}
         alg = {"k_stream_hist": BYTES_STREAM_HIST * n, "k_scatter": BYTES_SCATTER * n}
         alg.update({name: BYTES_COLLIDE * cnt for name, cnt in class_particles.items()})
+        alg["k_collide (all classes, concurrent)"] = BYTES_COLLIDE * sum(class_particles.values())
         dom = max(per_kernel, key=lambda k: per_kernel[k]["ms_total"])
         dom_ms = per_kernel[dom]["ms_per_launch"]
         achieved = alg.get(dom, 0) / (dom_ms * 1e-3) / 1e9 if dom_ms else 0.0

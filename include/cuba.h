@@ -149,8 +149,11 @@ int cuba_run_host(const double box[3], const int ncell[3], int64_t n,
  * ~1 us per event, no device-side serialisation beyond the stream's own order);
  * cuba_profile_read synchronises and returns, for each of the CUBA_PROFILE_GROUPS kernel
  * groups, the summed device time in milliseconds and the number of launches since the last
- * enable, then clears the log.  HOST outputs of CUBA_PROFILE_GROUPS entries each. */
-#define CUBA_PROFILE_GROUPS 15
+ * enable, then clears the log.  HOST outputs of CUBA_PROFILE_GROUPS entries each.
+ * Mode 1 times the collision kernels as one group (the size classes run concurrently on
+ * internal streams, as in normal operation); mode 2 serialises them on the caller's stream and
+ * times every class by itself (diagnostic: slower than normal operation); 0 switches off. */
+#define CUBA_PROFILE_GROUPS 16
 int cuba_profile_enable(cuba_ctx *ctx, int on);
 int cuba_profile_read(cuba_ctx *ctx, double *ms_sum, uint64_t *launches);
 const char *cuba_profile_name(int group);

@@ -387,8 +387,9 @@ static int cmp_shuf(const void *a, const void *b)
 
 /* ------------------------------------------------------------------------------------
  * S5 collisions inside one cell holding slots [lo, hi).
- *   - pairs: A4/A7 per round, order the cell by the key (Philox word 0 keyed by the
- *     persistent pid) << 32 | pid and pair order[2k] with order[2k+1];
+ *   - pairs: A4/A7 per round, order the cell by the key (a Philox word keyed by the
+ *     persistent pid: word rho mod 4 of the call with counter {pid, t, rho div 4, SHUF})
+ *     << 32 | pid and pair order[2k] with order[2k+1];
  *   - P22 of Eq. 3 scaled by cn = n(n-1)/(2 floor(n/2)) so that floor(n/2) tested pairs
  *     carry the rate of all n(n-1)/2 pairs (north_star "(n_cell-1)"; A5 for odd n);
  *   - A6: if the largest possible scaled P (v_rel <= 2) exceeds 1, split the step into R
@@ -409,8 +410,8 @@ static int collide_cell(oracle_state *st, uint32_t c, int64_t lo, int64_t hi, do
     for (int rho = 0; rho < R; ++rho) {
         for (int64_t j = 0; j < n; ++j) {
             uint32_t w[4];
-            draw(st->seed, st->pid[lo + j], st->t, (uint32_t)rho, TAG_SHUF, 0, w);
-            order[j].key = ((uint64_t)w[0] << 32) | (uint64_t)st->pid[lo + j];
+            draw(st->seed, st->pid[lo + j], st->t, (uint32_t)rho >> 2, TAG_SHUF, 0, w);
+            order[j].key = ((uint64_t)w[rho & 3] << 32) | (uint64_t)st->pid[lo + j];
             order[j].slot = lo + j;
         }
         qsort(order, (size_t)n, sizeof(shuf_item), cmp_shuf); /* keys are unique (pid is) */
@@ -574,8 +575,8 @@ void oracle_shuffle_order(uint64_t seed, uint32_t t, uint32_t rho, int64_t n,
     shuf_item *o = (shuf_item *)malloc((size_t)n * sizeof(shuf_item));
     for (int64_t j = 0; j < n; ++j) {
         uint32_t w[4];
-        draw(seed, pids[j], t, rho, TAG_SHUF, 0, w);
-        o[j].key = ((uint64_t)w[0] << 32) | (uint64_t)pids[j];
+        draw(seed, pids[j], t, rho >> 2, TAG_SHUF, 0, w);
+        o[j].key = ((uint64_t)w[rho & 3] << 32) | (uint64_t)pids[j];
         o[j].slot = j;
     }
     qsort(o, (size_t)n, sizeof(shuf_item), cmp_shuf);

@@ -233,12 +233,13 @@ class Cuba:
         m = int(tr.n_pairs)
         return Trace(cell_of_pid, cell[:m], rnd[:m], pa[:m], pb[:m], P[:m], u[:m], dec[:m])
 
-    def profile_enable(self, on=True):
-        _check(lib().cuba_profile_enable(self._h, int(bool(on))))
+    def profile_enable(self, mode=1):
+        """0 off, 1 per-kernel events (collision classes as one concurrent group), 2 classes serialised."""
+        _check(lib().cuba_profile_enable(self._h, int(mode)))
 
     def profile_read(self):
         """{kernel group: (summed device ms, launches)} since profile_enable."""
-        G = 15
+        G = 16
         ms = (c_double * G)()
         cnt = (c_uint64 * G)()
         _check(lib().cuba_profile_read(self._h, ms, cnt))

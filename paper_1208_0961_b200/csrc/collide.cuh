@@ -65,6 +65,13 @@ __device__ __forceinline__ void draw_direction(uint64_t seed, uint32_t pid, uint
     nx = 0.0; ny = 0.0; nz = 1.0;
 }
 
+// Shuffle key of round rho (A7): word rho mod 4 of the call for rounds 4*floor(rho/4)..+3.
+__device__ __forceinline__ uint32_t shuf_word(const U4 &w, int rho)
+{
+    const int q = rho & 3;
+    return q == 0 ? w.x : (q == 1 ? w.y : (q == 2 ? w.z : w.w));
+}
+
 template <int THREADS>
 __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t *s_warp, uint32_t &total)
 {
@@ -125,7 +132,7 @@ __device__ __forceinline__ void collide_cell(const CollideParams &P, uint32_t c,
     for (int rho = 0; rho < R; ++rho) {
         // (a) keys and bucket counts; the arrival slot only serves to park the element
         for (uint32_t j = tid; j < n; j += THREADS) {
-            const uint32_t k = draw(P.seed, spid[j], P.t, (uint32_t)rho, kTagShuf, 0).x;
+            const uint32_t k = shuf_word(draw(P.seed, spid[j], P.t, (uint32_t)rho >> 2, kTagShuf, 0), rho);
             skey[j] = k;
             sord[j] = (IdxT)atomicAdd(&sbkt[__umulhi(k, n)], 1u);
         }
@@ -278,6 +285,7 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
     const uint32_t nb = 2u * n;
     uint16_t *sb16 = reinterpret_cast<uint16_t *>(sbkt);
     double *sS = reinterpret_cast<double *>(skey);   // Mandelstam s of the colliding pairs (skey is dead by then)
+    U4 shuf[ITEMS];                                  // shuffle words of my particles: one Philox call per 4 rounds
 
 #pragma unroll
     for (int it = 0; it < ITEMS; ++it) {
@@ -299,7 +307,8 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
         for (int it = 0; it < ITEMS; ++it) {
             const uint32_t j = tid + it * THREADS;
             if (j < n) {
-                const uint32_t k = draw(P.seed, spid[j], P.t, (uint32_t)rho, kTagShuf, 0).x;
+                if ((rho & 3) == 0) shuf[it] = draw(P.seed, spid[j], P.t, (uint32_t)rho >> 2, kTagShuf, 0);
+                const uint32_t k = shuf_word(shuf[it], rho);
                 skey[j] = k;
                 const uint32_t b = __umulhi(k, nb);
                 const uint32_t sh = (b & 1u) * 16u;
@@ -332,21 +341,33 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
             if (j < n) stmp[(uint32_t)sb16[__umulhi(skey[j], nb)] + (uint32_t)sord[j]] = (uint16_t)j;
         }
         __syncthreads();
-        // (d) final rank = bucket start + number of bucket mates with a smaller (key, pid)
+        // (d) final rank = bucket start + number of bucket mates with a smaller (key, pid).
+        // Buckets hold 1.5 elements on average (own bucket), so the first four slots are
+        // compared in straight-line code on full warps; bigger buckets and equal 32-bit keys
+        // (2^-32 per mate) take the loop.
 #pragma unroll
         for (int it = 0; it < ITEMS; ++it) {
             const uint32_t j = tid + it * THREADS;
             if (j < n) {
                 const uint32_t k = skey[j];
                 const uint32_t b = __umulhi(k, nb);
-                const uint32_t beg = sb16[b], end = sb16[b + 1];
-                uint32_t rank = beg;
-                if (end - beg > 1u) {
+                const uint32_t beg = sb16[b], cnt = (uint32_t)sb16[b + 1] - beg;
+                const uint32_t last = n - 1u;
+                const uint32_t k0 = skey[stmp[beg]];
+                const uint32_t k1 = skey[stmp[min(beg + 1u, last)]];
+                const uint32_t k2 = skey[stmp[min(beg + 2u, last)]];
+                const uint32_t k3 = skey[stmp[min(beg + 3u, last)]];
+                uint32_t rank = beg + (k0 < k ? 1u : 0u) + ((cnt > 1u && k1 < k) ? 1u : 0u) +
+                                ((cnt > 2u && k2 < k) ? 1u : 0u) + ((cnt > 3u && k3 < k) ? 1u : 0u);
+                const uint32_t same = (k0 == k ? 1u : 0u) + ((cnt > 1u && k1 == k) ? 1u : 0u) +
+                                      ((cnt > 2u && k2 == k) ? 1u : 0u) + ((cnt > 3u && k3 == k) ? 1u : 0u);
+                if (cnt > 4u || same > 1u) {
                     const uint32_t id = spid[j];
-                    for (uint32_t q = beg; q < end; ++q) {
+                    rank = beg;
+                    for (uint32_t q = beg; q < beg + cnt; ++q) {
                         const uint32_t jj = stmp[q];
-                        const uint32_t k2 = skey[jj];
-                        rank += (k2 < k || (k2 == k && spid[jj] < id)) ? 1u : 0u;
+                        const uint32_t kk = skey[jj];
+                        rank += (kk < k || (kk == k && spid[jj] < id)) ? 1u : 0u;
                     }
                 }
                 sord[rank] = (uint16_t)j;   // arrival slots in sord are dead after (c)
@@ -485,7 +506,7 @@ k_collide(CollideParams P)
     flush_counters<THREADS>(P, n_pairs, n_coll, n_near);
 }
 
-constexpr size_t collide_smem_bytes(int cap) { return (size_t)cap * 48 + 16; }
+constexpr size_t collide_smem_bytes(int cap) { return (size_t)cap * 48 + 32; }
 
 // Overflow class: cells larger than the biggest shared-memory class.  Same routine, scratch
 // in global memory (momenta are updated in place in the particle store; the cached energy

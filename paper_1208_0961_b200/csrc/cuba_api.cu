@@ -107,6 +107,9 @@ struct cuba_ctx {
     int cur;
     int grid_cls[kSmemClasses], grid_o, grid_hist, grid_scat;
     double *h_obs;       // pinned staging for observables
+    cudaStream_t cls_stream[kNumClasses] = {};   // the collision classes run concurrently, fenced into `stream`
+    cudaEvent_t ev_fork = nullptr, ev_join[kNumClasses] = {};
+    int prof_mode = 0;   // 0 off, 1 events per kernel (collision classes as one concurrent group), 2 classes serialised
     bool prof_on = false;
     std::vector<cudaEvent_t> prof_pool;          // reused events
     std::vector<std::pair<cudaEvent_t, int>> prof_log;   // (event, group) in stream order; group -1 = step start
@@ -171,7 +174,7 @@ static int sync_and_check(cuba_ctx *ctx)
     return device_flags_to_error(f);
 }
 
-enum { G_MEMSET = 0, G_STREAM_HIST, G_GATHER, G_SCAN, G_CELL_START, G_CARRY, G_SCATTER, G_COLLIDE0 };
+enum { G_MEMSET = 0, G_STREAM_HIST, G_GATHER, G_SCAN, G_CELL_START, G_CARRY, G_SCATTER, G_COLLIDE_ALL, G_COLLIDE0 };
 static_assert(G_COLLIDE0 + kNumClasses == CUBA_PROFILE_GROUPS, "profile groups");
 
 static void prof_mark(cuba_ctx *ctx, int group)
@@ -236,8 +239,22 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
                       ctx->at<uint32_t>(lay.pidB)};
     ctx->cur = 0;
     ctx->h_obs = nullptr;
-    auto fail = [&](int code) { if (ctx->h_obs) cudaFreeHost(ctx->h_obs); delete ctx; return code; };
+    auto fail = [&](int code) {
+        if (ctx->h_obs) cudaFreeHost(ctx->h_obs);
+        if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+        for (int k = 0; k < kNumClasses; ++k) {
+            if (ctx->cls_stream[k]) cudaStreamDestroy(ctx->cls_stream[k]);
+            if (ctx->ev_join[k]) cudaEventDestroy(ctx->ev_join[k]);
+        }
+        delete ctx;
+        return code;
+    };
     if (!cuda_ok(cudaMallocHost(&ctx->h_obs, (4 + kObsMaxSlabs) * sizeof(double)), "cudaMallocHost")) return fail(CUBA_ERR_CUDA);
+    if (!cuda_ok(cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming), "cudaEventCreate")) return fail(CUBA_ERR_CUDA);
+    for (int k = 0; k < kNumClasses; ++k) {
+        if (!cuda_ok(cudaStreamCreateWithFlags(&ctx->cls_stream[k], cudaStreamNonBlocking), "cudaStreamCreate")) return fail(CUBA_ERR_CUDA);
+        if (!cuda_ok(cudaEventCreateWithFlags(&ctx->ev_join[k], cudaEventDisableTiming), "cudaEventCreate")) return fail(CUBA_ERR_CUDA);
+    }
 
 #define CUBA_OCC(K, T, I, C, MB)                                                                                          \
     if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, false>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]); \
@@ -302,6 +319,11 @@ void cuba_destroy(cuba_ctx *ctx)
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
     if (ctx->h_obs) cudaFreeHost(ctx->h_obs);
+    for (int k = 0; k < kNumClasses; ++k) {
+        if (ctx->cls_stream[k]) { cudaStreamSynchronize(ctx->cls_stream[k]); cudaStreamDestroy(ctx->cls_stream[k]); }
+        if (ctx->ev_join[k]) cudaEventDestroy(ctx->ev_join[k]);
+    }
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     for (auto &pe : ctx->prof_log) cudaEventDestroy(pe.first);
     for (auto e : ctx->prof_pool) cudaEventDestroy(e);
     delete ctx;
@@ -334,19 +356,38 @@ static int launch_collide(cuba_ctx *ctx, double base, const TraceDev *td)
     uint32_t *zero = ctx->at<uint32_t>(lay.zero);
     uint32_t *lists = ctx->at<uint32_t>(lay.class_list);
     auto cls = [&](int k) { P.list = lists + (size_t)k * ctx->g.ncells; P.list_count = zero + k; P.work = zero + 8 + k; };
-    cudaStream_t st = ctx->stream;
+    // The classes are independent (disjoint cells): fork them onto their own streams so that
+    // small classes fill the tail of the big ones, then join back into the caller's stream.
+    // Profile mode 2 serialises them on the caller's stream to time each class by itself.
+    const bool serial = ctx->prof_mode == 2;
+    cudaStream_t main = ctx->stream;
+    if (!serial) CU(cudaEventRecord(ctx->ev_fork, main));
 #define CUBA_LAUNCH(K, T, I, C, MB)                                                              \
-    cls(K);                                                                                      \
-    k_collide<T, I, C, MB, TRACE><<<ctx->grid_cls[K], T, collide_smem_bytes(C), st>>>(P);        \
-    LAUNCHED();                                                                                  \
-    prof_mark(ctx, G_COLLIDE0 + K);
-    CUBA_FOR_EACH_CLASS(CUBA_LAUNCH)
+    {                                                                                            \
+        cudaStream_t st = serial ? main : ctx->cls_stream[K];                                    \
+        if (!serial) CU(cudaStreamWaitEvent(st, ctx->ev_fork, 0));                               \
+        cls(K);                                                                                  \
+        k_collide<T, I, C, MB, TRACE><<<ctx->grid_cls[K], T, collide_smem_bytes(C), st>>>(P);    \
+        LAUNCHED();                                                                              \
+        if (serial) prof_mark(ctx, G_COLLIDE0 + K);                                              \
+        else { CU(cudaEventRecord(ctx->ev_join[K], st)); CU(cudaStreamWaitEvent(main, ctx->ev_join[K], 0)); } \
+    }
+    // biggest cells first: they are the long poles
+#define CUBA_REV(X) X(6, 1024, 5, 4544, 1) X(5, 512, 4, 2048, 2) X(4, 352, 4, 1408, 3) X(3, 224, 4, 896, 4) X(2, 128, 4, 512, 8) X(1, 64, 4, 256, 12) X(0, 32, 4, 128, 16)
+    CUBA_REV(CUBA_LAUNCH)
+#undef CUBA_REV
 #undef CUBA_LAUNCH
-    cls(kSmemClasses);
-    k_collide_overflow<TRACE><<<ctx->grid_o, 1024, 0, st>>>(P, reinterpret_cast<unsigned long long *>(zero + 16),
-                                                           ctx->at<double>(lay.arenaE));
-    LAUNCHED();
-    prof_mark(ctx, G_COLLIDE0 + kSmemClasses);
+    {
+        cudaStream_t st = serial ? main : ctx->cls_stream[kSmemClasses];
+        if (!serial) CU(cudaStreamWaitEvent(st, ctx->ev_fork, 0));
+        cls(kSmemClasses);
+        k_collide_overflow<TRACE><<<ctx->grid_o, 1024, 0, st>>>(P, reinterpret_cast<unsigned long long *>(zero + 16),
+                                                               ctx->at<double>(lay.arenaE));
+        LAUNCHED();
+        if (serial) prof_mark(ctx, G_COLLIDE0 + kSmemClasses);
+        else { CU(cudaEventRecord(ctx->ev_join[kSmemClasses], st)); CU(cudaStreamWaitEvent(main, ctx->ev_join[kSmemClasses], 0)); }
+    }
+    if (!serial) prof_mark(ctx, G_COLLIDE_ALL);
     return CUBA_OK;
 }
 
@@ -555,6 +596,7 @@ const char *cuba_profile_name(int group)
 {
     static const char *names[CUBA_PROFILE_GROUPS] = {
         "memset_cnt", "k_stream_hist", "k_gather", "k_scan_blocks", "k_cell_start", "k_carry", "k_scatter",
+        "k_collide (all classes, concurrent)",
 #define CUBA_NAME(K, T, I, C, MB) "k_collide<T=" #T ",cap=" #C ">",
         CUBA_FOR_EACH_CLASS(CUBA_NAME)
 #undef CUBA_NAME
@@ -569,6 +611,7 @@ int cuba_profile_enable(cuba_ctx *ctx, int on)
     for (auto &pe : ctx->prof_log) ctx->prof_pool.push_back(pe.first);
     ctx->prof_log.clear();
     ctx->prof_on = on != 0;
+    ctx->prof_mode = on;
     return CUBA_OK;
 }
 
