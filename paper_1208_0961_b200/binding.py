@@ -66,7 +66,8 @@ class Trace:
 
 
 def lib_path() -> str:
-    return os.path.join(_HERE, "libcuba.so")
+    """In-tree library; CUBA_LIB_PATH overrides it (used to compare experimental builds)."""
+    return os.environ.get("CUBA_LIB_PATH") or os.path.join(_HERE, "libcuba.so")
 
 
 _lib = None

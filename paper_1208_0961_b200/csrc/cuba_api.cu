@@ -36,14 +36,21 @@ bool cuda_ok(cudaError_t e, const char *what)
 // in particles, min CTAs per SM).  A cell goes to the first class whose capacity holds it; a
 // cell beyond the last capacity goes to the global-memory overflow kernel.  Thread counts are
 // about a quarter of the capacity so that every thread owns <= 4 particles and <= 2 pairs.
+// Listed (and launched) biggest first: the big cells are the long poles.
+#ifndef CUBA_C4_T   // class 4 (the ~1350-particle hot cells of the 25M-particle Riemann problem) is tunable at build time
+#define CUBA_C4_T 256
+#define CUBA_C4_I 6
+#define CUBA_C4_CAP 1536
+#define CUBA_C4_MB 3
+#endif
 #define CUBA_FOR_EACH_CLASS(X) \
-    X(0, 32, 4, 128, 16)       \
-    X(1, 64, 4, 256, 12)       \
-    X(2, 128, 4, 512, 8)       \
-    X(3, 224, 4, 896, 4)       \
-    X(4, 352, 4, 1408, 3)      \
+    X(6, 1024, 5, 4544, 1)     \
     X(5, 512, 4, 2048, 2)      \
-    X(6, 1024, 5, 4544, 1)
+    X(4, CUBA_C4_T, CUBA_C4_I, CUBA_C4_CAP, CUBA_C4_MB) \
+    X(3, 224, 4, 896, 4)       \
+    X(2, 128, 4, 512, 8)       \
+    X(1, 64, 4, 256, 12)       \
+    X(0, 32, 4, 128, 16)
 constexpr int kSmemClasses = 7;
 static_assert(kSmemClasses + 1 == kNumClasses, "class table");
 
@@ -372,10 +379,7 @@ static int launch_collide(cuba_ctx *ctx, double base, const TraceDev *td)
         if (serial) prof_mark(ctx, G_COLLIDE0 + K);                                              \
         else { CU(cudaEventRecord(ctx->ev_join[K], st)); CU(cudaStreamWaitEvent(main, ctx->ev_join[K], 0)); } \
     }
-    // biggest cells first: they are the long poles
-#define CUBA_REV(X) X(6, 1024, 5, 4544, 1) X(5, 512, 4, 2048, 2) X(4, 352, 4, 1408, 3) X(3, 224, 4, 896, 4) X(2, 128, 4, 512, 8) X(1, 64, 4, 256, 12) X(0, 32, 4, 128, 16)
-    CUBA_REV(CUBA_LAUNCH)
-#undef CUBA_REV
+    CUBA_FOR_EACH_CLASS(CUBA_LAUNCH)
 #undef CUBA_LAUNCH
     {
         cudaStream_t st = serial ? main : ctx->cls_stream[kSmemClasses];
@@ -596,11 +600,13 @@ const char *cuba_profile_name(int group)
 {
     static const char *names[CUBA_PROFILE_GROUPS] = {
         "memset_cnt", "k_stream_hist", "k_gather", "k_scan_blocks", "k_cell_start", "k_carry", "k_scatter",
-        "k_collide (all classes, concurrent)",
-#define CUBA_NAME(K, T, I, C, MB) "k_collide<T=" #T ",cap=" #C ">",
-        CUBA_FOR_EACH_CLASS(CUBA_NAME)
+        "k_collide (all classes, concurrent)"};
+#define CUBA_STR2(x) #x
+#define CUBA_STR(x) CUBA_STR2(x)
+#define CUBA_NAME(K, T, I, C, MB) names[G_COLLIDE0 + K] = "k_collide<T=" CUBA_STR(T) ",cap=" CUBA_STR(C) ">";
+    CUBA_FOR_EACH_CLASS(CUBA_NAME)
 #undef CUBA_NAME
-        "k_collide_overflow"};
+    names[G_COLLIDE0 + kSmemClasses] = "k_collide_overflow";
     return (group >= 0 && group < CUBA_PROFILE_GROUPS) ? names[group] : "?";
 }
 
