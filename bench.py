@@ -146,6 +146,19 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def reduce_over_ranks(dist, device, ms, e2e_s, n, pairs, launches):
+    """Whole-job aggregation for N independent replicas: the time is the MAX over ranks, the
+    work (particles, pair evaluations, launches) the SUM.  `dist` is torch.distributed or None."""
+    if dist is None:
+        return ms, e2e_s, float(n), float(pairs), int(launches)
+    import torch
+    t = torch.tensor([ms, e2e_s], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    s = torch.tensor([float(n), float(pairs), float(launches)], device=device, dtype=torch.float64)
+    dist.all_reduce(s, op=dist.ReduceOp.SUM)
+    return float(t[0]), float(t[1]), float(s[0]), float(s[1]), int(s[2])
+
+
 def workloads_name(config):
     return {0: "configs[0] thermal box 8^3 fm^3, r_test=2 (13.8k particles)",
             1: "configs[1] Riemann 32^3 fm^3, r_test=10 (2.49M particles)",
@@ -255,17 +268,10 @@ def main():
     sim.close()
 
     # ---- reduce over ranks: max time, summed work --------------------------------------
-    if world > 1:
-        t = torch.tensor([ms, e2e["s"] if e2e else 0.0], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t[0])
-        if e2e:
-            e2e["s"] = float(t[1])
-        s = torch.tensor([float(n), float(pairs), float(launches)], device=dev, dtype=torch.float64)
-        dist.all_reduce(s, op=dist.ReduceOp.SUM)
-        n_total, pairs_total, launches = float(s[0]), float(s[1]), int(s[2])
-    else:
-        n_total, pairs_total = float(n), float(pairs)
+    ms, e2e_s, n_total, pairs_total, launches = reduce_over_ranks(
+        dist if world > 1 else None, dev, ms, e2e["s"] if e2e else 0.0, n, pairs, launches)
+    if e2e:
+        e2e["s"] = e2e_s
     sampler.stop_flag = True
 
     if rank == 0:
