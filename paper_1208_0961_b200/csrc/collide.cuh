@@ -18,6 +18,7 @@ namespace cuba {
 
 struct CollideParams {
     uint64_t seed;
+    uint32_t rk[20];      // Philox round keys: rk[2r] = seed_lo + r*0x9E3779B9, rk[2r+1] = seed_hi + r*0xBB67AE85
     uint32_t t;           // global step index
     double base;          // sigma*dt/(r_test*V_cell): Eq. 3 without v_rel
     const uint32_t *cell_start;
@@ -41,6 +42,21 @@ struct CollideParams {
 __device__ __forceinline__ double u53(uint32_t w0, uint32_t w1)
 {
     return ((double)(w0 >> 5) * 67108864.0 + (double)(w1 >> 6)) * (1.0 / 9007199254740992.0);
+}
+
+// draw() with the key schedule taken from the kernel parameters (constant bank operands):
+// the same function of (seed, id, t, rho, tag, sub), without 18 key additions per call.
+__device__ __forceinline__ U4 drawk(const CollideParams &P, uint32_t id, uint32_t rho, uint32_t tag, uint32_t sub)
+{
+    uint32_t c0 = id, c1 = P.t, c2 = rho, c3 = (tag << 16) | sub;
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ P.rk[2 * r], n2 = hi0 ^ c3 ^ P.rk[2 * r + 1];
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    }
+    return U4{c0, c1, c2, c3};
 }
 
 // Marsaglia disc rejection (A11): words (x,y) of call m>>1 for even attempts, (z,w) for odd.
@@ -219,23 +235,51 @@ __device__ __forceinline__ void collide_cell(const CollideParams &P, uint32_t c,
     if (tid == 0) atomicAdd(&P.counters[2], (unsigned long long)R);
 }
 
-// One pair: Eq. 3 decision.  Returns hit; s (Mandelstam) through s_out.
-__device__ __forceinline__ bool pair_decide(const CollideParams &P, uint32_t ida, uint32_t rho, double scale,
-                                            double pax, double pay, double paz, double Ea,
-                                            double pbx, double pby, double pbz, double Eb,
-                                            double &s_out, double &prob_out, double &u_out)
+// ---- shared-memory classes ------------------------------------------------------------
+// Same results as the generic routine above, organised for issue efficiency on sm_100a:
+//   * every phase works on groups of G items per thread with clamped, unguarded loads so
+//     that the G Philox / fp64 chains of a thread interleave (only stores are predicated);
+//   * 2n buckets with 16-bit counters packed two per word; the keys themselves are parked in
+//     bucket order, so an element ranks itself from five consecutive words (no indirection)
+//     and buckets with more than four elements or equal 32-bit keys take a rare slow path;
+//   * the Eq. 3 decision compares u*(EaEb)^2 with |d|^2*scale/2 (no division); only a
+//     decision inside a 4e-9 band around the threshold is redone with the exact operation
+//     order of the oracle, so the decisions (and the near-threshold counter, A16) are the
+//     oracle's bit for bit; the division for s is paid by the pairs that collide;
+//   * hits are compacted per warp, and a warp scatters its own hits right away: pairs are
+//     disjoint, so no block barrier separates decision and scatter;
+//   * the energy of an outgoing momentum is only recomputed when another round will read it.
+// Five block barriers per round.
+
+// 53-bit uniform from two Philox words, same value as u53(): both halves are exact integers
+// below 2^27 placed in the mantissa of 2^52, so every operation below is exact.
+__device__ __forceinline__ double u53_bits(uint32_t w0, uint32_t w1)
 {
-    const double ee = Ea * Eb;
-    const double dx = Eb * pax - Ea * pbx;
-    const double dy = Eb * pay - Ea * pby;
-    const double dz = Eb * paz - Ea * pbz;
-    const double s = ((dx * dx + dy * dy) + dz * dz) / ee;   // (p_a+p_b)^2, A9
-    const double vrel = 0.5 * (s / ee);                       // s/(2 E_a E_b)
-    const double prob = vrel * scale;                         // Eq. 3 * cn/R
-    const U4 w = draw(P.seed, ida, P.t, rho, kTagDec, 0);
-    const double u = u53(w.x, w.y);
-    s_out = s; prob_out = prob; u_out = u;
-    return u < prob;
+    const double hi = __hiloint2double(0x43300000, (int)(w0 >> 5)) - 4503599627370496.0;
+    const double lo = __hiloint2double(0x43300000, (int)(w1 >> 6)) - 4503599627370496.0;
+    return (hi * 67108864.0 + lo) * (1.0 / 9007199254740992.0);
+}
+
+// Marsaglia disc rejection (A11) with the key schedule from the parameters.
+__device__ __forceinline__ void draw_direction_k(const CollideParams &P, uint32_t pid, uint32_t rho,
+                                                 double &nx, double &ny, double &nz)
+{
+    for (uint32_t call = 0; call < 65536u; ++call) {
+        const U4 w = drawk(P, pid, rho, kTagDir, call);
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+            const uint32_t wa = half ? w.z : w.x, wb = half ? w.w : w.y;
+            const double a = ((double)wa + 0.5) * (1.0 / 2147483648.0) - 1.0;
+            const double b = ((double)wb + 0.5) * (1.0 / 2147483648.0) - 1.0;
+            const double q = a * a + b * b;
+            if (q < 1.0) {
+                const double h = sqrt(1.0 - q);
+                nx = (2.0 * a) * h; ny = (2.0 * b) * h; nz = 1.0 - 2.0 * q;
+                return;
+            }
+        }
+    }
+    nx = 0.0; ny = 0.0; nz = 1.0;
 }
 
 // Boost to the CM frame, isotropic direction, boost back (closed form A10).
@@ -245,7 +289,7 @@ __device__ __forceinline__ void pair_scatter(const CollideParams &P, uint32_t id
                                              double q[6])
 {
     double nx, ny, nz;
-    draw_direction(P.seed, ida, P.t, rho, nx, ny, nz);
+    draw_direction_k(P, ida, rho, nx, ny, nz);
     const double rs = sqrt(s);
     const double Pvx = pax + pbx, Pvy = pay + pby, Pvz = paz + pbz;
     const double Et = Ea + Eb;
@@ -260,181 +304,318 @@ __device__ __forceinline__ void pair_scatter(const CollideParams &P, uint32_t id
     q[5] = 0.5 * (Pvz * f2 - rs * nz);
 }
 
-// Shared-memory classes: THREADS threads, at most THREADS*ITEMS particles, compile-time trip
-// counts.  Differences to the generic routine, all invisible in the results:
-//   * 2n buckets with 16-bit counters packed two per word (expected occupancy 1/2);
-//   * pairs that collide are compacted into a list first, so the expensive scatter path runs
-//     on full warps instead of on the ~25 % of lanes that hit in a round.
-template <int THREADS, int ITEMS, bool TRACE>
+// Exclusive block scan with one barrier; s_warp is next written a round (several barriers) later.
+template <int THREADS>
+__device__ __forceinline__ uint32_t block_exclusive_scan_1b(uint32_t v, uint32_t *s_warp)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    uint32_t inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (THREADS == 32) return inc - v;
+    if (lane == 31) s_warp[wid] = inc;
+    __syncthreads();
+    uint32_t w = (lane < THREADS / 32) ? s_warp[lane] : 0u;
+    uint32_t winc = w;
+#pragma unroll
+    for (int o = 1; o < THREADS / 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, winc, o);
+        if (lane >= o) winc += t;
+    }
+    return __shfl_sync(0xFFFFFFFFu, winc - w, wid) + inc - v;
+}
+
+#ifndef CUBA_FORCE_SLOW_PATHS   // test builds set this to 1: every element / pair takes the rare paths
+#define CUBA_FORCE_SLOW_PATHS 0
+#endif
+
+// Rare path of the in-bucket ranking: buckets with more than four elements, or equal 32-bit
+// keys (then the pid decides, A7; the keys of the other particles are recomputed).
+__device__ __noinline__ uint32_t slow_rank(uint64_t seed, uint32_t t, const uint32_t *spark, const uint32_t *spid,
+                                           uint32_t n, uint32_t nb, uint32_t j, uint32_t k, uint32_t beg, int rho)
+{
+    const uint32_t b = __umulhi(k, nb);
+    uint32_t rank = beg, same = 0;
+    for (uint32_t q = beg; q < n; ++q) {
+        const uint32_t kk = spark[q];
+        if (__umulhi(kk, nb) != b) break;
+        rank += kk < k ? 1u : 0u;
+        same += kk == k ? 1u : 0u;
+    }
+    if (CUBA_FORCE_SLOW_PATHS || same > 1u) {
+        const uint32_t id = spid[j];
+        for (uint32_t i = 0; i < n; ++i) {
+            const uint32_t id2 = spid[i];
+            if (id2 < id && shuf_word(draw(seed, id2, t, (uint32_t)rho >> 2, kTagShuf, 0), rho) == k) rank += 1u;
+        }
+    }
+    return rank;
+}
+
+// Rare path of the Eq. 3 decision: the exact operation order of the oracle.
+// Returns bit 0: hit, bit 1: |u - P| <= 1e-12 (A16).
+__device__ __noinline__ uint32_t exact_decision(double dd, double ee, double u, double scale)
+{
+    const double s = dd / ee;                 // (p_a+p_b)^2, A9
+    const double vrel = 0.5 * (s / ee);       // s/(2 E_a E_b)
+    const double prob = vrel * scale;         // Eq. 3 * cn/R
+    return (u < prob ? 1u : 0u) | (fabs(u - prob) <= 1e-12 ? 2u : 0u);
+}
+
+// Per-CTA statistics in shared memory: [0] pairs, [1] collisions, [2] near-threshold decisions;
+// and the constants of the current cell that are only needed at a few places (kept out of
+// registers across the register-hungry phases).
+struct CtaStats {
+    unsigned long long v[3];
+    double scale, hscale;     // Eq. 3 factor cn*base/R of the current cell, and half of it
+    uint32_t lo;              // first slot of the current cell
+};
+
+template <int THREADS, int ITEMS, int G, bool TRACE>
 __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32_t c, uint32_t lo, uint32_t n,
                                                   double *sp0, double *sp1, double *sp2, double *sE,
-                                                  uint32_t *spid, uint32_t *skey, uint32_t *sbkt,
-                                                  uint16_t *sord, uint16_t *stmp, uint32_t *s_warp,
-                                                  uint32_t *s_nhit,
-                                                  unsigned long long &n_pairs, unsigned long long &n_coll,
-                                                  unsigned long long &n_near)
+                                                  uint32_t *spid, uint32_t *spark, uint32_t *sbkt,
+                                                  uint16_t *sord, uint32_t *s_warp, CtaStats *stats)
 {
-    const int tid = threadIdx.x, lane = tid & 31;
+    static_assert(ITEMS % G == 0, "items are processed in groups of G");
+    constexpr int NG = ITEMS / G;
+    constexpr int PITEMS = (ITEMS + 1) / 2;          // pairs per thread
+    constexpr int SCAN = ITEMS | 1;                  // words per thread in the scan (odd stride: no bank conflicts)
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const double cn = (n & 1u) ? (double)n : (double)(n - 1u);
     const double pmax = (2.0 * cn) * P.base;
     int R;
     if (!(pmax <= 64.0)) { if (tid == 0) atomicOr(P.flags, kFlagRounds); R = 64; }
     else R = (pmax <= 1.0) ? 1 : (int)ceil(pmax);
-    const double scale = (cn * P.base) / (double)R;
-    const uint32_t npairs = n >> 1;
-    const uint32_t nb = 2u * n;
+    if (tid == 0) {
+        const double scale = (cn * P.base) / (double)R;
+        stats->scale = scale; stats->hscale = 0.5 * scale; stats->lo = lo;
+    }
+    const uint32_t npairs = n >> 1, nb = 2u * n, last = n - 1u;
     uint16_t *sb16 = reinterpret_cast<uint16_t *>(sbkt);
-    double *sS = reinterpret_cast<double *>(skey);   // Mandelstam s of the colliding pairs (skey is dead by then)
-    U4 shuf[ITEMS];                                  // shuffle words of my particles: one Philox call per 4 rounds
+    uint16_t *shit = reinterpret_cast<uint16_t *>(spark) + wid * (PITEMS * 32);   // this warp's hit list
+    uint32_t key[ITEMS], aux[ITEMS], keep[ITEMS];
 
+    // ---- stage the cell: momenta, energies, pids; clear the bucket counters -----------------
 #pragma unroll
-    for (int it = 0; it < ITEMS; ++it) {
-        const uint32_t j = tid + it * THREADS;
-        if (j < n) {
-            const double a = P.px[lo + j], b = P.py[lo + j], cc = P.pz[lo + j];
-            sp0[j] = a; sp1[j] = b; sp2[j] = cc;
-            sE[j] = energy(a, b, cc);
-            spid[j] = P.pid[lo + j];
-            sbkt[j] = 0;
+    for (int g = 0; g < NG; ++g) {
+        if ((uint32_t)(g * G * THREADS) >= n) break;
+        double a[G], b[G], cc[G];
+        uint32_t id[G];
+#pragma unroll
+        for (int i = 0; i < G; ++i) {
+            const uint32_t jc = lo + min((uint32_t)(tid + (g * G + i) * THREADS), last);
+            a[i] = P.px[jc]; b[i] = P.py[jc]; cc[i] = P.pz[jc]; id[i] = P.pid[jc];
+        }
+#pragma unroll
+        for (int i = 0; i < G; ++i) {
+            const uint32_t j = tid + (g * G + i) * THREADS;
+            const double e = energy(a[i], b[i], cc[i]);
+            if (j < n) { sp0[j] = a[i]; sp1[j] = b[i]; sp2[j] = cc[i]; sE[j] = e; spid[j] = id[i]; sbkt[j] = 0; }
         }
     }
-    if (tid == 0) { sbkt[n] = 0; *s_nhit = 0; }
     __syncthreads();
 
+    uint32_t warp_hits = 0;
     for (int rho = 0; rho < R; ++rho) {
-        // (a) keys, bucket counts; the arrival slot only serves to park the element
+        // (a) shuffle keys (A7: word rho mod 4 of the call for rounds 4*(rho div 4)..+3; one call
+        // serves two rounds, the second word is kept) and bucket counts
 #pragma unroll
-        for (int it = 0; it < ITEMS; ++it) {
-            const uint32_t j = tid + it * THREADS;
-            if (j < n) {
-                if ((rho & 3) == 0) shuf[it] = draw(P.seed, spid[j], P.t, (uint32_t)rho >> 2, kTagShuf, 0);
-                const uint32_t k = shuf_word(shuf[it], rho);
-                skey[j] = k;
-                const uint32_t b = __umulhi(k, nb);
+        for (int g = 0; g < NG; ++g) {
+            if ((uint32_t)(g * G * THREADS) >= n) break;
+            if ((rho & 1) == 0) {
+#pragma unroll
+                for (int i = 0; i < G; ++i) {
+                    const int it = g * G + i;
+                    const uint32_t jc = min((uint32_t)(tid + it * THREADS), last);
+                    const U4 w = drawk(P, spid[jc], (uint32_t)rho >> 2, kTagShuf, 0);
+                    key[it] = (rho & 2) ? w.z : w.x;
+                    keep[it] = (rho & 2) ? w.w : w.y;
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < G; ++i) key[g * G + i] = keep[g * G + i];
+            }
+#pragma unroll
+            for (int i = 0; i < G; ++i) {
+                const int it = g * G + i;
+                const uint32_t j = tid + it * THREADS;
+                const uint32_t b = __umulhi(key[it], nb);
                 const uint32_t sh = (b & 1u) * 16u;
-                const uint32_t old = atomicAdd(&sbkt[b >> 1], 1u << sh);
-                sord[j] = (uint16_t)((old >> sh) & 0xFFFFu);
+                aux[it] = 0;
+                if (j < n) aux[it] = (atomicAdd(&sbkt[b >> 1], 1u << sh) >> sh) & 0xFFFFu;   // arrival slot
             }
         }
         __syncthreads();
-        // (b) exclusive scan of the 2n counters (n words), contiguous chunk of words per thread
+        // (b) exclusive scan of the 2n counters (n words), a contiguous chunk of words per thread
         {
-            const uint32_t chunk = (n + THREADS - 1) / THREADS;
+            const uint32_t chunk = ((n + THREADS - 1) / THREADS) | 1u;
             const uint32_t w0 = min(n, tid * chunk), w1 = min(n, w0 + chunk);
-            uint32_t sum = 0;
-            for (uint32_t w = w0; w < w1; ++w) { const uint32_t v = sbkt[w]; sum += (v & 0xFFFFu) + (v >> 16); }
-            uint32_t total;
-            uint32_t run = block_exclusive_scan<THREADS>(sum, s_warp, total);
-            for (uint32_t w = w0; w < w1; ++w) {
-                const uint32_t v = sbkt[w];
-                const uint32_t mid = run + (v & 0xFFFFu);
-                sbkt[w] = run | (mid << 16);
-                run = mid + (v >> 16);
+            uint32_t v[SCAN], sum = 0;
+#pragma unroll
+            for (int q = 0; q < SCAN; ++q) {
+                v[q] = (w0 + q < w1) ? sbkt[w0 + q] : 0u;
+                sum += (v[q] & 0xFFFFu) + (v[q] >> 16);
             }
-            if (tid == 0) sbkt[n] = n;   // start of the sentinel bucket 2n
+            uint32_t run = block_exclusive_scan_1b<THREADS>(sum, s_warp);
+#pragma unroll
+            for (int q = 0; q < SCAN; ++q) {
+                const uint32_t mid = run + (v[q] & 0xFFFFu);
+                if (w0 + q < w1) sbkt[w0 + q] = run | (mid << 16);
+                run = mid + (v[q] >> 16);
+            }
         }
         __syncthreads();
-        // (c) park element j at its arrival slot inside its bucket
+        // (c) park the key at bucket start + arrival slot; four sentinels behind the last key
 #pragma unroll
-        for (int it = 0; it < ITEMS; ++it) {
-            const uint32_t j = tid + it * THREADS;
-            if (j < n) stmp[(uint32_t)sb16[__umulhi(skey[j], nb)] + (uint32_t)sord[j]] = (uint16_t)j;
+        for (int g = 0; g < NG; ++g) {
+            if ((uint32_t)(g * G * THREADS) >= n) break;
+#pragma unroll
+            for (int i = 0; i < G; ++i) {
+                const int it = g * G + i;
+                const uint32_t j = tid + it * THREADS;
+                const uint32_t beg = sb16[__umulhi(key[it], nb)];
+                if (j < n) spark[beg + aux[it]] = key[it];
+                aux[it] = (j < n) ? beg : 0u;
+            }
+        }
+        if (tid < 4) spark[n + tid] = 0xFFFFFFFFu;
+        __syncthreads();
+        // (d) rank = bucket start + number of bucket mates with a smaller key.  Keys beyond the
+        // bucket are larger (the bucket index is monotone in the key), so four words decide a
+        // bucket of up to four; the fifth tells whether the bucket is bigger.
+#pragma unroll
+        for (int g = 0; g < NG; ++g) {
+            if ((uint32_t)(g * G * THREADS) >= n) break;
+            uint32_t rank[G];
+            bool slow[G];
+#pragma unroll
+            for (int i = 0; i < G; ++i) {
+                const int it = g * G + i;
+                const uint32_t k = key[it], beg = aux[it];
+                const uint32_t k0 = spark[beg], k1 = spark[beg + 1], k2 = spark[beg + 2], k3 = spark[beg + 3],
+                               k4 = spark[beg + 4];
+                rank[i] = beg + (k0 < k ? 1u : 0u) + (k1 < k ? 1u : 0u) + (k2 < k ? 1u : 0u) + (k3 < k ? 1u : 0u);
+                const uint32_t same = (k0 == k ? 1u : 0u) + (k1 == k ? 1u : 0u) + (k2 == k ? 1u : 0u) + (k3 == k ? 1u : 0u);
+                slow[i] = (tid + it * THREADS < n) &&
+                          (CUBA_FORCE_SLOW_PATHS || same != 1u || __umulhi(k4, nb) == __umulhi(k, nb));
+            }
+            bool any = false;
+#pragma unroll
+            for (int i = 0; i < G; ++i) any = any || slow[i];
+            if (any) {
+#pragma unroll
+                for (int i = 0; i < G; ++i)
+                    if (slow[i]) rank[i] = slow_rank(P.seed, P.t, spark, spid, n, nb, tid + (g * G + i) * THREADS,
+                                                     key[g * G + i], aux[g * G + i], rho);
+            }
+#pragma unroll
+            for (int i = 0; i < G; ++i) {
+                const uint32_t j = tid + (g * G + i) * THREADS;
+                if (j < n) {
+                    sord[rank[i]] = (uint16_t)j;
+                    sbkt[j] = 0;                 // the counters are free: clear them for the next round
+                }
+            }
         }
         __syncthreads();
-        // (d) final rank = bucket start + number of bucket mates with a smaller (key, pid).
-        // Buckets hold 1.5 elements on average (own bucket), so the first four slots are
-        // compared in straight-line code on full warps; bigger buckets and equal 32-bit keys
-        // (2^-32 per mate) take the loop.
+        // (e1) pair order[2k] with order[2k+1]: Eq. 3 decision; this warp's hits go to its list
+        uint32_t nh = 0;
+        {
+            const double scale = *reinterpret_cast<volatile double *>(&stats->scale);
+            const double hscale = *reinterpret_cast<volatile double *>(&stats->hscale);
+            double dd[PITEMS], ee[PITEMS], u[PITEMS];
+            uint32_t ida[PITEMS];
 #pragma unroll
-        for (int it = 0; it < ITEMS; ++it) {
-            const uint32_t j = tid + it * THREADS;
-            if (j < n) {
-                const uint32_t k = skey[j];
-                const uint32_t b = __umulhi(k, nb);
-                const uint32_t beg = sb16[b], cnt = (uint32_t)sb16[b + 1] - beg;
-                const uint32_t last = n - 1u;
-                const uint32_t k0 = skey[stmp[beg]];
-                const uint32_t k1 = skey[stmp[min(beg + 1u, last)]];
-                const uint32_t k2 = skey[stmp[min(beg + 2u, last)]];
-                const uint32_t k3 = skey[stmp[min(beg + 3u, last)]];
-                uint32_t rank = beg + (k0 < k ? 1u : 0u) + ((cnt > 1u && k1 < k) ? 1u : 0u) +
-                                ((cnt > 2u && k2 < k) ? 1u : 0u) + ((cnt > 3u && k3 < k) ? 1u : 0u);
-                const uint32_t same = (k0 == k ? 1u : 0u) + ((cnt > 1u && k1 == k) ? 1u : 0u) +
-                                      ((cnt > 2u && k2 == k) ? 1u : 0u) + ((cnt > 3u && k3 == k) ? 1u : 0u);
-                if (cnt > 4u || same > 1u) {
-                    const uint32_t id = spid[j];
-                    rank = beg;
-                    for (uint32_t q = beg; q < beg + cnt; ++q) {
-                        const uint32_t jj = stmp[q];
-                        const uint32_t kk = skey[jj];
-                        rank += (kk < k || (kk == k && spid[jj] < id)) ? 1u : 0u;
+            for (int it = 0; it < PITEMS; ++it) {
+                const uint32_t kc = min((uint32_t)(tid + it * THREADS), npairs - 1u);
+                const uint32_t ab = *reinterpret_cast<const uint32_t *>(sord + 2 * kc);
+                const uint32_t a = ab & 0xFFFFu, b = ab >> 16;
+                const double Ea = sE[a], Eb = sE[b];
+                const double dx = Eb * sp0[a] - Ea * sp0[b];
+                const double dy = Eb * sp1[a] - Ea * sp1[b];
+                const double dz = Eb * sp2[a] - Ea * sp2[b];
+                ida[it] = spid[a];
+                ee[it] = Ea * Eb;
+                dd[it] = (dx * dx + dy * dy) + dz * dz;
+            }
+#pragma unroll
+            for (int it = 0; it < PITEMS; ++it) {
+                const U4 w = drawk(P, ida[it], (uint32_t)rho, kTagDec, 0);
+                u[it] = u53_bits(w.x, w.y);
+            }
+#pragma unroll
+            for (int it = 0; it < PITEMS; ++it) {
+                const uint32_t k = tid + it * THREADS;
+                bool hit;
+                if (TRACE) {
+                    const double s = dd[it] / ee[it];         // (p_a+p_b)^2, A9
+                    const double vrel = 0.5 * (s / ee[it]);   // s/(2 E_a E_b)
+                    const double prob = vrel * scale;         // Eq. 3 * cn/R
+                    hit = u[it] < prob;
+                    if (k < npairs) {
+                        if (fabs(u[it] - prob) <= 1e-12) atomicAdd(&stats->v[2], 1ull);
+                        const uint32_t ab = *reinterpret_cast<const uint32_t *>(sord + 2 * k);
+                        const unsigned long long e = P.trace_off[c] + (unsigned long long)rho * npairs + k;
+                        P.tr_cell[e] = c; P.tr_round[e] = (uint32_t)rho; P.tr_pa[e] = ida[it]; P.tr_pb[e] = spid[ab >> 16];
+                        P.tr_P[e] = prob; P.tr_u[e] = u[it]; P.tr_dec[e] = hit ? 1 : 0;
+                    }
+                } else {
+                    // sign(u - P) from u*(EaEb)^2 - |d|^2*scale/2; the exact form only inside a band
+                    // far wider than the rounding error (it also catches NaN, inf and underflow)
+                    const double ee2 = ee[it] * ee[it];
+                    const double diff = u[it] * ee2 - dd[it] * hscale;
+                    hit = diff < 0.0;
+                    if (CUBA_FORCE_SLOW_PATHS || !(fabs(diff) > 4e-9 * ee2) || !(ee2 > 1e-280)) {
+                        const uint32_t r = exact_decision(dd[it], ee[it], u[it], scale);
+                        hit = (r & 1u) != 0;
+                        if ((r & 2u) && k < npairs) atomicAdd(&stats->v[2], 1ull);
                     }
                 }
-                sord[rank] = (uint16_t)j;   // arrival slots in sord are dead after (c)
+                hit = hit && k < npairs;
+                const uint32_t hm = __ballot_sync(0xFFFFFFFFu, hit);
+                if (hit) shit[nh + __popc(hm & lanemask_lt())] = (uint16_t)k;
+                nh += __popc(hm);
             }
         }
-        __syncthreads();
-        // (e1) pair order[2k] with order[2k+1]: Eq. 3 decision; colliding pairs go to a list
-#pragma unroll
-        for (int it = 0; it < (ITEMS + 1) / 2; ++it) {
-            const uint32_t k = tid + it * THREADS;
-            bool hit = false;
-            double s = 0.0;
-            if (k < npairs) {
-                const uint32_t a = sord[2 * k], b = sord[2 * k + 1];
-                const uint32_t ida = spid[a];
-                double prob, u;
-                hit = pair_decide(P, ida, (uint32_t)rho, scale, sp0[a], sp1[a], sp2[a], sE[a],
-                                  sp0[b], sp1[b], sp2[b], sE[b], s, prob, u);
-                n_pairs += 1;
-                if (fabs(u - prob) <= 1e-12) n_near += 1;
-                if (TRACE) {
-                    const unsigned long long e = P.trace_off[c] + (unsigned long long)rho * npairs + k;
-                    P.tr_cell[e] = c; P.tr_round[e] = (uint32_t)rho; P.tr_pa[e] = ida; P.tr_pb[e] = spid[b];
-                    P.tr_P[e] = prob; P.tr_u[e] = u; P.tr_dec[e] = hit ? 1 : 0;
-                }
-            }
-            const uint32_t hm = __ballot_sync(0xFFFFFFFFu, hit);
-            if (hm) {
-                uint32_t basep = 0;
-                if (lane == 0) basep = atomicAdd(s_nhit, (uint32_t)__popc(hm));
-                basep = __shfl_sync(0xFFFFFFFFu, basep, 0);
-                if (hit) {
-                    const uint32_t pos = basep + __popc(hm & lanemask_lt());
-                    stmp[pos] = (uint16_t)k;      // stmp and skey are dead after (d)
-                    sS[k] = s;
-                }
-            }
-        }
-        // the bucket counters are free from here on: clear them for the next round
-#pragma unroll
-        for (int it = 0; it < ITEMS; ++it) {
-            const uint32_t j = tid + it * THREADS;
-            if (j < n) sbkt[j] = 0;
-        }
-        if (tid == 0) sbkt[n] = 0;
-        __syncthreads();
-        // (e2) scatter the colliding pairs, densely
-        const uint32_t nhit = *s_nhit;
-        for (uint32_t h = tid; h < nhit; h += THREADS) {
-            const uint32_t k = stmp[h];
-            const uint32_t a = sord[2 * k], b = sord[2 * k + 1];
+        __syncwarp();
+        // (e2) scatter this warp's colliding pairs, densely
+        for (uint32_t h = lane; h < nh; h += 32) {
+            const uint32_t k = shit[h];
+            const uint32_t ab = *reinterpret_cast<const uint32_t *>(sord + 2 * k);
+            const uint32_t a = ab & 0xFFFFu, b = ab >> 16;
+            const double pax = sp0[a], pay = sp1[a], paz = sp2[a], Ea = sE[a];
+            const double pbx = sp0[b], pby = sp1[b], pbz = sp2[b], Eb = sE[b];
+            const double ee = Ea * Eb;
+            const double dx = Eb * pax - Ea * pbx;
+            const double dy = Eb * pay - Ea * pby;
+            const double dz = Eb * paz - Ea * pbz;
+            const double s = ((dx * dx + dy * dy) + dz * dz) / ee;
             double q[6];
-            pair_scatter(P, spid[a], (uint32_t)rho, sS[k], sp0[a], sp1[a], sp2[a], sE[a],
-                         sp0[b], sp1[b], sp2[b], sE[b], q);
-            sp0[a] = q[0]; sp1[a] = q[1]; sp2[a] = q[2]; sE[a] = energy(q[0], q[1], q[2]);
-            sp0[b] = q[3]; sp1[b] = q[4]; sp2[b] = q[5]; sE[b] = energy(q[3], q[4], q[5]);
+            pair_scatter(P, spid[a], (uint32_t)rho, s, pax, pay, paz, Ea, pbx, pby, pbz, Eb, q);
+            sp0[a] = q[0]; sp1[a] = q[1]; sp2[a] = q[2];
+            sp0[b] = q[3]; sp1[b] = q[4]; sp2[b] = q[5];
+            if (rho + 1 < R) { sE[a] = energy(q[0], q[1], q[2]); sE[b] = energy(q[3], q[4], q[5]); }
         }
-        if (tid == 0) n_coll += nhit;
-        __syncthreads();
-        if (tid == 0) *s_nhit = 0;
+        warp_hits += nh;
+        __syncwarp();   // the hit list is rewritten in the next round
     }
+    __syncthreads();
+    const uint32_t lo_w = *reinterpret_cast<volatile uint32_t *>(&stats->lo);
 #pragma unroll
-    for (int it = 0; it < ITEMS; ++it) {
-        const uint32_t j = tid + it * THREADS;
-        if (j < n) { P.px[lo + j] = sp0[j]; P.py[lo + j] = sp1[j]; P.pz[lo + j] = sp2[j]; }
+    for (int g = 0; g < NG; ++g) {
+        if ((uint32_t)(g * G * THREADS) >= n) break;
+#pragma unroll
+        for (int i = 0; i < G; ++i) {
+            const uint32_t j = tid + (g * G + i) * THREADS;
+            if (j < n) { P.px[lo_w + j] = sp0[j]; P.py[lo_w + j] = sp1[j]; P.pz[lo_w + j] = sp2[j]; }
+        }
     }
-    if (tid == 0) atomicAdd(&P.counters[2], (unsigned long long)R);
+    if (lane == 0 && warp_hits) atomicAdd(&stats->v[1], (unsigned long long)warp_hits);
+    if (tid == 0) { stats->v[0] += (unsigned long long)R * npairs; atomicAdd(&P.counters[2], (unsigned long long)R); }
 }
 
 template <int THREADS>
@@ -459,27 +640,31 @@ __device__ __forceinline__ void prefetch_l2(const void *p)
     asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
 }
 
-// Shared-memory classes: CAP particles at most, 48 B of shared memory per particle.  The next
+// Shared-memory classes: CAP particles at most, 46 B of shared memory per particle.  The next
 // work item is fetched one cell ahead and its momenta / pids are prefetched into L2 while
 // the current cell is processed, so the load phase does not wait on DRAM.
 template <int THREADS, int ITEMS, int CAP, int MIN_BLOCKS, bool TRACE>
 __global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
 k_collide(CollideParams P)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    static_assert(CAP <= THREADS * ITEMS && CAP < 65536, "class capacity");
+#ifndef CUBA_G6
+#define CUBA_G6 3
+#endif
+    constexpr int G = (ITEMS == 6) ? CUBA_G6 : ((ITEMS % 2 == 0) ? 2 : ITEMS);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     double *sp0 = reinterpret_cast<double *>(smem_raw);
     double *sp1 = sp0 + CAP, *sp2 = sp1 + CAP, *sE = sp2 + CAP;
     uint32_t *spid = reinterpret_cast<uint32_t *>(sE + CAP);
-    uint32_t *skey = spid + CAP;
-    uint32_t *sbkt = skey + CAP;                 // CAP + 2 words = 2 CAP + 4 packed counters
-    uint16_t *sord = reinterpret_cast<uint16_t *>(sbkt + CAP + 2);
-    uint16_t *stmp = sord + CAP;
+    uint32_t *spark = spid + CAP;                // CAP keys + 4 sentinels (+ pad); hit lists between (d) and (c)
+    uint32_t *sbkt = spark + CAP + 8;            // CAP words = 2 CAP packed 16-bit counters
+    uint16_t *sord = reinterpret_cast<uint16_t *>(sbkt + CAP + 8);
     __shared__ uint32_t s_warp[32];
     __shared__ uint32_t s_item[2];
-    __shared__ uint32_t s_nhit;
+    __shared__ CtaStats s_stats;
 
     const uint32_t nlist = *P.list_count;
-    unsigned long long n_pairs = 0, n_coll = 0, n_near = 0;
+    if (threadIdx.x < 3) s_stats.v[threadIdx.x] = 0;
     if (threadIdx.x == 0) s_item[0] = atomicAdd(P.work, 1u);
     __syncthreads();
     uint32_t item = s_item[0];
@@ -498,15 +683,19 @@ k_collide(CollideParams P)
         }
         const uint32_t c = P.list[item];
         const uint32_t lo = P.cell_start[c], n = P.cell_start[c + 1] - lo;
-        collide_cell_smem<THREADS, ITEMS, TRACE>(P, c, lo, n, sp0, sp1, sp2, sE, spid, skey, sbkt, sord,
-                                                 stmp, s_warp, &s_nhit, n_pairs, n_coll, n_near);
+        collide_cell_smem<THREADS, ITEMS, G, TRACE>(P, c, lo, n, sp0, sp1, sp2, sE, spid, spark, sbkt, sord,
+                                                    s_warp, &s_stats);
         __syncthreads();
         item = next;
     }
-    flush_counters<THREADS>(P, n_pairs, n_coll, n_near);
+    if (threadIdx.x == 0) {
+        if (s_stats.v[0]) atomicAdd(&P.counters[0], s_stats.v[0]);
+        if (s_stats.v[1]) atomicAdd(&P.counters[1], s_stats.v[1]);
+        if (s_stats.v[2]) atomicAdd(&P.counters[3], s_stats.v[2]);
+    }
 }
 
-constexpr size_t collide_smem_bytes(int cap) { return (size_t)cap * 48 + 32; }
+constexpr size_t collide_smem_bytes(int cap) { return (size_t)cap * 46 + 64; }
 
 // Overflow class: cells larger than the biggest shared-memory class.  Same routine, scratch
 // in global memory (momenta are updated in place in the particle store; the cached energy

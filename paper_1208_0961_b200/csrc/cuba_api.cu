@@ -351,6 +351,10 @@ static int launch_collide(cuba_ctx *ctx, double base, const TraceDev *td)
     Soa &cur = ctx->set[ctx->cur];
     CollideParams P{};
     P.seed = ctx->seed; P.t = ctx->t; P.base = base;
+    for (uint32_t r = 0; r < 10; ++r) {               // Philox4x32-10 key schedule (Salmon et al., SC'11)
+        P.rk[2 * r] = (uint32_t)ctx->seed + r * 0x9E3779B9u;
+        P.rk[2 * r + 1] = (uint32_t)(ctx->seed >> 32) + r * 0xBB67AE85u;
+    }
     P.cell_start = ctx->at<uint32_t>(lay.cell_start);
     P.px = cur.px; P.py = cur.py; P.pz = cur.pz; P.pid = cur.pid;
     P.counters = ctx->at<unsigned long long>(lay.counters);
