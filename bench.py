@@ -38,7 +38,9 @@ UNIT = "particle-updates/s"
 BYTES_STREAM_HIST = 48      # reads x,y,z,px,py,pz
 BYTES_SCATTER = 104         # reads 6 fp64 + pid, writes 6 fp64 + pid
 BYTES_COLLIDE = 52          # reads px,py,pz,pid, writes px,py,pz (cells with n >= 2)
-BYTES_STEP = BYTES_STREAM_HIST + BYTES_SCATTER + BYTES_COLLIDE   # 204, SURVEY.md 8(d)
+BYTES_COLLIDE_FUSED = 76    # + reads x,y,z: the kernel also does S1-S3 + histogram of the next step (no k_stream_hist pass)
+BYTES_STEP = BYTES_STREAM_HIST + BYTES_SCATTER + BYTES_COLLIDE   # 204: the method as specified
+BYTES_STEP_FUSED = BYTES_SCATTER + BYTES_COLLIDE_FUSED           # 180: what the fused schedule actually has to move
 
 
 def peaks():
@@ -176,6 +178,7 @@ def main():
     ap.add_argument("--impl", default="cuba", choices=["cuba", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-fuse", action="store_true", help="run the separate k_stream_hist pass every step (A/B diagnostic)")
     ap.add_argument("--profile-mode", type=int, default=1, help="1: normal operation; 2: serialise the collision classes (diagnostic)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuba" else args.warmup
@@ -212,6 +215,9 @@ def main():
     host = [torch.from_numpy(a).pin_memory() for a in w.arrays()]
     sim = cuba.Cuba(w.box, w.ncell, *[h.to(dev) for h in host], w.n_test, w.seed)
     n = w.n
+    fused = not args.no_fuse
+    sim.set_option(1, 1 if fused else 0)
+    bytes_collide = BYTES_COLLIDE_FUSED if fused else BYTES_COLLIDE
 
     sampler = ClockSampler(local)
     sampler.start()
@@ -245,7 +251,8 @@ def main():
     collide_names = [k for k in prof if k.startswith("k_collide<") or k == "k_collide_overflow"]
     caps = [int(re.search(r"cap=(\d+)", k).group(1)) for k in collide_names if "cap=" in k]
     cls = np.searchsorted(caps, counts, side="left")
-    class_particles = {name: int(counts[(cls == k) & (counts >= 2)].sum()) for k, name in enumerate(collide_names)}
+    class_particles = {name: int(counts[(cls == k) & (counts >= (1 if fused else 2))].sum())
+                       for k, name in enumerate(collide_names)}
 
     # ---- observables timed separately --------------------------------------------------
     torch.cuda.synchronize()
@@ -282,8 +289,8 @@ def main():
         per_kernel = {k: {"ms_per_launch": (v[0] / v[1]) if v[1] else 0.0, "launches": v[1], "ms_total": v[0]}
                       for k, v in prof.items()}
         alg = {"k_stream_hist": BYTES_STREAM_HIST * n, "k_scatter": BYTES_SCATTER * n}
-        alg.update({name: BYTES_COLLIDE * cnt for name, cnt in class_particles.items()})
-        alg["k_collide (all classes, concurrent)"] = BYTES_COLLIDE * sum(class_particles.values())
+        alg.update({name: bytes_collide * cnt for name, cnt in class_particles.items()})
+        alg["k_collide (all classes, concurrent)"] = bytes_collide * sum(class_particles.values())
         dom = max(per_kernel, key=lambda k: per_kernel[k]["ms_total"])
         dom_ms = per_kernel[dom]["ms_per_launch"]
         achieved = alg.get(dom, 0) / (dom_ms * 1e-3) / 1e9 if dom_ms else 0.0
@@ -300,7 +307,9 @@ def main():
             "config": {"workload": workloads_name(args.config), "n_particles": n, "ncells": sim.ncells,
                        "l2": "inputs larger than L2 (%.2f GB state per copy vs 126 MB L2), no flush" % (52 * n / 1e9)
                        if 52 * n > 4 * 126e6 else "state comparable to L2: cache-resident, not a roofline config",
-                       "parallelism": "replicas x%d" % world if world > 1 else "single GPU"},
+                       "parallelism": "replicas x%d" % world if world > 1 else "single GPU",
+                       "schedule": "fused: collide(t) also writes the histogram of step t+1 (CUBA_OPT_FUSE_HIST=1)"
+                       if fused else "separate k_stream_hist pass (CUBA_OPT_FUSE_HIST=0)"},
             "pair_evals_per_s": pairs_total / sec,
             "pairs_per_step": pairs_total / args.steps,
             "observables_ms": obs_ms,
@@ -309,7 +318,9 @@ def main():
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                          "alg_bytes_per_launch": alg.get(dom, 0),
-                         "step": {"alg_bytes_per_particle": BYTES_STEP, "achieved": BYTES_STEP * value / world / 1e9,
+                         "step": {"alg_bytes_per_particle": BYTES_STEP,
+                                  "moved_bytes_per_particle": BYTES_STEP_FUSED if fused else BYTES_STEP,
+                                  "achieved": BYTES_STEP * value / world / 1e9,
                                   "frac": BYTES_STEP * value / world / 1e9 / peak, "frac_of_8TBps_nominal": BYTES_STEP * value / world / 8e12},
                          "kernels": kernels},
         }

@@ -112,6 +112,16 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
  * surface at the next synchronising call. */
 int cuba_step(cuba_ctx *ctx, int nsteps, double dt, double sigma);
 
+/* Execution options (results are bit-identical for every setting; they only change how the
+ * step is scheduled on the device).  CUBA_OPT_FUSE_HIST (default 1): the collision kernel of
+ * step t also performs S1-S3 of step t+1 on the momenta it holds on chip and writes the
+ * (cell, direction) histogram of the counting sort, so that consecutive steps with the same
+ * dt skip the separate streaming/histogram pass; a step whose dt differs from the previous
+ * one (or that follows cuba_init / cuba_step_traced) runs that pass.  value 0 always runs the
+ * separate pass.  Errors: CUBA_ERR_NULL, CUBA_ERR_VALUE (unknown option or value). */
+#define CUBA_OPT_FUSE_HIST 1
+int cuba_set_option(cuba_ctx *ctx, int option, int value);
+
 /* PAPER.md:66 (total energy) and PAPER.md:68-70 Fig. 2 (energy density along x).
  * total = (sum E, sum px, sum py, sum pz) in GeV; edens[j] = sum_{i in slab j} E_i /
  * (n_test * V_slab) in GeV/fm^3 for nslab equal slabs along x (lab-frame T^00, A15).
@@ -153,7 +163,7 @@ int cuba_run_host(const double box[3], const int ncell[3], int64_t n,
  * Mode 1 times the collision kernels as one group (the size classes run concurrently on
  * internal streams, as in normal operation); mode 2 serialises them on the caller's stream and
  * times every class by itself (diagnostic: slower than normal operation); 0 switches off. */
-#define CUBA_PROFILE_GROUPS 16
+#define CUBA_PROFILE_GROUPS 17
 int cuba_profile_enable(cuba_ctx *ctx, int on);
 int cuba_profile_read(cuba_ctx *ctx, double *ms_sum, uint64_t *launches);
 const char *cuba_profile_name(int group);

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 EXPORTS = ("cuba_workspace_bytes", "cuba_init", "cuba_step", "cuba_observables", "cuba_state",
            "cuba_get_particles", "cuba_get_cells", "cuba_step_traced", "cuba_counters", "cuba_run_host", "cuba_destroy",
            "cuba_strerror", "cuba_last_cuda_error", "cuba_launch_count", "cuba_profile_enable",
-           "cuba_profile_read", "cuba_profile_name")
+           "cuba_profile_read", "cuba_profile_name", "cuba_set_option")
 
 
 class CubaError(RuntimeError):
@@ -103,6 +103,7 @@ def lib():
         L.cuba_last_cuda_error.restype = c_char_p
         L.cuba_launch_count.restype = c_uint64
         L.cuba_profile_enable.argtypes = [c_void_p, c_int]
+        L.cuba_set_option.argtypes = [c_void_p, c_int, c_int]
         L.cuba_profile_read.argtypes = [c_void_p, dp, POINTER(c_uint64)]
         L.cuba_profile_name.argtypes = [c_int]
         L.cuba_profile_name.restype = c_char_p
@@ -234,13 +235,17 @@ class Cuba:
         m = int(tr.n_pairs)
         return Trace(cell_of_pid, cell[:m], rnd[:m], pa[:m], pb[:m], P[:m], u[:m], dec[:m])
 
+    def set_option(self, option: int, value: int):
+        """cuba_set_option (OPT_FUSE_HIST = 1)."""
+        _check(lib().cuba_set_option(self._h, int(option), int(value)))
+
     def profile_enable(self, mode=1):
         """0 off, 1 per-kernel events (collision classes as one concurrent group), 2 classes serialised."""
         _check(lib().cuba_profile_enable(self._h, int(mode)))
 
     def profile_read(self):
         """{kernel group: (summed device ms, launches)} since profile_enable."""
-        G = 16
+        G = 17
         ms = (c_double * G)()
         cnt = (c_uint64 * G)()
         _check(lib().cuba_profile_read(self._h, ms, cnt))

@@ -10,8 +10,9 @@
 //                        turned into exclusive offsets in place; their sum is the new count
 //   K_S/K_F              exclusive scan of the new counts -> cell_start
 //   K_carry              per tile: particles of the tile's first cell that sit in earlier tiles
+//   K_D  k_dest_base     off[d][c_old] += cell_start[c_new(c_old, d)] (one gather per particle later)
 //   K_C  k_scatter       per particle again: S1-S3 recomputed, stable rank inside its
-//                        (c_old, d) group from warp ballots, dest = cell_start[c_new] +
+//                        (c_old, d) group from warp votes, dest = cell_start[c_new] +
 //                        off[d][c_old] + rank.  No atomics touch the order: the placement is
 //                        the stable counting sort of north_star (3), deterministic by construction.
 // HBM traffic per particle-step: K_A reads 48 B, K_C reads 52 B and writes 52 B.
@@ -160,46 +161,54 @@ k_stream_hist(Geom g, double dt, int64_t n, int64_t ntiles, Soa in, uint32_t *__
 }
 
 // ---- K_B ------------------------------------------------------------------------------
-// One thread per NEW cell.  Sources in ascending linear index (x slowest) == ascending
-// previous array position, which is what makes the placement stable (A8).
-__global__ void __launch_bounds__(256)
+// A block owns 256 NEW cells (the unit of the block-sum scan); each of its 32 warps takes 8 of
+// them, lane q < 27 the q-th source.  Sources in ascending linear index (x slowest) == ascending
+// previous array position, which is what makes the placement stable (A8).  The 8 gathers of a
+// lane are issued together; a warp scan turns the counts into exclusive offsets.
+constexpr int kGatherThreads = 1024;
+constexpr int kGatherCellsPerWarp = 256 / (kGatherThreads / 32);
+
+__global__ void __launch_bounds__(kGatherThreads)
 k_gather(Geom g, uint32_t *__restrict__ cnt, uint32_t *__restrict__ count_new,
          uint32_t *__restrict__ block_sum)
 {
-    __shared__ uint32_t s_warp[8];
-    const uint32_t c = blockIdx.x * 256u + threadIdx.x;
-    uint32_t run = 0;
-    if (c < g.ncells) {
-        const int iz = c % g.nc[2];
-        const int iy = (c / g.nc[2]) % g.nc[1];
-        const int ix = c / (g.nc[2] * g.nc[1]);
-        for (int ox = -1; ox <= 1; ++ox) {
-            const int sx = ix + ox;
-            if (sx < 0 || sx >= g.nc[0]) continue;
-            for (int oy = -1; oy <= 1; ++oy) {
-                const int sy = iy + oy;
-                if (sy < 0 || sy >= g.nc[1]) continue;
-                for (int oz = -1; oz <= 1; ++oz) {
-                    const int sz = iz + oz;
-                    if (sz < 0 || sz >= g.nc[2]) continue;
-                    const int dcode = (1 - ox) * 9 + (1 - oy) * 3 + (1 - oz);   // the source moved by -o
-                    const size_t e = (size_t)dcode * g.ncells + cell_linear(g, sx, sy, sz);
-                    const uint32_t v = cnt[e];
-                    cnt[e] = run;
-                    run += v;
-                }
-            }
-        }
-        count_new[c] = run;
-    }
-    uint32_t s = run;
+    __shared__ uint32_t s_warp[kGatherThreads / 32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int ox = lane / 9 - 1, oy = (lane / 3) % 3 - 1, oz = lane % 3 - 1;   // source = new cell + o
+    const int dcode = (1 - ox) * 9 + (1 - oy) * 3 + (1 - oz);                  // the source moved by -o
+    uint32_t v[kGatherCellsPerWarp];
+    size_t e[kGatherCellsPerWarp];
+    bool ok[kGatherCellsPerWarp];
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
-    if ((threadIdx.x & 31) == 0) s_warp[threadIdx.x >> 5] = s;
+    for (int k = 0; k < kGatherCellsPerWarp; ++k) {
+        const uint32_t c = blockIdx.x * 256u + wid * kGatherCellsPerWarp + k;
+        const int sz = (int)(c % (uint32_t)g.nc[2]) + oz;
+        const int sy = (int)((c / (uint32_t)g.nc[2]) % (uint32_t)g.nc[1]) + oy;
+        const int sx = (int)(c / ((uint32_t)g.nc[2] * (uint32_t)g.nc[1])) + ox;
+        ok[k] = lane < kDirs && c < g.ncells && sx >= 0 && sx < g.nc[0] && sy >= 0 && sy < g.nc[1] && sz >= 0 && sz < g.nc[2];
+        e[k] = ok[k] ? (size_t)dcode * g.ncells + cell_linear(g, sx, sy, sz) : 0;
+        v[k] = ok[k] ? cnt[e[k]] : 0u;
+    }
+    uint32_t wsum = 0;
+#pragma unroll
+    for (int k = 0; k < kGatherCellsPerWarp; ++k) {
+        const uint32_t c = blockIdx.x * 256u + wid * kGatherCellsPerWarp + k;
+        uint32_t inc = v[k];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (ok[k]) cnt[e[k]] = inc - v[k];
+        const uint32_t total = __shfl_sync(0xFFFFFFFFu, inc, 31);
+        if (lane == 0 && c < g.ncells) count_new[c] = total;
+        wsum += total;
+    }
+    if (lane == 0) s_warp[wid] = wsum;
     __syncthreads();
     if (threadIdx.x == 0) {
         uint32_t t = 0;
-        for (int w = 0; w < 8; ++w) t += s_warp[w];
+        for (int w = 0; w < kGatherThreads / 32; ++w) t += s_warp[w];
         block_sum[blockIdx.x] = t;
     }
 }
@@ -255,7 +264,7 @@ struct ClassTable {
 __global__ void __launch_bounds__(256)
 k_cell_start(uint32_t ncells, const uint32_t *__restrict__ count_new,
              const uint32_t *__restrict__ block_prefix, uint32_t *__restrict__ cell_start,
-             ClassTable ct, uint32_t *__restrict__ class_count, uint32_t *__restrict__ class_list,
+             ClassTable ct, uint32_t *__restrict__ class_count, uint4 *__restrict__ class_list,
              unsigned long long *__restrict__ max_occ)
 {
     __shared__ uint32_t s_warp[8];
@@ -277,9 +286,10 @@ k_cell_start(uint32_t ncells, const uint32_t *__restrict__ count_new,
         cell_start[c] = start;
         if (c == ncells - 1) cell_start[ncells] = start + v;
     }
-    // size class (warp-aggregated append; the list order does not affect any result)
+    // size class (warp-aggregated append; the list order does not affect any result).  Cells with
+    // a single particle have no pair but take part in the fused histogram of the next step.
     int k = -1;
-    if (v >= 2) {
+    if (v >= 1) {
         k = 0;
         while (v > ct.max_n[k]) ++k;
     }
@@ -289,12 +299,28 @@ k_cell_start(uint32_t ncells, const uint32_t *__restrict__ count_new,
         uint32_t pos = 0;
         if (lane == leader) pos = atomicAdd(&class_count[k], (uint32_t)__popc(peers));
         pos = __shfl_sync(peers, pos, leader) + __popc(peers & lanemask_lt());
-        class_list[(size_t)k * ncells + pos] = c;
+        class_list[(size_t)k * ncells + pos] = make_uint4(c, start, v, 0u);   // {cell, first slot, population}: no dependent loads in the consumer
     }
     uint32_t vmax = v;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) vmax = max(vmax, __shfl_xor_sync(0xFFFFFFFFu, vmax, o));
     if (lane == 0 && vmax > 0) atomicMax(max_occ, (unsigned long long)vmax);
+}
+
+// ---- K_D: dest_base[d][c_old] = cell_start[c_new(c_old, d)] + off[d][c_old], in place ------
+// One thread per (direction, old cell): the scatter then needs a single table gather per
+// particle, which it can issue as soon as the direction is known.
+__global__ void __launch_bounds__(256)
+k_dest_base(Geom g, uint32_t *__restrict__ off, const uint32_t *__restrict__ cell_start)
+{
+    const uint32_t c = blockIdx.x * 256u + threadIdx.x;
+    const int d = blockIdx.y;
+    if (c >= g.ncells) return;
+    const int iz = (int)(c % (uint32_t)g.nc[2]) + d % 3 - 1;
+    const int iy = (int)((c / (uint32_t)g.nc[2]) % (uint32_t)g.nc[1]) + (d / 3) % 3 - 1;
+    const int ix = (int)(c / ((uint32_t)g.nc[2] * (uint32_t)g.nc[1])) + d / 9 - 1;
+    if (ix < 0 || ix >= g.nc[0] || iy < 0 || iy >= g.nc[1] || iz < 0 || iz >= g.nc[2]) return;   // no particle goes there
+    off[(size_t)d * g.ncells + c] += cell_start[cell_linear(g, ix, iy, iz)];
 }
 
 // ---- K_carry ---------------------------------------------------------------------------
@@ -330,9 +356,8 @@ k_carry(int ntiles, const uint32_t *__restrict__ tile_rec, uint32_t *__restrict_
 // prefix_d(li) - prefix_d(first particle of c_old in the tile) [+ carry if that is li 0].
 template <bool WITH_CELL_OF_PID>
 __global__ void __launch_bounds__(kTileThreads, 3)
-k_scatter(Geom g, double dt, int64_t n, int64_t ntiles, Soa in, Soa out, const uint32_t *__restrict__ off,
-          const uint32_t *__restrict__ cell_start, const uint32_t *__restrict__ carry,
-          uint32_t *__restrict__ cell_of_pid)
+k_scatter(Geom g, double dt, int64_t n, int64_t ntiles, Soa in, Soa out, const uint32_t *__restrict__ dest_base,
+          const uint32_t *__restrict__ carry, uint32_t *__restrict__ cell_of_pid)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     TileStage<7> *stage = reinterpret_cast<TileStage<7> *>(smem_raw);
@@ -342,6 +367,7 @@ k_scatter(Geom g, double dt, int64_t n, int64_t ntiles, Soa in, Soa out, const u
     __shared__ uint32_t s_pref[kTileRows][kDirs];
     __shared__ uint32_t s_head[kTileRows];
     __shared__ int s_lasthead[kTileRows];
+    __shared__ uint32_t s_carry[32];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     if (tid == 0) { mbar_init(&s_bar[0], 1); mbar_init(&s_bar[1], 1); mbar_fence_init(); }
     __syncthreads();
@@ -356,6 +382,9 @@ k_scatter(Geom g, double dt, int64_t n, int64_t ntiles, Soa in, Soa out, const u
         const int64_t base = tile * kTile;
 
         Moved m[kTileItems];
+        uint32_t dbase[kTileItems];   // cell_start[c_new] + off[d][c_old]: gathered now, used after the ranking
+        if (tid < kDirs) s_carry[tid] = carry[(size_t)tile * kTileRec + tid];
+        for (int e = tid; e < kTileRows * kDirs; e += kTileThreads) (&s_ball[0][0])[e] = 0;
 #pragma unroll
         for (int j = 0; j < kTileItems; ++j) {
             const int li = j * kTileThreads + tid;
@@ -363,6 +392,7 @@ k_scatter(Geom g, double dt, int64_t n, int64_t ntiles, Soa in, Soa out, const u
             if (base + li < n)
                 m[j] = move_particle(g, dt, st.v[0][li], st.v[1][li], st.v[2][li], st.v[3][li], st.v[4][li], st.v[5][li]);
             s_cold[li] = m[j].c_old;
+            dbase[j] = (m[j].d >= 0) ? dest_base[(size_t)m[j].d * g.ncells + m[j].c_old] : 0u;
         }
         __syncthreads();
 #pragma unroll
@@ -371,13 +401,9 @@ k_scatter(Geom g, double dt, int64_t n, int64_t ntiles, Soa in, Soa out, const u
             const int li = j * kTileThreads + tid;
             const bool valid = (base + li) < n;
             const int dd = m[j].d;
-            uint32_t mine = 0;
-#pragma unroll
-            for (int q = 0; q < kDirs; ++q) {
-                const uint32_t bq = __ballot_sync(0xFFFFFFFFu, dd == q);
-                if (lane == q) mine = bq;
-            }
-            if (lane < kDirs) s_ball[r][lane] = mine;
+            // one bit mask per direction present in the row (absent directions stay zero)
+            const uint32_t peers = __match_any_sync(0xFFFFFFFFu, dd);
+            if (dd >= 0 && (peers & lanemask_lt()) == 0) s_ball[r][dd] = peers;
             const bool head = valid && (li == 0 || s_cold[li - 1] != m[j].c_old);
             const uint32_t hb = __ballot_sync(0xFFFFFFFFu, head);
             if (lane == 0) s_head[r] = hb;
@@ -413,8 +439,8 @@ k_scatter(Geom g, double dt, int64_t n, int64_t ntiles, Soa in, Soa out, const u
             const int rs = sli >> 5, ls = sli & 31;
             const uint32_t pre_s = s_pref[rs][dd] + __popc(s_ball[rs][dd] & ((1u << ls) - 1u));
             uint32_t rank = pre_i - pre_s;
-            if (sli == 0) rank += carry[(size_t)tile * kTileRec + dd];
-            const uint32_t dest = cell_start[m[j].c_new] + off[(size_t)dd * g.ncells + m[j].c_old] + rank;
+            if (sli == 0) rank += s_carry[dd];
+            const uint32_t dest = dbase[j] + rank;
             const uint32_t id = st.pid[li];
             out.x[dest] = m[j].x; out.y[dest] = m[j].y; out.z[dest] = m[j].z;
             out.px[dest] = m[j].px; out.py[dest] = m[j].py; out.pz[dest] = m[j].pz;

@@ -22,15 +22,24 @@ struct CollideParams {
     uint32_t t;           // global step index
     double base;          // sigma*dt/(r_test*V_cell): Eq. 3 without v_rel
     const uint32_t *cell_start;
-    const uint32_t *list; // cells of this size class
+    const uint4 *list;    // cells of this size class: {cell, first slot, population, -}
     const uint32_t *list_count;
-    uint32_t *work;       // dynamic work counter of this class
+    uint32_t *work;       // dynamic work counter of this class (overflow kernel)
     double *px, *py, *pz;
     const uint32_t *pid;
     unsigned long long *counters; // [0] pairs [1] collisions [2] rounds [3] near-threshold [4] overflow cells
     uint32_t *flags;
     // overflow class only: global scratch, 4 u32 per particle of the cell
     uint32_t *arena;
+    // fused histogram of the NEXT step (next_dt > 0): the cell's CTA holds the final momenta on
+    // chip, and the old cell of every particle is the cell itself, so S1-S3 of step t+1 are done
+    // here and the (cell, direction) counts and the per-tile carries are written directly --
+    // the separate k_stream_hist / k_carry pass (48 B per particle) disappears.
+    double next_dt;
+    Geom g;
+    const double *x, *y, *z;
+    uint32_t *cnt;        // [27][ncells], cleared beforehand (empty cells stay zero)
+    uint32_t *carry;      // [ntiles][kTileRec]
     // trace (TRACE instantiation only)
     const unsigned long long *trace_off;  // per cell: first pair record
     uint32_t *tr_cell, *tr_round, *tr_pa, *tr_pb;
@@ -133,6 +142,7 @@ __device__ __forceinline__ void collide_cell(const CollideParams &P, uint32_t c,
     int R;
     if (!(pmax <= 64.0)) { if (tid == 0) atomicOr(P.flags, kFlagRounds); R = 64; }
     else R = (pmax <= 1.0) ? 1 : (int)ceil(pmax);
+    if (n < 2u) R = 0;
     const double scale = (cn * P.base) / (double)R;
     const uint32_t npairs = n >> 1;
 
@@ -233,6 +243,52 @@ __device__ __forceinline__ void collide_cell(const CollideParams &P, uint32_t c,
         P.px[lo + j] = sp0[j]; P.py[lo + j] = sp1[j]; P.pz[lo + j] = sp2[j];
     }
     if (tid == 0) atomicAdd(&P.counters[2], (unsigned long long)R);
+}
+
+__device__ __forceinline__ void prefetch_l2(const void *p)
+{
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+
+// ---- fused histogram of the next step ---------------------------------------------------
+// Direction code of a particle of cell (ix0,iy0,iz0) after S1-S3 with time step dt: the same
+// arithmetic as move_particle() in bin.cuh (k_stream_hist / k_scatter), so the counts written
+// here equal those k_stream_hist would produce from the written-back store.
+__device__ __forceinline__ int next_direction(const Geom &g, double dt, int ix0, int iy0, int iz0,
+                                              double x, double y, double z, double px, double py, double pz, double E)
+{
+    const double w = dt / E;                         // PAPER.md:34 Eq. 2 with c = 1
+    x = x + px * w;
+    y = y + py * w;
+    z = z + pz * w;
+    reflect_axis(x, px, g.L[0]);
+    reflect_axis(y, py, g.L[1]);
+    reflect_axis(z, pz, g.L[2]);
+    const int dx = axis_index(x, g.inv_d[0], g.nc[0]) - ix0 + 1;
+    const int dy = axis_index(y, g.inv_d[1], g.nc[1]) - iy0 + 1;
+    const int dz = axis_index(z, g.inv_d[2], g.nc[2]) - iz0 + 1;
+    return ((unsigned)dx <= 2u && (unsigned)dy <= 2u && (unsigned)dz <= 2u) ? (dx * 9 + dy * 3 + dz) : -1;
+}
+
+// Tile segments of a cell: the flat passes work on tiles of kTile consecutive slots; segment k of
+// the cell [lo, lo+n) is its intersection with tile (lo / kTile) + k.  s_seg[k][d] counts the
+// cell's particles of segment k that move in direction d.  From it:
+//   cnt[d][c]              = sum over all segments                      (what K_A accumulates)
+//   carry[tile T0+k][d]    = sum over segments before k, k >= 1         (what k_carry derives)
+//   carry[tile T0][d]      = 0 if the cell starts exactly at the tile start
+// Every tile start lies in exactly one non-empty cell, so every carry row is written once.
+template <int THREADS>
+__device__ __forceinline__ void hist_publish(const CollideParams &P, uint32_t c, uint32_t lo, uint32_t n,
+                                             const uint32_t *s_seg)
+{
+    const uint32_t T0 = lo / kTile, nseg = (lo + n - 1u) / kTile - T0 + 1u;
+    for (uint32_t e = threadIdx.x; e < nseg * kDirs; e += THREADS) {
+        const uint32_t k = e / kDirs, d = e - k * kDirs;
+        uint32_t before = 0;
+        for (uint32_t q = 0; q < k; ++q) before += s_seg[q * kDirs + d];
+        if (k > 0 || lo % kTile == 0) P.carry[(size_t)(T0 + k) * kTileRec + d] = before;
+        if (k == nseg - 1u) P.cnt[(size_t)d * P.g.ncells + c] = before + s_seg[k * kDirs + d];
+    }
 }
 
 // ---- shared-memory classes ------------------------------------------------------------
@@ -369,16 +425,23 @@ __device__ __noinline__ uint32_t exact_decision(double dd, double ee, double u, 
 // and the constants of the current cell that are only needed at a few places (kept out of
 // registers across the register-hungry phases).
 struct CtaStats {
-    unsigned long long v[3];
     double scale, hscale;     // Eq. 3 factor cn*base/R of the current cell, and half of it
     uint32_t lo;              // first slot of the current cell
+    uint32_t near;            // near-threshold decisions of this CTA (A16; rare)
+};
+
+// Per-thread accumulators over all cells of a CTA, flushed once at the end of the kernel.
+struct ThreadStats {
+    unsigned long long pairs, rounds;   // uniform over the CTA; thread 0 flushes
+    uint32_t hits;                       // uniform over a warp; lane 0 flushes
 };
 
 template <int THREADS, int ITEMS, int G, bool TRACE>
 __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32_t c, uint32_t lo, uint32_t n,
                                                   double *sp0, double *sp1, double *sp2, double *sE,
                                                   uint32_t *spid, uint32_t *spark, uint32_t *sbkt,
-                                                  uint16_t *sord, uint32_t *s_warp, CtaStats *stats)
+                                                  uint16_t *sord, uint32_t *s_warp, CtaStats *stats,
+                                                  uint32_t *s_seg, ThreadStats &acc, uint32_t lo_next, uint32_t n_next)
 {
     static_assert(ITEMS % G == 0, "items are processed in groups of G");
     constexpr int NG = ITEMS / G;
@@ -390,6 +453,8 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
     int R;
     if (!(pmax <= 64.0)) { if (tid == 0) atomicOr(P.flags, kFlagRounds); R = 64; }
     else R = (pmax <= 1.0) ? 1 : (int)ceil(pmax);
+    if (n < 2u) R = 0;          // a single particle has no partner; it is here for the fused histogram only
+    const bool hist = P.next_dt > 0.0;
     if (tid == 0) {
         const double scale = (cn * P.base) / (double)R;
         stats->scale = scale; stats->hscale = 0.5 * scale; stats->lo = lo;
@@ -417,7 +482,16 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
             if (j < n) { sp0[j] = a[i]; sp1[j] = b[i]; sp2[j] = cc[i]; sE[j] = e; spid[j] = id[i]; sbkt[j] = 0; }
         }
     }
+    if (hist)
+        for (uint32_t e = tid; e < ((lo + n - 1u) / kTile - lo / kTile + 1u) * kDirs; e += THREADS) s_seg[e] = 0;
     __syncthreads();
+    // the CTA's next cell goes to L2 while this one is processed, so its load phase does not wait on DRAM
+    for (uint32_t l = tid * 16u; n_next && l < n_next + 16u; l += THREADS * 16u) {   // one 128 B line of doubles per thread
+        const uint32_t e = lo_next + min(l, n_next - 1u);
+        prefetch_l2(P.px + e); prefetch_l2(P.py + e); prefetch_l2(P.pz + e);
+        if ((l & 16u) == 0) prefetch_l2(P.pid + e);
+        if (hist) { prefetch_l2(P.x + e); prefetch_l2(P.y + e); prefetch_l2(P.z + e); }
+    }
 
     uint32_t warp_hits = 0;
     for (int rho = 0; rho < R; ++rho) {
@@ -557,7 +631,7 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
                     const double prob = vrel * scale;         // Eq. 3 * cn/R
                     hit = u[it] < prob;
                     if (k < npairs) {
-                        if (fabs(u[it] - prob) <= 1e-12) atomicAdd(&stats->v[2], 1ull);
+                        if (fabs(u[it] - prob) <= 1e-12) atomicAdd(&stats->near, 1u);
                         const uint32_t ab = *reinterpret_cast<const uint32_t *>(sord + 2 * k);
                         const unsigned long long e = P.trace_off[c] + (unsigned long long)rho * npairs + k;
                         P.tr_cell[e] = c; P.tr_round[e] = (uint32_t)rho; P.tr_pa[e] = ida[it]; P.tr_pb[e] = spid[ab >> 16];
@@ -572,7 +646,7 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
                     if (CUBA_FORCE_SLOW_PATHS || !(fabs(diff) > 4e-9 * ee2) || !(ee2 > 1e-280)) {
                         const uint32_t r = exact_decision(dd[it], ee[it], u[it], scale);
                         hit = (r & 1u) != 0;
-                        if ((r & 2u) && k < npairs) atomicAdd(&stats->v[2], 1ull);
+                        if ((r & 2u) && k < npairs) atomicAdd(&stats->near, 1u);
                     }
                 }
                 hit = hit && k < npairs;
@@ -598,13 +672,26 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
             pair_scatter(P, spid[a], (uint32_t)rho, s, pax, pay, paz, Ea, pbx, pby, pbz, Eb, q);
             sp0[a] = q[0]; sp1[a] = q[1]; sp2[a] = q[2];
             sp0[b] = q[3]; sp1[b] = q[4]; sp2[b] = q[5];
-            if (rho + 1 < R) { sE[a] = energy(q[0], q[1], q[2]); sE[b] = energy(q[3], q[4], q[5]); }
+            if (rho + 1 < R || hist) { sE[a] = energy(q[0], q[1], q[2]); sE[b] = energy(q[3], q[4], q[5]); }
         }
         warp_hits += nh;
         __syncwarp();   // the hit list is rewritten in the next round
     }
     __syncthreads();
     const uint32_t lo_w = *reinterpret_cast<volatile uint32_t *>(&stats->lo);
+    // positions for the fused histogram: all loads of a thread in flight before anything waits on them
+#ifndef CUBA_HB_ALL
+#define CUBA_HB_ALL 0
+#endif
+    constexpr int HB = (THREADS >= 512 || !CUBA_HB_ALL) ? ((ITEMS % 2 == 0) ? 2 : 1) : ITEMS;
+    double xx[HB], yy[HB], zz[HB];
+    if (hist && HB == ITEMS) {
+#pragma unroll
+        for (int it = 0; it < HB; ++it) {
+            const uint32_t jc = lo_w + min((uint32_t)(tid + it * THREADS), last);
+            xx[it] = P.x[jc]; yy[it] = P.y[jc]; zz[it] = P.z[jc];
+        }
+    }
 #pragma unroll
     for (int g = 0; g < NG; ++g) {
         if ((uint32_t)(g * G * THREADS) >= n) break;
@@ -614,8 +701,72 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
             if (j < n) { P.px[lo_w + j] = sp0[j]; P.py[lo_w + j] = sp1[j]; P.pz[lo_w + j] = sp2[j]; }
         }
     }
-    if (lane == 0 && warp_hits) atomicAdd(&stats->v[1], (unsigned long long)warp_hits);
-    if (tid == 0) { stats->v[0] += (unsigned long long)R * npairs; atomicAdd(&P.counters[2], (unsigned long long)R); }
+    acc.hits += warp_hits;
+    acc.pairs += (unsigned long long)R * npairs;
+    acc.rounds += (unsigned long long)R;
+
+    // ---- fused histogram of the next step (S1-S3 of step t+1 on the final momenta) ----------
+    if (hist) {
+        const uint32_t T0 = lo_w / kTile;
+        const int iz0 = (int)(c % (uint32_t)P.g.nc[2]);
+        const int iy0 = (int)((c / (uint32_t)P.g.nc[2]) % (uint32_t)P.g.nc[1]);
+        const int ix0 = (int)(c / ((uint32_t)P.g.nc[2] * (uint32_t)P.g.nc[1]));
+#pragma unroll
+        for (int g = 0; g < ITEMS / HB; ++g) {
+            if ((uint32_t)(g * HB * THREADS) >= n) break;
+            if (HB != ITEMS) {
+#pragma unroll
+                for (int i = 0; i < HB; ++i) {
+                    const uint32_t jc = lo_w + min((uint32_t)(tid + (g * HB + i) * THREADS), last);
+                    xx[i] = P.x[jc]; yy[i] = P.y[jc]; zz[i] = P.z[jc];
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < HB; ++i) {
+                const uint32_t j = tid + (g * HB + i) * THREADS, jj = min(j, last);
+                const int d = next_direction(P.g, P.next_dt, ix0, iy0, iz0, xx[i], yy[i], zz[i],
+                                             sp0[jj], sp1[jj], sp2[jj], sE[jj]);
+                const bool valid = j < n;
+                if (valid && d < 0) atomicOr(P.flags, kFlagMoved);
+                const uint32_t key = ((lo_w + jj) / kTile - T0) * kDirs + (uint32_t)max(d, 0);
+                const uint32_t active = __ballot_sync(0xFFFFFFFFu, valid);
+                if (valid) {
+                    const uint32_t peers = __match_any_sync(active, key);
+                    if ((peers & lanemask_lt()) == 0) atomicAdd(&s_seg[key], (uint32_t)__popc(peers));
+                }
+            }
+        }
+        __syncthreads();
+        hist_publish<THREADS>(P, c, lo_w, n, s_seg);
+    }
+}
+
+// Fused histogram for the overflow class: any n, one tile segment after the other.
+template <int THREADS>
+__device__ __forceinline__ void hist_cell_generic(const CollideParams &P, uint32_t c, uint32_t lo, uint32_t n,
+                                                  const double *sE, uint32_t *s_run)
+{
+    const int tid = threadIdx.x;
+    const uint32_t T0 = lo / kTile, nseg = (lo + n - 1u) / kTile - T0 + 1u;
+    const int iz0 = (int)(c % (uint32_t)P.g.nc[2]);
+    const int iy0 = (int)((c / (uint32_t)P.g.nc[2]) % (uint32_t)P.g.nc[1]);
+    const int ix0 = (int)(c / ((uint32_t)P.g.nc[2] * (uint32_t)P.g.nc[1]));
+    if (tid < kDirs) s_run[tid] = 0;
+    __syncthreads();
+    for (uint32_t k = 0; k < nseg; ++k) {
+        if (tid < kDirs && (k > 0 || lo % kTile == 0)) P.carry[(size_t)(T0 + k) * kTileRec + tid] = s_run[tid];
+        __syncthreads();
+        const uint32_t j0 = max(lo, (T0 + k) * (uint32_t)kTile) - lo;
+        const uint32_t j1 = min(lo + n, (T0 + k + 1u) * (uint32_t)kTile) - lo;
+        for (uint32_t j = j0 + tid; j < j1; j += THREADS) {
+            const int d = next_direction(P.g, P.next_dt, ix0, iy0, iz0, P.x[lo + j], P.y[lo + j], P.z[lo + j],
+                                         P.px[lo + j], P.py[lo + j], P.pz[lo + j], sE[j]);
+            if (d < 0) atomicOr(P.flags, kFlagMoved);
+            atomicAdd(&s_run[max(d, 0)], 1u);
+        }
+        __syncthreads();
+    }
+    if (tid < kDirs) P.cnt[(size_t)tid * P.g.ncells + c] = s_run[tid];
 }
 
 template <int THREADS>
@@ -633,11 +784,6 @@ __device__ __forceinline__ void flush_counters(const CollideParams &P, unsigned 
         if (n_coll) atomicAdd(&P.counters[1], n_coll);
         if (n_near) atomicAdd(&P.counters[3], n_near);
     }
-}
-
-__device__ __forceinline__ void prefetch_l2(const void *p)
-{
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
 }
 
 // Shared-memory classes: CAP particles at most, 46 B of shared memory per particle.  The next
@@ -660,38 +806,49 @@ k_collide(CollideParams P)
     uint32_t *sbkt = spark + CAP + 8;            // CAP words = 2 CAP packed 16-bit counters
     uint16_t *sord = reinterpret_cast<uint16_t *>(sbkt + CAP + 8);
     __shared__ uint32_t s_warp[32];
-    __shared__ uint32_t s_item[2];
     __shared__ CtaStats s_stats;
+    __shared__ uint32_t s_seg[((CAP + kTile - 2) / kTile + 1) * kDirs];   // a cell of CAP particles spans at most this many tiles
 
+    // Static round-robin over the class list: the cells of a class have similar populations, and
+    // a known next index lets the next entry be loaded a whole cell ahead (no atomic -> list ->
+    // cell_start chain of dependent global loads between cells).
     const uint32_t nlist = *P.list_count;
-    if (threadIdx.x < 3) s_stats.v[threadIdx.x] = 0;
+    if (threadIdx.x == 0) s_stats.near = 0;
+    ThreadStats acc{0ull, 0ull, 0u};
+#ifndef CUBA_STATIC_RR
+#define CUBA_STATIC_RR 0
+#endif
+#if CUBA_STATIC_RR
+    uint32_t item = blockIdx.x;
+    uint4 cur = make_uint4(0u, 0u, 0u, 0u);
+    if (item < nlist) cur = P.list[item];
+    for (; item < nlist; item += gridDim.x) {
+        uint4 nxt = make_uint4(0u, 0u, 0u, 0u);
+        if (item + gridDim.x < nlist) nxt = P.list[item + gridDim.x];   // first used after the staging barrier
+#else
+    __shared__ uint32_t s_item[2];
     if (threadIdx.x == 0) s_item[0] = atomicAdd(P.work, 1u);
     __syncthreads();
     uint32_t item = s_item[0];
+    uint4 cur = make_uint4(0u, 0u, 0u, 0u);
+    if (item < nlist) cur = P.list[item];
     for (int it = 0; item < nlist; ++it) {
         if (threadIdx.x == 0) s_item[(it + 1) & 1] = atomicAdd(P.work, 1u);
         __syncthreads();
-        const uint32_t next = s_item[(it + 1) & 1];
-        if (next < nlist) {
-            const uint32_t c2 = P.list[next];
-            const uint32_t lo2 = P.cell_start[c2], n2 = P.cell_start[c2 + 1] - lo2;
-            for (uint32_t l = threadIdx.x * 16u; l < n2 + 16u; l += THREADS * 16u) {   // one 128 B line per thread
-                const uint32_t e = lo2 + min(l, n2 - 1u);
-                prefetch_l2(P.px + e); prefetch_l2(P.py + e); prefetch_l2(P.pz + e);
-                if ((l & 16u) == 0) prefetch_l2(P.pid + e);
-            }
-        }
-        const uint32_t c = P.list[item];
-        const uint32_t lo = P.cell_start[c], n = P.cell_start[c + 1] - lo;
-        collide_cell_smem<THREADS, ITEMS, G, TRACE>(P, c, lo, n, sp0, sp1, sp2, sE, spid, spark, sbkt, sord,
-                                                    s_warp, &s_stats);
+        item = s_item[(it + 1) & 1];
+        uint4 nxt = make_uint4(0u, 0u, 0u, 0u);
+        if (item < nlist) nxt = P.list[item];
+#endif
+        collide_cell_smem<THREADS, ITEMS, G, TRACE>(P, cur.x, cur.y, cur.z, sp0, sp1, sp2, sE, spid, spark, sbkt, sord,
+                                                    s_warp, &s_stats, s_seg, acc, nxt.y, nxt.z);
         __syncthreads();
-        item = next;
+        cur = nxt;
     }
+    if ((threadIdx.x & 31) == 0 && acc.hits) atomicAdd(&P.counters[1], (unsigned long long)acc.hits);
     if (threadIdx.x == 0) {
-        if (s_stats.v[0]) atomicAdd(&P.counters[0], s_stats.v[0]);
-        if (s_stats.v[1]) atomicAdd(&P.counters[1], s_stats.v[1]);
-        if (s_stats.v[2]) atomicAdd(&P.counters[3], s_stats.v[2]);
+        if (acc.pairs) atomicAdd(&P.counters[0], acc.pairs);
+        if (acc.rounds) atomicAdd(&P.counters[2], acc.rounds);
+        if (s_stats.near) atomicAdd(&P.counters[3], (unsigned long long)s_stats.near);
     }
 }
 
@@ -707,6 +864,7 @@ k_collide_overflow(CollideParams P, unsigned long long *arena_cursor, double *ar
     __shared__ uint32_t s_warp[32];
     __shared__ uint32_t s_item;
     __shared__ unsigned long long s_base;
+    __shared__ uint32_t s_run[32];
     const uint32_t nlist = *P.list_count;
     unsigned long long n_pairs = 0, n_coll = 0, n_near = 0;
     for (;;) {
@@ -714,8 +872,8 @@ k_collide_overflow(CollideParams P, unsigned long long *arena_cursor, double *ar
         __syncthreads();
         const uint32_t item = s_item;
         if (item >= nlist) break;
-        const uint32_t c = P.list[item];
-        const uint32_t lo = P.cell_start[c], n = P.cell_start[c + 1] - lo;
+        const uint4 ent = P.list[item];
+        const uint32_t c = ent.x, lo = ent.y, n = ent.z;
         if (threadIdx.x == 0) {
             s_base = atomicAdd(arena_cursor, (unsigned long long)n + 2ull);
             atomicAdd(&P.counters[4], 1ull);
@@ -728,6 +886,8 @@ k_collide_overflow(CollideParams P, unsigned long long *arena_cursor, double *ar
         collide_cell<1024, TRACE, uint32_t>(P, c, lo, n, P.px + lo, P.py + lo, P.pz + lo, arena_E + b,
                                             const_cast<uint32_t *>(P.pid) + lo, skey, sbkt, sord, stmp,
                                             s_warp, n_pairs, n_coll, n_near);
+        __syncthreads();
+        if (P.next_dt > 0.0) hist_cell_generic<1024>(P, c, lo, n, arena_E + b, s_run);
         __syncthreads();
     }
     flush_counters<1024>(P, n_pairs, n_coll, n_near);

@@ -83,7 +83,7 @@ Layout make_layout(int64_t n, int64_t ncells)
     L.block_sum = take((size_t)L.nblocks_cells * 4);
     L.tile_rec = take((size_t)L.ntiles * kTileRec * 4);
     L.carry = take((size_t)L.ntiles * kTileRec * 4);
-    L.class_list = take((size_t)kNumClasses * ncells * 4);
+    L.class_list = take((size_t)kNumClasses * ncells * 16);
     L.zero = take(kZeroWords * 4);
     L.counters = take(8 * 8);
     L.flags = take(4);
@@ -116,6 +116,8 @@ struct cuba_ctx {
     double *h_obs;       // pinned staging for observables
     cudaStream_t cls_stream[kNumClasses] = {};   // the collision classes run concurrently, fenced into `stream`
     cudaEvent_t ev_fork = nullptr, ev_join[kNumClasses] = {};
+    bool fuse_hist = true;   // CUBA_OPT_FUSE_HIST
+    double pre_dt = 0.0;     // > 0: cnt / carry already hold the histogram of the next step for this dt
     int prof_mode = 0;   // 0 off, 1 events per kernel (collision classes as one concurrent group), 2 classes serialised
     bool prof_on = false;
     std::vector<cudaEvent_t> prof_pool;          // reused events
@@ -181,7 +183,7 @@ static int sync_and_check(cuba_ctx *ctx)
     return device_flags_to_error(f);
 }
 
-enum { G_MEMSET = 0, G_STREAM_HIST, G_GATHER, G_SCAN, G_CELL_START, G_CARRY, G_SCATTER, G_COLLIDE_ALL, G_COLLIDE0 };
+enum { G_MEMSET = 0, G_STREAM_HIST, G_GATHER, G_SCAN, G_CELL_START, G_CARRY, G_DEST_BASE, G_SCATTER, G_COLLIDE_ALL, G_COLLIDE0 };
 static_assert(G_COLLIDE0 + kNumClasses == CUBA_PROFILE_GROUPS, "profile groups");
 
 static void prof_mark(cuba_ctx *ctx, int group)
@@ -345,12 +347,19 @@ struct TraceDev {
 };
 
 template <bool TRACE>
-static int launch_collide(cuba_ctx *ctx, double base, const TraceDev *td)
+static int launch_collide(cuba_ctx *ctx, double base, const TraceDev *td, double next_dt)
 {
     const Layout &lay = ctx->lay;
     Soa &cur = ctx->set[ctx->cur];
     CollideParams P{};
     P.seed = ctx->seed; P.t = ctx->t; P.base = base;
+    P.next_dt = next_dt; P.g = ctx->g;
+    P.x = cur.x; P.y = cur.y; P.z = cur.z;
+    P.cnt = ctx->at<uint32_t>(lay.cnt); P.carry = ctx->at<uint32_t>(lay.carry);
+    if (next_dt > 0.0) {      // the scatter of this step has consumed the offsets; empty cells must read as zero
+        CU(cudaMemsetAsync(P.cnt, 0, (size_t)kDirs * ctx->g.ncells * 4, ctx->stream));
+        prof_mark(ctx, G_MEMSET);
+    }
     for (uint32_t r = 0; r < 10; ++r) {               // Philox4x32-10 key schedule (Salmon et al., SC'11)
         P.rk[2 * r] = (uint32_t)ctx->seed + r * 0x9E3779B9u;
         P.rk[2 * r + 1] = (uint32_t)(ctx->seed >> 32) + r * 0xBB67AE85u;
@@ -365,7 +374,7 @@ static int launch_collide(cuba_ctx *ctx, double base, const TraceDev *td)
         P.tr_P = td->P; P.tr_u = td->u; P.tr_dec = td->dec;
     }
     uint32_t *zero = ctx->at<uint32_t>(lay.zero);
-    uint32_t *lists = ctx->at<uint32_t>(lay.class_list);
+    uint4 *lists = ctx->at<uint4>(lay.class_list);
     auto cls = [&](int k) { P.list = lists + (size_t)k * ctx->g.ncells; P.list_count = zero + k; P.work = zero + 8 + k; };
     // The classes are independent (disjoint cells): fork them onto their own streams so that
     // small classes fill the tail of the big ones, then join back into the caller's stream.
@@ -422,14 +431,18 @@ static int enqueue_bin(cuba_ctx *ctx, double dt, uint32_t *cell_of_pid)
     Soa &in = ctx->set[ctx->cur], &outp = ctx->set[1 - ctx->cur];
     uint32_t *cnt = ctx->at<uint32_t>(lay.cnt);
     uint32_t *zero = ctx->at<uint32_t>(lay.zero);
+    const bool have_hist = ctx->pre_dt > 0.0 && ctx->pre_dt == dt;   // written by the previous step's collision kernel
+    ctx->pre_dt = 0.0;
     prof_mark(ctx, -1);
-    CU(cudaMemsetAsync(cnt, 0, (size_t)kDirs * ncells * 4, st));
-    prof_mark(ctx, G_MEMSET);
-    k_stream_hist<<<ctx->grid_hist, kTileThreads, 2 * sizeof(TileStage<6>), st>>>(ctx->g, dt, n, lay.ntiles, in, cnt, ctx->at<uint32_t>(lay.tile_rec),
-                                                                  ctx->at<uint32_t>(lay.flags));
-    LAUNCHED();
-    prof_mark(ctx, G_STREAM_HIST);
-    k_gather<<<(unsigned)lay.nblocks_cells, 256, 0, st>>>(ctx->g, cnt, ctx->at<uint32_t>(lay.count_new),
+    if (!have_hist) {
+        CU(cudaMemsetAsync(cnt, 0, (size_t)kDirs * ncells * 4, st));
+        prof_mark(ctx, G_MEMSET);
+        k_stream_hist<<<ctx->grid_hist, kTileThreads, 2 * sizeof(TileStage<6>), st>>>(ctx->g, dt, n, lay.ntiles, in, cnt, ctx->at<uint32_t>(lay.tile_rec),
+                                                                      ctx->at<uint32_t>(lay.flags));
+        LAUNCHED();
+        prof_mark(ctx, G_STREAM_HIST);
+    }
+    k_gather<<<(unsigned)lay.nblocks_cells, kGatherThreads, 0, st>>>(ctx->g, cnt, ctx->at<uint32_t>(lay.count_new),
                                                           ctx->at<uint32_t>(lay.block_sum));
     LAUNCHED();
     prof_mark(ctx, G_GATHER);
@@ -443,19 +456,24 @@ static int enqueue_bin(cuba_ctx *ctx, double dt, uint32_t *cell_of_pid)
     ct.max_n[kSmemClasses] = 0xFFFFFFFFu;
     k_cell_start<<<(unsigned)lay.nblocks_cells, 256, 0, st>>>(ncells, ctx->at<uint32_t>(lay.count_new),
                                                               ctx->at<uint32_t>(lay.block_sum), ctx->at<uint32_t>(lay.cell_start),
-                                                              ct, zero, ctx->at<uint32_t>(lay.class_list),
+                                                              ct, zero, ctx->at<uint4>(lay.class_list),
                                                               ctx->at<unsigned long long>(lay.max_occ));
     LAUNCHED();
     prof_mark(ctx, G_CELL_START);
-    k_carry<<<(unsigned)((lay.ntiles + 7) / 8), 256, 0, st>>>((int)lay.ntiles, ctx->at<uint32_t>(lay.tile_rec),
-                                                              ctx->at<uint32_t>(lay.carry));
+    if (!have_hist) {
+        k_carry<<<(unsigned)((lay.ntiles + 7) / 8), 256, 0, st>>>((int)lay.ntiles, ctx->at<uint32_t>(lay.tile_rec),
+                                                                  ctx->at<uint32_t>(lay.carry));
+        LAUNCHED();
+        prof_mark(ctx, G_CARRY);
+    }
+    k_dest_base<<<dim3((unsigned)lay.nblocks_cells, kDirs), 256, 0, st>>>(ctx->g, cnt, ctx->at<uint32_t>(lay.cell_start));
     LAUNCHED();
-    prof_mark(ctx, G_CARRY);
+    prof_mark(ctx, G_DEST_BASE);
     if (cell_of_pid)
-        k_scatter<true><<<ctx->grid_scat, kTileThreads, 2 * sizeof(TileStage<7>), st>>>(ctx->g, dt, n, lay.ntiles, in, outp, cnt, ctx->at<uint32_t>(lay.cell_start),
+        k_scatter<true><<<ctx->grid_scat, kTileThreads, 2 * sizeof(TileStage<7>), st>>>(ctx->g, dt, n, lay.ntiles, in, outp, cnt,
                                                                        ctx->at<uint32_t>(lay.carry), cell_of_pid);
     else
-        k_scatter<false><<<ctx->grid_scat, kTileThreads, 2 * sizeof(TileStage<7>), st>>>(ctx->g, dt, n, lay.ntiles, in, outp, cnt, ctx->at<uint32_t>(lay.cell_start),
+        k_scatter<false><<<ctx->grid_scat, kTileThreads, 2 * sizeof(TileStage<7>), st>>>(ctx->g, dt, n, lay.ntiles, in, outp, cnt,
                                                                         ctx->at<uint32_t>(lay.carry), nullptr);
     LAUNCHED();
     prof_mark(ctx, G_SCATTER);
@@ -473,8 +491,10 @@ int cuba_step(cuba_ctx *ctx, int nsteps, double dt, double sigma)
     for (int s = 0; s < nsteps; ++s) {
         rc = enqueue_bin(ctx, dt, nullptr);
         if (rc != CUBA_OK) return rc;
-        rc = launch_collide<false>(ctx, base, nullptr);
+        const double next_dt = ctx->fuse_hist ? dt : 0.0;
+        rc = launch_collide<false>(ctx, base, nullptr, next_dt);
         if (rc != CUBA_OK) return rc;
+        ctx->pre_dt = next_dt;
         ctx->t += 1;
         ctx->steps += 1;
     }
@@ -527,7 +547,7 @@ int cuba_step_traced(cuba_ctx *ctx, double dt, double sigma, cuba_trace *out)
         CU(cudaMalloc(&td.pa, m * 4)); CU(cudaMalloc(&td.pb, m * 4));
         CU(cudaMalloc(&td.P, m * 8)); CU(cudaMalloc(&td.u, m * 8)); CU(cudaMalloc(&td.dec, m));
         CU(cudaMemcpy(td.off, off.data(), ((size_t)ncells + 1) * 8, cudaMemcpyHostToDevice));
-        r = launch_collide<true>(ctx, base, &td);
+        r = launch_collide<true>(ctx, base, &td, 0.0);
         if (r != CUBA_OK) return r;
         ctx->t += 1;
         ctx->steps += 1;
@@ -547,6 +567,15 @@ int cuba_step_traced(cuba_ctx *ctx, double dt, double sigma, cuba_trace *out)
     rc = body();
     release();
     return rc;
+}
+
+int cuba_set_option(cuba_ctx *ctx, int option, int value)
+{
+    if (!ctx) return CUBA_ERR_NULL;
+    if (option != CUBA_OPT_FUSE_HIST || (value != 0 && value != 1)) return CUBA_ERR_VALUE;
+    ctx->fuse_hist = value != 0;
+    if (!ctx->fuse_hist) ctx->pre_dt = 0.0;
+    return CUBA_OK;
 }
 
 int cuba_observables(cuba_ctx *ctx, double total[4], int nslab, double *edens)
@@ -603,7 +632,7 @@ int cuba_get_particles(cuba_ctx *ctx, uint32_t *pid, double *x, double *y, doubl
 const char *cuba_profile_name(int group)
 {
     static const char *names[CUBA_PROFILE_GROUPS] = {
-        "memset_cnt", "k_stream_hist", "k_gather", "k_scan_blocks", "k_cell_start", "k_carry", "k_scatter",
+        "memset_cnt", "k_stream_hist", "k_gather", "k_scan_blocks", "k_cell_start", "k_carry", "k_dest_base", "k_scatter",
         "k_collide (all classes, concurrent)"};
 #define CUBA_STR2(x) #x
 #define CUBA_STR(x) CUBA_STR2(x)

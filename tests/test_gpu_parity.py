@@ -138,6 +138,38 @@ def test_k_steps_equal_k_single_steps_and_determinism(cuba):
     assert np.array_equal(a.observables(16)[1], c.observables(16)[1])   # reductions are order-fixed
 
 
+def test_fused_histogram_schedule_is_bit_identical(cuba, oracle_mod):
+    """CUBA_OPT_FUSE_HIST: the collision kernel of step t writes the counting-sort histogram
+    of step t+1.  Same results as the separate pass and as the oracle, also when dt changes
+    between calls (the prepared histogram is for the wrong dt and must be discarded), after a
+    traced step, and for all size classes incl. the overflow kernel and single-particle cells."""
+    w = workloads.riemann(L=(6.0, 3.0, 2.0), ncell=(12, 3, 2), r_test=90.0, sigma_gev2=50.0, dt=0.05, seed=21)
+    fused, plain = cuba.Cuba.from_workload(w), cuba.Cuba.from_workload(w)
+    plain.set_option(1, 0)
+    o = oracle_mod.Oracle.from_workload(w)
+    schedule = [(3, w.dt), (1, w.dt), (2, 0.5 * w.dt), (1, w.dt), (2, w.dt)]
+    for k, dt in schedule:
+        fused.step(k, dt, w.sigma)
+        plain.step(k, dt, w.sigma)
+        o.step(k, dt, w.sigma)
+        for a, b, c in zip(fused.particles(), plain.particles(), o.particles()):
+            assert np.array_equal(a, b) and np.array_equal(a, c)
+        assert np.array_equal(fused.cell_start(), o.cells()[1])
+    fused.step_traced(w.dt, w.sigma)
+    plain.step_traced(w.dt, w.sigma)
+    fused.step(2, w.dt, w.sigma)
+    plain.step(2, w.dt, w.sigma)
+    o.step(3, w.dt, w.sigma)
+    for a, b, c in zip(fused.particles(), plain.particles(), o.particles()):
+        assert np.array_equal(a, b) and np.array_equal(a, c)
+    cf, cp, co = fused.counters(), plain.counters(), o.counters()
+    assert (cf.pairs, cf.collisions, cf.rounds) == (cp.pairs, cp.collisions, cp.rounds) == \
+           (co["pairs"], co["collisions"], co["rounds"])
+    assert cf.device_flags == 0 and cp.device_flags == 0
+    with pytest.raises(cuba.CubaError):
+        fused.set_option(99, 1)
+
+
 @pytest.mark.parametrize("case", ["single", "two", "one_cell_overflow", "flat_grid", "empty_cells"])
 def test_edge_cases_match_oracle(cuba, oracle_mod, case):
     rng = np.random.default_rng(77)
