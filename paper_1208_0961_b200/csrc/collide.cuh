@@ -16,6 +16,10 @@
 
 namespace cuba {
 
+#ifndef CUBA_FORCE_SLOW_PATHS   // test builds set this to 1: every element / pair takes the rare paths
+#define CUBA_FORCE_SLOW_PATHS 0
+#endif
+
 struct CollideParams {
     uint64_t seed;
     uint32_t rk[20];      // Philox round keys: rk[2r] = seed_lo + r*0x9E3779B9, rk[2r+1] = seed_hi + r*0xBB67AE85
@@ -270,6 +274,68 @@ __device__ __forceinline__ int next_direction(const Geom &g, double dt, int ix0,
     return ((unsigned)dx <= 2u && (unsigned)dy <= 2u && (unsigned)dz <= 2u) ? (dx * 9 + dy * 3 + dz) : -1;
 }
 
+// Per-cell constants of the fused histogram, written by thread 0 when the cell is set up.
+struct HistCell {
+    int i0[3];            // cell coordinates (x slowest)
+    double i0d[3];        // the same as doubles
+    int lo_code[3];       // per-axis direction component of a particle that leaves through the lower face:
+    int hi_code[3];       //   0 / 2, or 1 where that face is a wall (elastic reflection back into the cell, A12)
+};
+
+__device__ __forceinline__ void hist_cell_setup(const Geom &g, uint32_t c, HistCell *h)
+{
+    h->i0[2] = (int)(c % (uint32_t)g.nc[2]);
+    h->i0[1] = (int)((c / (uint32_t)g.nc[2]) % (uint32_t)g.nc[1]);
+    h->i0[0] = (int)(c / ((uint32_t)g.nc[2] * (uint32_t)g.nc[1]));
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        h->i0d[k] = (double)h->i0[k];
+        h->lo_code[k] = h->i0[k] == 0 ? 1 : 0;
+        h->hi_code[k] = h->i0[k] == g.nc[k] - 1 ? 1 : 2;
+    }
+}
+
+__device__ __forceinline__ double rcp_approx(double a)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a));   // ~20 good bits from the upper word
+    return r;
+}
+
+// One axis of the guarded estimate: t = position after the move in units of the cell edge,
+// relative to the cell's lower face (the cell is [0,1)).  Away from the faces (and dt < cell edge
+// means |t - 0.5| < 1.5) the direction component follows from t alone: inside -> 1; beyond the
+// upper face -> 2, beyond the lower -> 0, or 1 if that face is a wall (the reflected position lies
+// in the same cell).  Within kHistEps of a face -- or anything unexpected, NaN included -- the
+// caller redoes the particle with the exact operation order.
+constexpr double kHistEps = 1e-4;   // the estimate is good to ~1e-9; the band is generous
+
+__device__ __forceinline__ int axis_code(double t, int lo_code, int hi_code, bool &safe)
+{
+    const double a = fabs(t - 0.5);
+    const bool inside = a < 0.5 - kHistEps;
+    const bool outside = a > 0.5 + kHistEps && a < 1.5 - kHistEps;
+    safe = safe && (inside || outside);
+    return inside ? 1 : (t > 0.5 ? hi_code : lo_code);
+}
+
+// Direction code of a particle: the same value as next_direction(), computed without the fp64
+// division (hardware reciprocal estimate + one Newton step, fused multiply-adds) wherever the
+// outcome is not within kHistEps of changing.
+__device__ __forceinline__ int next_direction_guarded(const Geom &g, double dt, const HistCell &h,
+                                                      double x, double y, double z, double px, double py, double pz, double E)
+{
+    double r = rcp_approx(E);
+    r = __fma_rn(r, __fma_rn(-E, r, 1.0), r);
+    const double w = dt * r;
+    bool safe = true;
+    const int dx = axis_code(__fma_rn(__fma_rn(px, w, x), g.inv_d[0], -h.i0d[0]), h.lo_code[0], h.hi_code[0], safe);
+    const int dy = axis_code(__fma_rn(__fma_rn(py, w, y), g.inv_d[1], -h.i0d[1]), h.lo_code[1], h.hi_code[1], safe);
+    const int dz = axis_code(__fma_rn(__fma_rn(pz, w, z), g.inv_d[2], -h.i0d[2]), h.lo_code[2], h.hi_code[2], safe);
+    if (CUBA_FORCE_SLOW_PATHS || !safe) return next_direction(g, dt, h.i0[0], h.i0[1], h.i0[2], x, y, z, px, py, pz, E);
+    return dx * 9 + dy * 3 + dz;
+}
+
 // Tile segments of a cell: the flat passes work on tiles of kTile consecutive slots; segment k of
 // the cell [lo, lo+n) is its intersection with tile (lo / kTile) + k.  s_seg[k][d] counts the
 // cell's particles of segment k that move in direction d.  From it:
@@ -384,9 +450,6 @@ __device__ __forceinline__ uint32_t block_exclusive_scan_1b(uint32_t v, uint32_t
     return __shfl_sync(0xFFFFFFFFu, winc - w, wid) + inc - v;
 }
 
-#ifndef CUBA_FORCE_SLOW_PATHS   // test builds set this to 1: every element / pair takes the rare paths
-#define CUBA_FORCE_SLOW_PATHS 0
-#endif
 
 // Rare path of the in-bucket ranking: buckets with more than four elements, or equal 32-bit
 // keys (then the pid decides, A7; the keys of the other particles are recomputed).
@@ -428,6 +491,7 @@ struct CtaStats {
     double scale, hscale;     // Eq. 3 factor cn*base/R of the current cell, and half of it
     uint32_t lo;              // first slot of the current cell
     uint32_t near;            // near-threshold decisions of this CTA (A16; rare)
+    HistCell h;               // fused histogram: constants of the current cell
 };
 
 // Per-thread accumulators over all cells of a CTA, flushed once at the end of the kernel.
@@ -458,6 +522,7 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
     if (tid == 0) {
         const double scale = (cn * P.base) / (double)R;
         stats->scale = scale; stats->hscale = 0.5 * scale; stats->lo = lo;
+        if (hist) hist_cell_setup(P.g, c, &stats->h);
     }
     const uint32_t npairs = n >> 1, nb = 2u * n, last = n - 1u;
     uint16_t *sb16 = reinterpret_cast<uint16_t *>(sbkt);
@@ -680,10 +745,10 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
     __syncthreads();
     const uint32_t lo_w = *reinterpret_cast<volatile uint32_t *>(&stats->lo);
     // positions for the fused histogram: all loads of a thread in flight before anything waits on them
-#ifndef CUBA_HB_ALL
-#define CUBA_HB_ALL 0
+#ifndef CUBA_HB6
+#define CUBA_HB6 2
 #endif
-    constexpr int HB = (THREADS >= 512 || !CUBA_HB_ALL) ? ((ITEMS % 2 == 0) ? 2 : 1) : ITEMS;
+    constexpr int HB = (ITEMS == 6) ? CUBA_HB6 : ((ITEMS % 2 == 0) ? 2 : 1);
     double xx[HB], yy[HB], zz[HB];
     if (hist && HB == ITEMS) {
 #pragma unroll
@@ -708,9 +773,7 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
     // ---- fused histogram of the next step (S1-S3 of step t+1 on the final momenta) ----------
     if (hist) {
         const uint32_t T0 = lo_w / kTile;
-        const int iz0 = (int)(c % (uint32_t)P.g.nc[2]);
-        const int iy0 = (int)((c / (uint32_t)P.g.nc[2]) % (uint32_t)P.g.nc[1]);
-        const int ix0 = (int)(c / ((uint32_t)P.g.nc[2] * (uint32_t)P.g.nc[1]));
+        const HistCell &hc = stats->h;
 #pragma unroll
         for (int g = 0; g < ITEMS / HB; ++g) {
             if ((uint32_t)(g * HB * THREADS) >= n) break;
@@ -724,8 +787,8 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
 #pragma unroll
             for (int i = 0; i < HB; ++i) {
                 const uint32_t j = tid + (g * HB + i) * THREADS, jj = min(j, last);
-                const int d = next_direction(P.g, P.next_dt, ix0, iy0, iz0, xx[i], yy[i], zz[i],
-                                             sp0[jj], sp1[jj], sp2[jj], sE[jj]);
+                const int d = next_direction_guarded(P.g, P.next_dt, hc, xx[i], yy[i], zz[i],
+                                                     sp0[jj], sp1[jj], sp2[jj], sE[jj]);
                 const bool valid = j < n;
                 if (valid && d < 0) atomicOr(P.flags, kFlagMoved);
                 const uint32_t key = ((lo_w + jj) / kTile - T0) * kDirs + (uint32_t)max(d, 0);
@@ -809,23 +872,12 @@ k_collide(CollideParams P)
     __shared__ CtaStats s_stats;
     __shared__ uint32_t s_seg[((CAP + kTile - 2) / kTile + 1) * kDirs];   // a cell of CAP particles spans at most this many tiles
 
-    // Static round-robin over the class list: the cells of a class have similar populations, and
-    // a known next index lets the next entry be loaded a whole cell ahead (no atomic -> list ->
-    // cell_start chain of dependent global loads between cells).
+    // Dynamic work distribution, claimed one cell ahead so that the next cell can be prefetched
+    // into L2.  (Measured alternatives, both slower because they lengthen the tail of the list:
+    // a static round-robin, +0.10 ms at configs[2]; claiming three cells ahead, +0.09 ms.)
     const uint32_t nlist = *P.list_count;
     if (threadIdx.x == 0) s_stats.near = 0;
     ThreadStats acc{0ull, 0ull, 0u};
-#ifndef CUBA_STATIC_RR
-#define CUBA_STATIC_RR 0
-#endif
-#if CUBA_STATIC_RR
-    uint32_t item = blockIdx.x;
-    uint4 cur = make_uint4(0u, 0u, 0u, 0u);
-    if (item < nlist) cur = P.list[item];
-    for (; item < nlist; item += gridDim.x) {
-        uint4 nxt = make_uint4(0u, 0u, 0u, 0u);
-        if (item + gridDim.x < nlist) nxt = P.list[item + gridDim.x];   // first used after the staging barrier
-#else
     __shared__ uint32_t s_item[2];
     if (threadIdx.x == 0) s_item[0] = atomicAdd(P.work, 1u);
     __syncthreads();
@@ -837,8 +889,7 @@ k_collide(CollideParams P)
         __syncthreads();
         item = s_item[(it + 1) & 1];
         uint4 nxt = make_uint4(0u, 0u, 0u, 0u);
-        if (item < nlist) nxt = P.list[item];
-#endif
+        if (item < nlist) nxt = P.list[item];   // first used after the staging barrier
         collide_cell_smem<THREADS, ITEMS, G, TRACE>(P, cur.x, cur.y, cur.z, sp0, sp1, sp2, sE, spid, spark, sbkt, sord,
                                                     s_warp, &s_stats, s_seg, acc, nxt.y, nxt.z);
         __syncthreads();
