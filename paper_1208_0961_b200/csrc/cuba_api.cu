@@ -62,7 +62,7 @@ struct Layout {
     int64_t ntiles, nblocks_cells, rs_blocks, arena_entries;
 };
 
-constexpr int kObsGrid = 296;
+constexpr int kObsGrid = 148 * 4;   // resident CTAs: 4 per SM at 64 registers
 constexpr int kZeroWords = 32;   // class_count[8], work[8], arena cursor (u64 = 2 words), pad
 
 Layout make_layout(int64_t n, int64_t ncells)
@@ -591,7 +591,7 @@ int cuba_observables(cuba_ctx *ctx, double total[4], int nslab, double *edens)
     k_observe_partial<<<kObsGrid, kObsThreads, (size_t)kObsWarps * nslab * 8, st>>>(ctx->n, cur.x, cur.px, cur.py, cur.pz,
                                                                                   inv_w, nslab, partial);
     LAUNCHED();
-    k_observe_final<<<(4 + nslab + 255) / 256, 256, 0, st>>>(kObsGrid, nslab, partial, vol, result);
+    k_observe_final<<<(4 + nslab + 7) / 8, 256, 0, st>>>(kObsGrid, nslab, partial, vol, result);
     LAUNCHED();
     CU(cudaMemcpyAsync(ctx->h_obs, result, (size_t)(4 + nslab) * 8, cudaMemcpyDeviceToHost, st));
     int rc = sync_and_check(ctx);

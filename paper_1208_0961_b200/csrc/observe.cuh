@@ -9,10 +9,12 @@ namespace cuba {
 
 constexpr int kObsThreads = 256;
 constexpr int kObsWarps = kObsThreads / 32;
+constexpr int kObsItems = 4;                    // particles per thread per tile: 16 independent loads in flight
+constexpr int kObsTile = kObsThreads * kObsItems;
 constexpr int kObsMaxSlabs = 1024;
 
 // partial layout per block: [0..3] totals, [4 .. 4+nslab) slab energies
-__global__ void __launch_bounds__(kObsThreads)
+__global__ void __launch_bounds__(kObsThreads, 4)
 k_observe_partial(int64_t n, const double *__restrict__ x, const double *__restrict__ px,
                   const double *__restrict__ py, const double *__restrict__ pz, double inv_w,
                   int nslab, double *__restrict__ partial)
@@ -24,29 +26,32 @@ k_observe_partial(int64_t n, const double *__restrict__ x, const double *__restr
     for (int s = lane; s < nslab; s += 32) bins[s] = 0.0;
     __syncwarp();
     double tE = 0.0, tx = 0.0, ty = 0.0, tz = 0.0;
-    const int64_t ntiles = (n + kObsThreads - 1) / kObsThreads;
+    const int64_t ntiles = (n + kObsTile - 1) / kObsTile;
     for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int64_t i = tile * kObsThreads + tid;
-        const bool valid = i < n;
-        double E = 0.0;
-        int slab = -1;
-        if (valid) {
-            const double a = px[i], b = py[i], c = pz[i];
-            E = energy(a, b, c);
-            tE += E; tx += a; ty += b; tz += c;
-            slab = min(max(__double2int_rz(x[i] * inv_w), 0), nslab - 1);
-        }
-        // the store is sorted with x slowest, so a warp sees one or two slabs: peel them off
-        uint32_t todo = __ballot_sync(0xFFFFFFFFu, valid);
-        while (todo) {
-            const int leader = __ffs(todo) - 1;
-            const int s0 = __shfl_sync(0xFFFFFFFFu, slab, leader);
-            const bool mine = valid && slab == s0;
-            double v = mine ? E : 0.0;
+        double a[kObsItems], b[kObsItems], c[kObsItems], xx[kObsItems];
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
-            if (lane == 0) bins[s0] += v;
-            todo &= ~__ballot_sync(0xFFFFFFFFu, mine);
+        for (int k = 0; k < kObsItems; ++k) {
+            const int64_t i = min(tile * kObsTile + k * kObsThreads + tid, n - 1);
+            a[k] = px[i]; b[k] = py[i]; c[k] = pz[i]; xx[k] = x[i];
+        }
+#pragma unroll
+        for (int k = 0; k < kObsItems; ++k) {
+            const bool valid = tile * kObsTile + k * kObsThreads + tid < n;
+            const double E = valid ? energy(a[k], b[k], c[k]) : 0.0;
+            if (valid) { tE += E; tx += a[k]; ty += b[k]; tz += c[k]; }
+            const int slab = valid ? min(max(__double2int_rz(xx[k] * inv_w), 0), nslab - 1) : -1;
+            // the store is sorted with x slowest, so a warp sees one or two slabs: peel them off
+            uint32_t todo = __ballot_sync(0xFFFFFFFFu, valid);
+            while (todo) {
+                const int leader = __ffs(todo) - 1;
+                const int s0 = __shfl_sync(0xFFFFFFFFu, slab, leader);
+                const bool mine = valid && slab == s0;
+                double v = mine ? E : 0.0;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+                if (lane == 0) bins[s0] += v;
+                todo &= ~__ballot_sync(0xFFFFFFFFu, mine);
+            }
         }
     }
 #pragma unroll
@@ -71,16 +76,20 @@ k_observe_partial(int64_t n, const double *__restrict__ x, const double *__restr
     }
 }
 
-// result[0..3] totals, result[4..] = slab energy / (r_test * V_slab)
+// result[0..3] totals, result[4..] = slab energy / (r_test * V_slab).  One warp per output: lane l
+// adds the partials of blocks l, l+32, ... in that order, then a fixed shuffle tree: the order of
+// the summation does not depend on scheduling.
 __global__ void __launch_bounds__(256)
 k_observe_final(int nblocks, int nslab, const double *__restrict__ partial, double vol,
                 double *__restrict__ result)
 {
-    const int e = blockIdx.x * 256 + threadIdx.x;
+    const int e = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     if (e >= 4 + nslab) return;
     double s = 0.0;
-    for (int b = 0; b < nblocks; ++b) s += partial[(size_t)b * (4 + nslab) + e];
-    result[e] = (e < 4) ? s : s / vol;
+    for (int b = lane; b < nblocks; b += 32) s += partial[(size_t)b * (4 + nslab) + e];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
+    if (lane == 0) result[e] = (e < 4) ? s : s / vol;
 }
 
 }  // namespace cuba
