@@ -43,6 +43,12 @@ BYTES_STEP = BYTES_STREAM_HIST + BYTES_SCATTER + BYTES_COLLIDE   # 204, SURVEY.m
 BYTES_STEP_FUSED = BYTES_SCATTER + BYTES_COLLIDE_FUSED           # 180: what the fused schedule actually has to move
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
+# `ncu --set full` capture (profiles/r01_v4_summary.md): (config, fused schedule, kernel group) -> bytes.
+# The group is the hot collision class (1.487 + 0.508 GB) plus the cold one (0.138 + 0.029 GB).
+NCU_TRAFFIC = {(2, True, "k_collide (all classes, concurrent)"): 2.162e9}
+
+
 def peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -316,7 +322,7 @@ def main():
             "gpu_launches": int(launches),
             "clocks": sampler.summary(),
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                         "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((args.config, fused, dom)), "peak_source": peak_src,
                          "alg_bytes_per_launch": alg.get(dom, 0),
                          "step": {"alg_bytes_per_particle": BYTES_STEP,
                                   "moved_bytes_per_particle": BYTES_STEP_FUSED if fused else BYTES_STEP,
