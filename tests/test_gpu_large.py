@@ -24,7 +24,7 @@ def cuba():
     return c
 
 
-@pytest.mark.parametrize("config", [1, 2])
+@pytest.mark.parametrize("config", [1, 2, 3, 4])
 def test_full_size_step_sampled_against_oracle(cuba, oracle_mod, config):
     w = workloads.make(config)
     g = cuba.Cuba.from_workload(w)
