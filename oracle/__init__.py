@@ -67,6 +67,8 @@ def lib():
         L.oracle_step.argtypes = [c_void_p, c_int, c_double, c_double]
         L.oracle_step.restype = c_int
         L.oracle_observables.argtypes = [c_void_p, dp, c_int, dp]
+        L.oracle_observables_lrf.argtypes = [c_void_p, c_int, dp, dp]
+        L.oracle_landau_match.argtypes = [c_double] * 5 + [dp]
         L.oracle_get_particles.argtypes = [c_void_p, u32p] + [dp] * 6
         L.oracle_get_cells.argtypes = [c_void_p, u32p, u32p]
         L.oracle_counters.argtypes = [c_void_p, POINTER(c_uint64), dp]
@@ -161,6 +163,13 @@ def scatter(pa, pb, Ea, Eb, s, nhat):
     return qa, qb
 
 
+def landau_match(T00, T0x, Txx, Tyy, Tzz):
+    """(e, v, P_L, P_T) of one slab's tensor components."""
+    o = np.zeros(4)
+    lib().oracle_landau_match(float(T00), float(T0x), float(Txx), float(Tyy), float(Tzz), _dp(o))
+    return tuple(o)
+
+
 def shuffle_order(seed, t, rho, pids):
     pids = np.ascontiguousarray(pids, dtype=np.uint32)
     out = np.zeros_like(pids)
@@ -214,6 +223,13 @@ class Oracle:
         ed = np.zeros(nslab)
         lib().oracle_observables(self._h, _dp(tot), int(nslab), _dp(ed))
         return tot, ed
+
+    def observables_lrf(self, nslab):
+        """(T, lrf): T[5, nslab] = T00, T0x, Txx, Tyy, Tzz; lrf[4, nslab] = e, v, P_L, P_T."""
+        T = np.zeros((5, nslab))
+        out = np.zeros((4, nslab))
+        lib().oracle_observables_lrf(self._h, int(nslab), _dp(T), _dp(out))
+        return T, out
 
     def particles(self):
         """(pid, x, y, z, px, py, pz) in array order."""

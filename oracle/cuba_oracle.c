@@ -21,6 +21,7 @@
  *   44      testparticles (P22 reduced by r_test); boost to CM, choose the momentum
  *           randomly, boost back; elastic reflection off the six walls        -> S2, S5
  *   66      total energy is conserved                                         -> observables
+ *   62-72   energy density / flow of the Riemann problem, viscosity            -> LRF observables
  * Where the paper is silent (pair enumeration, shuffle, RNG, order inside a step, odd
  * cells, P > 1) the readings A1..A19 of DESIGN.md are followed; each is named at its use.
  *
@@ -29,7 +30,9 @@
  * four-momentum conservation and agreement with an explicit 4x4 Lorentz-matrix boost;
  * run-level energy conservation; collision rate vs the closed form; isotropy (KS);
  * thermal box stays Boltzmann (KS); initial energy density 3nT; free-streaming Riemann
- * closed form; counting sort vs brute force; pairing uniform over perfect matchings.
+ * closed form; counting sort vs brute force; pairing uniform over perfect matchings;
+ * Landau matching vs numpy's eigen-decomposition, hand-built slabs, tracelessness, and a
+ * boosted thermal ensemble (e = 3 n T, v = beta).
  * Parity unpinned: the paper's Fig. 2-4 curves and the BAMPS overlay (images and BAMPS
  * are not available).
  */
@@ -516,6 +519,60 @@ void oracle_observables(const oracle_state *st, double total[4], int nslab, doub
     double vol = ((st->n_test * (st->box[0] / (double)nslab)) * st->box[1]) * st->box[2];
     for (int j = 0; j < nslab; ++j) edens[j] = (slab[j].s + slab[j].c) / vol;
     free(slab);
+}
+
+/* ------------------------------------------------------------------------------------
+ * Local-rest-frame observables (the quantities the Riemann profiles of
+ * PAPER.md:66-72 and the viscosity discussion of PAPER.md:62-64, 74-82 are about).
+ * Kinetic energy-momentum tensor of the testparticles of slab j (transversely homogeneous
+ * set-up):  T^{mu nu}_j = sum_{i in j} p_i^mu p_i^nu / E_i / (r_test V_slab),
+ * components T00, T0x, Txx, Tyy, Tzz (T0y, T0z, Txy... vanish by symmetry on average and are
+ * not used).  Per particle: w = 1/E, contributions E, px, (px*px)*w, (py*py)*w, (pz*pz)*w.
+ * Landau matching for a flow along x (reading A22): the energy density in the local
+ * rest frame is the timelike eigenvalue of T^mu_nu restricted to (t, x),
+ *     e = ((T00 - Txx) + sqrt((T00 + Txx)^2 - 4 T0x^2)) / 2,   v = T0x / (e + Txx),
+ *     P_L = (e - T00) + Txx  (minus the other eigenvalue),      P_T = (Tyy + Tzz) / 2.
+ * A negative discriminant (rounding) counts as 0; e + Txx = 0 (empty slab) gives v = 0.
+ * ---------------------------------------------------------------------------------- */
+void oracle_landau_match(double T00, double T0x, double Txx, double Tyy, double Tzz, double out[4])
+{
+    double tr = T00 + Txx;
+    double disc = tr * tr - 4.0 * (T0x * T0x);
+    if (!(disc > 0.0)) disc = 0.0;
+    double e = 0.5 * ((T00 - Txx) + sqrt(disc));
+    double den = e + Txx;
+    out[0] = e;
+    out[1] = (den > 0.0) ? T0x / den : 0.0;
+    out[2] = (e - T00) + Txx;
+    out[3] = 0.5 * (Tyy + Tzz);
+}
+
+/* T: 5*nslab doubles (T00[nslab], T0x[nslab], Txx, Tyy, Tzz); lrf: 4*nslab (e, v, P_L, P_T) */
+void oracle_observables_lrf(const oracle_state *st, int nslab, double *T, double *lrf)
+{
+    ksum *acc = (ksum *)calloc((size_t)5 * nslab, sizeof(ksum));
+    double inv_w = (double)nslab / st->box[0];
+    for (int64_t i = 0; i < st->n; ++i) {
+        double px = st->px[i], py = st->py[i], pz = st->pz[i];
+        double E = energy(px, py, pz);
+        double w = 1.0 / E;
+        int j = (int)(st->x[i] * inv_w);
+        if (j > nslab - 1) j = nslab - 1;
+        if (j < 0) j = 0;
+        kadd(&acc[0 * nslab + j], E);
+        kadd(&acc[1 * nslab + j], px);
+        kadd(&acc[2 * nslab + j], (px * px) * w);
+        kadd(&acc[3 * nslab + j], (py * py) * w);
+        kadd(&acc[4 * nslab + j], (pz * pz) * w);
+    }
+    double vol = ((st->n_test * (st->box[0] / (double)nslab)) * st->box[1]) * st->box[2];
+    for (int k = 0; k < 5 * nslab; ++k) T[k] = (acc[k].s + acc[k].c) / vol;
+    for (int j = 0; j < nslab; ++j) {
+        double o[4];
+        oracle_landau_match(T[j], T[nslab + j], T[2 * nslab + j], T[3 * nslab + j], T[4 * nslab + j], o);
+        for (int k = 0; k < 4; ++k) lrf[k * nslab + j] = o[k];
+    }
+    free(acc);
 }
 
 /* ------------------------------------------------------------------------------------
