@@ -128,6 +128,17 @@ int cuba_set_option(cuba_ctx *ctx, int option, int value);
  * HOST outputs; synchronises the stream and reports pending device errors. */
 int cuba_observables(cuba_ctx *ctx, double total[4], int nslab, double *edens);
 
+/* Local-rest-frame observables (the quantities behind the Riemann profiles
+ * and the viscosity discussion of PAPER.md:62-72).  Kinetic energy-momentum tensor of the
+ * testparticles per x-slab, T^{mu nu} = sum p^mu p^nu / E / (n_test * V_slab) in GeV/fm^3:
+ *   T   HOST, 5*nslab doubles: T00[nslab], T0x[nslab], Txx[nslab], Tyy[nslab], Tzz[nslab];
+ *   lrf HOST, 4*nslab doubles: e[nslab] (energy density in the local rest frame, Landau matching
+ *       for a flow along x: e = ((T00-Txx) + sqrt((T00+Txx)^2 - 4 T0x^2))/2), v[nslab] (flow
+ *       velocity T0x/(e+Txx), 0 for an empty slab), P_L[nslab] = e - T00 + Txx, P_T[nslab] =
+ *       (Tyy+Tzz)/2.
+ * 1 <= nslab <= 256 (CUBA_ERR_SIZE otherwise).  Synchronises; reports pending device errors. */
+int cuba_observables_lrf(cuba_ctx *ctx, int nslab, double *T, double *lrf);
+
 /* Where the current state lives (DEVICE pointers, valid until the next cuba_step). */
 int cuba_state(cuba_ctx *ctx, cuba_soa *out);
 

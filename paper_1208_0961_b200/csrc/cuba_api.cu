@@ -88,8 +88,10 @@ Layout make_layout(int64_t n, int64_t ncells)
     L.counters = take(8 * 8);
     L.flags = take(4);
     L.max_occ = take(8);
-    L.obs_partial = take((size_t)kObsGrid * (4 + kObsMaxSlabs) * 8);
-    L.obs_result = take((size_t)(4 + kObsMaxSlabs) * 8);
+    constexpr size_t obs_words = (4 + kObsMaxSlabs) > kLrfComp * kLrfMaxSlabs ? (4 + kObsMaxSlabs) : kLrfComp * kLrfMaxSlabs;
+    constexpr size_t res_words = (4 + kObsMaxSlabs) > 9 * kLrfMaxSlabs ? (4 + kObsMaxSlabs) : 9 * kLrfMaxSlabs;
+    L.obs_partial = take((size_t)kObsGrid * obs_words * 8);
+    L.obs_result = take(res_words * 8);
     L.arena32 = take((size_t)L.arena_entries * 16);   // also the init sort's key/value double buffers
     L.arenaE = take((size_t)L.arena_entries * 8);
     L.rsH = take((size_t)256 * L.rs_blocks * 4);
@@ -258,7 +260,7 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
         delete ctx;
         return code;
     };
-    if (!cuda_ok(cudaMallocHost(&ctx->h_obs, (4 + kObsMaxSlabs) * sizeof(double)), "cudaMallocHost")) return fail(CUBA_ERR_CUDA);
+    if (!cuda_ok(cudaMallocHost(&ctx->h_obs, (9 * kLrfMaxSlabs > 4 + kObsMaxSlabs ? 9 * kLrfMaxSlabs : 4 + kObsMaxSlabs) * sizeof(double)), "cudaMallocHost")) return fail(CUBA_ERR_CUDA);
     if (!cuda_ok(cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming), "cudaEventCreate")) return fail(CUBA_ERR_CUDA);
     for (int k = 0; k < kNumClasses; ++k) {
         if (!cuda_ok(cudaStreamCreateWithFlags(&ctx->cls_stream[k], cudaStreamNonBlocking), "cudaStreamCreate")) return fail(CUBA_ERR_CUDA);
@@ -276,8 +278,10 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
     if (rc == CUBA_OK) rc = occupancy_grid(k_scatter<false>, kTileThreads, 2 * sizeof(TileStage<7>), sms, &ctx->grid_scat);
     if (rc != CUBA_OK) return fail(rc);
     ctx->grid_o = sms;
-    if (!cuda_ok(cudaFuncSetAttribute(k_observe_partial, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    if (!cuda_ok(cudaFuncSetAttribute(k_observe_partial<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       kObsWarps * kObsMaxSlabs * 8), "cudaFuncSetAttribute")) return fail(CUBA_ERR_CUDA);
+    if (!cuda_ok(cudaFuncSetAttribute(k_observe_partial<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      kObsWarps * kLrfComp * kLrfMaxSlabs * 8), "cudaFuncSetAttribute")) return fail(CUBA_ERR_CUDA);
 
     cudaStream_t st = ctx->stream;
     auto body = [&]() -> int {
@@ -588,7 +592,7 @@ int cuba_observables(cuba_ctx *ctx, double total[4], int nslab, double *edens)
     const double inv_w = (double)nslab / ctx->box[0];
     const double vol = ((ctx->n_test * (ctx->box[0] / (double)nslab)) * ctx->box[1]) * ctx->box[2];
     double *partial = ctx->at<double>(lay.obs_partial), *result = ctx->at<double>(lay.obs_result);
-    k_observe_partial<<<kObsGrid, kObsThreads, (size_t)kObsWarps * nslab * 8, st>>>(ctx->n, cur.x, cur.px, cur.py, cur.pz,
+    k_observe_partial<false><<<kObsGrid, kObsThreads, (size_t)kObsWarps * nslab * 8, st>>>(ctx->n, cur.x, cur.px, cur.py, cur.pz,
                                                                                   inv_w, nslab, partial);
     LAUNCHED();
     k_observe_final<<<(4 + nslab + 7) / 8, 256, 0, st>>>(kObsGrid, nslab, partial, vol, result);
@@ -598,6 +602,31 @@ int cuba_observables(cuba_ctx *ctx, double total[4], int nslab, double *edens)
     if (rc != CUBA_OK) return rc;
     memcpy(total, ctx->h_obs, 4 * sizeof(double));
     memcpy(edens, ctx->h_obs + 4, (size_t)nslab * sizeof(double));
+    return CUBA_OK;
+}
+
+int cuba_observables_lrf(cuba_ctx *ctx, int nslab, double *T, double *lrf)
+{
+    if (!ctx || !T || !lrf) return CUBA_ERR_NULL;
+    if (nslab < 1 || nslab > kLrfMaxSlabs) return CUBA_ERR_SIZE;
+    const Layout &lay = ctx->lay;
+    const Soa &cur = ctx->set[ctx->cur];
+    cudaStream_t st = ctx->stream;
+    const double inv_w = (double)nslab / ctx->box[0];
+    const double vol = ((ctx->n_test * (ctx->box[0] / (double)nslab)) * ctx->box[1]) * ctx->box[2];
+    double *partial = ctx->at<double>(lay.obs_partial), *result = ctx->at<double>(lay.obs_result);
+    const int grid = 148 * 3;           // 3 CTAs per SM (2 when nslab needs more than 75 KB of shared memory each)
+    static_assert(148 * 3 <= kObsGrid, "partial buffer is sized for kObsGrid blocks");
+    k_observe_partial<true><<<grid, kObsThreads, (size_t)kObsWarps * kLrfComp * nslab * 8, st>>>(ctx->n, cur.x, cur.px, cur.py, cur.pz,
+                                                                                              inv_w, nslab, partial);
+    LAUNCHED();
+    k_observe_lrf_final<<<(nslab + 7) / 8, 256, 0, st>>>(grid, nslab, partial, vol, result);
+    LAUNCHED();
+    CU(cudaMemcpyAsync(ctx->h_obs, result, (size_t)9 * nslab * 8, cudaMemcpyDeviceToHost, st));
+    int rc = sync_and_check(ctx);
+    if (rc != CUBA_OK) return rc;
+    memcpy(T, ctx->h_obs, (size_t)kLrfComp * nslab * sizeof(double));
+    memcpy(lrf, ctx->h_obs + (size_t)kLrfComp * nslab, (size_t)4 * nslab * sizeof(double));
     return CUBA_OK;
 }
 

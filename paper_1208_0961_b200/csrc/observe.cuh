@@ -12,22 +12,65 @@ constexpr int kObsWarps = kObsThreads / 32;
 constexpr int kObsItems = 4;                    // particles per thread per tile: 16 independent loads in flight
 constexpr int kObsTile = kObsThreads * kObsItems;
 constexpr int kObsMaxSlabs = 1024;
+constexpr int kLrfComp = 5;                     // T00, T0x, Txx, Tyy, Tzz
+constexpr int kLrfMaxSlabs = 256;               // kObsWarps * 5 * 256 doubles = 80 KB of shared memory
 
-// partial layout per block: [0..3] totals, [4 .. 4+nslab) slab energies
-__global__ void __launch_bounds__(kObsThreads, 4)
+// Every thread keeps a running sum for the slab of the particles it has seen last.  The store is
+// cell-sorted with x slowest and a CTA walks a contiguous range of tiles, so that slab changes a
+// handful of times per kernel; when it changes for any lane the whole warp reduces its running
+// sums (slab by slab, shuffle tree) into the warp's shared-memory bins and starts afresh.  When
+// and what is flushed depends on the data only, never on scheduling: the result is
+// bit-reproducible from run to run.
+template <int NC>
+__device__ __forceinline__ void warp_flush(double (&acc)[NC], int &slab, double *bins, int nslab, int lane)
+{
+    uint32_t todo = __ballot_sync(0xFFFFFFFFu, slab >= 0);
+    while (todo) {
+        const int leader = __ffs(todo) - 1;
+        const int s0 = __shfl_sync(0xFFFFFFFFu, slab, leader);
+        const bool mine = slab == s0;
+#pragma unroll
+        for (int q = 0; q < NC; ++q) {
+            double r = mine ? acc[q] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) r += __shfl_xor_sync(0xFFFFFFFFu, r, o);
+            if (lane == 0) bins[q * nslab + s0] += r;
+        }
+        todo &= ~__ballot_sync(0xFFFFFFFFu, mine);
+    }
+    slab = -1;
+#pragma unroll
+    for (int q = 0; q < NC; ++q) acc[q] = 0.0;
+}
+
+// LRF = false: energy density per slab (NC = 1) + totals (sum E, sum p); partial layout per
+//       block: [0..3] totals, [4 .. 4+nslab) slab energies.
+// LRF = true:  T00, T0x, Txx, Tyy, Tzz per slab (A22): per particle
+//       w = 1/E and the contributions E, px, (px*px)*w, (py*py)*w, (pz*pz)*w; partial layout
+//       per block: [comp][nslab].
+// One HBM pass over x, px, py, pz (32 B per particle).
+template <bool LRF>
+__global__ void __launch_bounds__(kObsThreads, LRF ? 3 : 4)
 k_observe_partial(int64_t n, const double *__restrict__ x, const double *__restrict__ px,
                   const double *__restrict__ py, const double *__restrict__ pz, double inv_w,
                   int nslab, double *__restrict__ partial)
 {
-    extern __shared__ double s_bins[];          // [kObsWarps][nslab]
+    constexpr int NC = LRF ? kLrfComp : 1;
+    extern __shared__ double s_bins[];          // [kObsWarps][NC][nslab]
     __shared__ double s_tot[kObsWarps][4];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    double *bins = s_bins + (size_t)wid * nslab;
-    for (int s = lane; s < nslab; s += 32) bins[s] = 0.0;
+    double *bins = s_bins + (size_t)wid * NC * nslab;
+    for (int s = lane; s < NC * nslab; s += 32) bins[s] = 0.0;
     __syncwarp();
     double tE = 0.0, tx = 0.0, ty = 0.0, tz = 0.0;
+    double acc[NC];
+#pragma unroll
+    for (int q = 0; q < NC; ++q) acc[q] = 0.0;
+    int cur = -1;
     const int64_t ntiles = (n + kObsTile - 1) / kObsTile;
-    for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const int64_t per = (ntiles + gridDim.x - 1) / gridDim.x;     // contiguous range of tiles per CTA
+    const int64_t t0 = blockIdx.x * per, t1 = min(ntiles, t0 + per);
+    for (int64_t tile = t0; tile < t1; ++tile) {
         double a[kObsItems], b[kObsItems], c[kObsItems], xx[kObsItems];
 #pragma unroll
         for (int k = 0; k < kObsItems; ++k) {
@@ -37,42 +80,47 @@ k_observe_partial(int64_t n, const double *__restrict__ x, const double *__restr
 #pragma unroll
         for (int k = 0; k < kObsItems; ++k) {
             const bool valid = tile * kObsTile + k * kObsThreads + tid < n;
-            const double E = valid ? energy(a[k], b[k], c[k]) : 0.0;
-            if (valid) { tE += E; tx += a[k]; ty += b[k]; tz += c[k]; }
-            const int slab = valid ? min(max(__double2int_rz(xx[k] * inv_w), 0), nslab - 1) : -1;
-            // the store is sorted with x slowest, so a warp sees one or two slabs: peel them off
-            uint32_t todo = __ballot_sync(0xFFFFFFFFu, valid);
-            while (todo) {
-                const int leader = __ffs(todo) - 1;
-                const int s0 = __shfl_sync(0xFFFFFFFFu, slab, leader);
-                const bool mine = valid && slab == s0;
-                double v = mine ? E : 0.0;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
-                if (lane == 0) bins[s0] += v;
-                todo &= ~__ballot_sync(0xFFFFFFFFu, mine);
+            const int slab = valid ? min(max(__double2int_rz(xx[k] * inv_w), 0), nslab - 1) : cur;
+            if (__any_sync(0xFFFFFFFFu, cur >= 0 && slab != cur)) warp_flush<NC>(acc, cur, bins, nslab, lane);
+            if (valid) {
+                const double E = energy(a[k], b[k], c[k]);
+                cur = slab;
+                acc[0] += E;
+                if (LRF) {
+                    const double w = 1.0 / E;
+                    acc[1 % NC] += a[k];
+                    acc[2 % NC] += (a[k] * a[k]) * w;
+                    acc[3 % NC] += (b[k] * b[k]) * w;
+                    acc[4 % NC] += (c[k] * c[k]) * w;
+                } else {
+                    tE += E; tx += a[k]; ty += b[k]; tz += c[k];
+                }
             }
         }
     }
+    warp_flush<NC>(acc, cur, bins, nslab, lane);
+    if (!LRF) {
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        tE += __shfl_xor_sync(0xFFFFFFFFu, tE, o);
-        tx += __shfl_xor_sync(0xFFFFFFFFu, tx, o);
-        ty += __shfl_xor_sync(0xFFFFFFFFu, ty, o);
-        tz += __shfl_xor_sync(0xFFFFFFFFu, tz, o);
+        for (int o = 16; o > 0; o >>= 1) {
+            tE += __shfl_xor_sync(0xFFFFFFFFu, tE, o);
+            tx += __shfl_xor_sync(0xFFFFFFFFu, tx, o);
+            ty += __shfl_xor_sync(0xFFFFFFFFu, ty, o);
+            tz += __shfl_xor_sync(0xFFFFFFFFu, tz, o);
+        }
+        if (lane == 0) { s_tot[wid][0] = tE; s_tot[wid][1] = tx; s_tot[wid][2] = ty; s_tot[wid][3] = tz; }
     }
-    if (lane == 0) { s_tot[wid][0] = tE; s_tot[wid][1] = tx; s_tot[wid][2] = ty; s_tot[wid][3] = tz; }
     __syncthreads();
-    double *out = partial + (size_t)blockIdx.x * (4 + nslab);
-    if (tid < 4) {
+    const int head = LRF ? 0 : 4;
+    double *out = partial + (size_t)blockIdx.x * (head + NC * nslab);
+    if (!LRF && tid < 4) {
         double s = 0.0;
         for (int w = 0; w < kObsWarps; ++w) s += s_tot[w][tid];
         out[tid] = s;
     }
-    for (int s = tid; s < nslab; s += kObsThreads) {
+    for (int s = tid; s < NC * nslab; s += kObsThreads) {
         double v = 0.0;
-        for (int w = 0; w < kObsWarps; ++w) v += s_bins[(size_t)w * nslab + s];
-        out[4 + s] = v;
+        for (int w = 0; w < kObsWarps; ++w) v += s_bins[(size_t)w * NC * nslab + s];
+        out[head + s] = v;
     }
 }
 
@@ -90,6 +138,39 @@ k_observe_final(int nblocks, int nslab, const double *__restrict__ partial, doub
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
     if (lane == 0) result[e] = (e < 4) ? s : s / vol;
+}
+
+// result: T[5][nslab] then lrf[4][nslab] = e, v, P_L, P_T (Landau matching for a flow along x).
+// One warp per slab; lanes sum the block partials in a fixed order.
+__global__ void __launch_bounds__(256)
+k_observe_lrf_final(int nblocks, int nslab, const double *__restrict__ partial, double vol,
+                    double *__restrict__ result)
+{
+    const int j = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (j >= nslab) return;
+    double T[kLrfComp];
+#pragma unroll
+    for (int q = 0; q < kLrfComp; ++q) {
+        double s = 0.0;
+        for (int b = lane; b < nblocks; b += 32) s += partial[((size_t)b * kLrfComp + q) * nslab + j];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xFFFFFFFFu, s, o);
+        T[q] = s / vol;
+    }
+    if (lane == 0) {
+#pragma unroll
+        for (int q = 0; q < kLrfComp; ++q) result[q * nslab + j] = T[q];
+        const double tr = T[0] + T[2];
+        double disc = tr * tr - 4.0 * (T[1] * T[1]);
+        if (!(disc > 0.0)) disc = 0.0;
+        const double e = 0.5 * ((T[0] - T[2]) + sqrt(disc));
+        const double den = e + T[2];
+        double *lrf = result + (size_t)kLrfComp * nslab;
+        lrf[0 * nslab + j] = e;
+        lrf[1 * nslab + j] = (den > 0.0) ? T[1] / den : 0.0;
+        lrf[2 * nslab + j] = (e - T[0]) + T[2];
+        lrf[3 * nslab + j] = 0.5 * (T[3] + T[4]);
+    }
 }
 
 }  // namespace cuba

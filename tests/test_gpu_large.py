@@ -70,8 +70,15 @@ def test_full_size_step_sampled_against_oracle(cuba, oracle_mod, config):
     expect = float((counts * (counts - 1) / 2.0).sum() * base)
     assert c1.collisions == 0 and c2.collisions == pytest.approx(expect, rel=0.01)
     # energy conservation over the two steps
-    tot1, _ = g.observables(64)
+    tot1, ed1 = g.observables(64)
     assert abs(tot1[0] - tot0[0]) / tot0[0] < 1e-10
+    # local-rest-frame observables at full size: properties that hold at any size
+    T, lrf = g.observables_lrf(64)
+    assert np.allclose(T[0], ed1, rtol=1e-12)                                   # T00 is the energy density
+    assert np.allclose(T[0], T[2] + T[3] + T[4], rtol=1e-12)                    # massless: traceless tensor
+    assert float(T[0].sum()) * (w.n_test * np.prod(w.box) / 64) == pytest.approx(tot1[0], rel=1e-12)
+    assert np.all(lrf[0] <= T[0] * (1 + 1e-12)) and np.all(np.abs(lrf[1]) < 1.0)
+    assert np.allclose(lrf[0], lrf[2] + 2.0 * lrf[3], rtol=1e-9)                # e = P_L + 2 P_T
     # sampled cells: the oracle collides the same particles (same pids, same seed, same t)
     # when fed the post-binning momenta; positions there are irrelevant to S5
     rng = np.random.default_rng(5)

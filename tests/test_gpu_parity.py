@@ -125,6 +125,46 @@ def test_riemann_profiles_over_many_steps(cuba, oracle_mod):
     assert_state_equal(g.particles(), o.particles())
 
 
+def assert_lrf_equal(got, ref):
+    """Tensor sums differ from the oracle's only by summation order (1e-12, DESIGN.md section 3);
+    the Landau-matched quantities go through a square root of a difference: 1e-10."""
+    (gT, gl), (oT, ol) = got, ref
+    scale = np.maximum(oT[0], 1e-300)                   # T00 of the slab sets the scale of every component
+    assert np.all(np.abs(gT - oT) <= REL * scale), "tensor components"
+    assert np.all(np.abs(gl[0] - ol[0]) <= 1e-10 * scale), "e"
+    assert np.all(np.abs(gl[1] - ol[1]) <= 1e-10), "v"
+    assert np.all(np.abs(gl[2:] - ol[2:]) <= 1e-10 * scale), "P_L, P_T"
+
+
+def test_lrf_observables_match_oracle(cuba, oracle_mod):
+    """T00, T0x, Txx, Tyy, Tzz per slab and the Landau matching, on an evolving
+    Riemann problem (a flow develops at the discontinuity), for several slab counts incl. the
+    limits, slabs that cut through cell layers, and empty slabs."""
+    w = workloads.riemann(L=(16.0, 4.0, 4.0), ncell=(16, 4, 4), r_test=10.0, seed=15)
+    g = cuba.Cuba.from_workload(w)
+    o = oracle_mod.Oracle.from_workload(w)
+    for nslab in (1, 16, 37, 256):
+        assert_lrf_equal(g.observables_lrf(nslab), o.observables_lrf(nslab))
+    g.step(25, w.dt, w.sigma)
+    o.step(25, w.dt, w.sigma)
+    for nslab in (1, 16, 37, 256):
+        assert_lrf_equal(g.observables_lrf(nslab), o.observables_lrf(nslab))
+    T, lrf = g.observables_lrf(16)
+    assert np.array_equal(np.isfinite(lrf), np.ones_like(lrf, dtype=bool))
+    assert lrf[1].max() > 0.05                          # matter flows from the hot to the cold side
+    assert np.allclose(T[0], g.observables(16)[1], rtol=REL)       # T00 is the energy density of Fig. 2
+    # empty slabs: particles only in x < 4 of a 16 fm box
+    w2 = workloads.thermal_box(L=(16.0, 2.0, 2.0), ncell=(16, 2, 2), count=5000, seed=8, r_test=3.0)
+    w2.x[:] = 4.0 * np.random.default_rng(2).random(w2.n)
+    g2, o2 = cuba.Cuba.from_workload(w2), oracle_mod.Oracle.from_workload(w2)
+    T2, l2 = g2.observables_lrf(8)
+    assert_lrf_equal((T2, l2), o2.observables_lrf(8))
+    assert np.all(T2[:, 2:] == 0.0) and np.all(l2[:, 2:] == 0.0)
+    for bad in (0, 257):
+        with pytest.raises(cuba.CubaError):
+            g.observables_lrf(bad)
+
+
 def test_k_steps_equal_k_single_steps_and_determinism(cuba):
     w = workloads.riemann_small()
     a, b, c = (cuba.Cuba.from_workload(w) for _ in range(3))
