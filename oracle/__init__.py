@@ -67,6 +67,8 @@ def lib():
         L.oracle_step.argtypes = [c_void_p, c_int, c_double, c_double]
         L.oracle_step.restype = c_int
         L.oracle_observables.argtypes = [c_void_p, dp, c_int, dp]
+        L.oracle_step_adaptive.argtypes = [c_void_p, c_int, c_double, c_double, dp, dp]
+        L.oracle_step_adaptive.restype = c_int
         L.oracle_observables_lrf.argtypes = [c_void_p, c_int, dp, dp]
         L.oracle_landau_match.argtypes = [c_double] * 5 + [dp]
         L.oracle_get_particles.argtypes = [c_void_p, u32p] + [dp] * 6
@@ -217,6 +219,15 @@ class Oracle:
         rc = lib().oracle_step(self._h, int(nsteps), float(dt), float(sigma))
         if rc != 0:
             raise OracleError(rc)
+
+    def step_adaptive(self, nsteps, dt_max, sigma):
+        """Variable dt (reading A23): returns (dt_used[nsteps], elapsed)."""
+        used = np.zeros(int(nsteps))
+        el = np.zeros(1)
+        rc = lib().oracle_step_adaptive(self._h, int(nsteps), float(dt_max), float(sigma), _dp(used), _dp(el))
+        if rc != 0:
+            raise OracleError(rc)
+        return used, float(el[0])
 
     def observables(self, nslab):
         tot = np.zeros(4)
