@@ -112,6 +112,18 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
  * surface at the next synchronising call. */
 int cuba_step(cuba_ctx *ctx, int nsteps, double dt, double sigma);
 
+/* Variable time step ("implement the parameter dt as variable"; DESIGN.md reading
+ * A23).  Before each of the nsteps steps, with n_max the population of the fullest cell of the
+ * current store and cn = n_max (odd) or n_max - 1 (even),
+ *     dt = min(dt_max, (1 - 2^-10) / ((2 cn) * sigma / (n_test * V_cell)))
+ * (dt_max if sigma = 0 or no cell holds two particles): the scaled Eq. 3 probability stays below
+ * 1 in that cell without extra rounds; cells that outgrow it in the step's own binning still get
+ * extra rounds.  Then the step runs exactly as cuba_step(ctx, 1, dt, sigma).  dt_used (HOST,
+ * nsteps doubles, may be NULL) receives the steps taken, *elapsed (HOST, may be NULL) their sum
+ * in step order.  Synchronises once per step (a 4-byte read-back of n_max).  Errors as
+ * cuba_step; the CFL check applies to every dt actually taken. */
+int cuba_step_adaptive(cuba_ctx *ctx, int nsteps, double dt_max, double sigma, double *dt_used, double *elapsed);
+
 /* Execution options (results are bit-identical for every setting; they only change how the
  * step is scheduled on the device).  CUBA_OPT_FUSE_HIST (default 1): the collision kernel of
  * step t also performs S1-S3 of step t+1 on the momenta it holds on chip and writes the

@@ -14,7 +14,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 EXPORTS = ("cuba_workspace_bytes", "cuba_init", "cuba_step", "cuba_observables", "cuba_state",
            "cuba_get_particles", "cuba_get_cells", "cuba_step_traced", "cuba_counters", "cuba_run_host", "cuba_destroy",
            "cuba_strerror", "cuba_last_cuda_error", "cuba_launch_count", "cuba_profile_enable",
-           "cuba_profile_read", "cuba_profile_name", "cuba_set_option", "cuba_observables_lrf")
+           "cuba_profile_read", "cuba_profile_name", "cuba_set_option", "cuba_observables_lrf",
+           "cuba_step_adaptive")
 
 
 class CubaError(RuntimeError):
@@ -105,6 +106,7 @@ def lib():
         L.cuba_profile_enable.argtypes = [c_void_p, c_int]
         L.cuba_set_option.argtypes = [c_void_p, c_int, c_int]
         L.cuba_observables_lrf.argtypes = [c_void_p, c_int, dp, dp]
+        L.cuba_step_adaptive.argtypes = [c_void_p, c_int, c_double, c_double, dp, dp]
         L.cuba_profile_read.argtypes = [c_void_p, dp, POINTER(c_uint64)]
         L.cuba_profile_name.argtypes = [c_int]
         L.cuba_profile_name.restype = c_char_p
@@ -235,6 +237,14 @@ class Cuba:
         _check(lib().cuba_step_traced(self._h, float(dt), float(sigma), ctypes.byref(tr)))
         m = int(tr.n_pairs)
         return Trace(cell_of_pid, cell[:m], rnd[:m], pa[:m], pb[:m], P[:m], u[:m], dec[:m])
+
+    def step_adaptive(self, nsteps, dt_max, sigma):
+        """cuba_step_adaptive: returns (dt_used[nsteps], elapsed)."""
+        used = np.zeros(int(nsteps))
+        el = (c_double * 1)()
+        _check(lib().cuba_step_adaptive(self._h, int(nsteps), float(dt_max), float(sigma),
+                                        used.ctypes.data_as(POINTER(c_double)), el))
+        return used, float(el[0])
 
     def observables_lrf(self, nslab):
         """cuba_observables_lrf: (T[5, nslab] = T00, T0x, Txx, Tyy, Tzz; lrf[4, nslab] = e, v, P_L, P_T)."""

@@ -265,7 +265,7 @@ __global__ void __launch_bounds__(256)
 k_cell_start(uint32_t ncells, const uint32_t *__restrict__ count_new,
              const uint32_t *__restrict__ block_prefix, uint32_t *__restrict__ cell_start,
              ClassTable ct, uint32_t *__restrict__ class_count, uint4 *__restrict__ class_list,
-             unsigned long long *__restrict__ max_occ)
+             unsigned long long *__restrict__ max_occ, uint32_t *__restrict__ step_max)
 {
     __shared__ uint32_t s_warp[8];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -304,7 +304,10 @@ k_cell_start(uint32_t ncells, const uint32_t *__restrict__ count_new,
     uint32_t vmax = v;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) vmax = max(vmax, __shfl_xor_sync(0xFFFFFFFFu, vmax, o));
-    if (lane == 0 && vmax > 0) atomicMax(max_occ, (unsigned long long)vmax);
+    if (lane == 0 && vmax > 0) {
+        atomicMax(max_occ, (unsigned long long)vmax);   // since cuba_init (cuba_counters)
+        atomicMax(step_max, vmax);                      // of this binning (cleared per step; feeds the variable time step)
+    }
 }
 
 // ---- K_D: dest_base[d][c_old] = cell_start[c_new(c_old, d)] + off[d][c_old], in place ------

@@ -2,6 +2,7 @@
 // stream-ordered kernel launches.  No CPU fallback: every entry point needs a CUDA device.
 #include "../../include/cuba.h"
 
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdio>
@@ -63,7 +64,8 @@ struct Layout {
 };
 
 constexpr int kObsGrid = 148 * 4;   // resident CTAs: 4 per SM at 64 registers
-constexpr int kZeroWords = 32;   // class_count[8], work[8], arena cursor (u64 = 2 words), pad
+constexpr int kZeroWords = 32;   // class_count[8], work[8], arena cursor (u64 = 2 words), [20] fullest cell of this binning, pad
+constexpr int kStepMaxWord = 20;
 
 Layout make_layout(int64_t n, int64_t ncells)
 {
@@ -118,6 +120,9 @@ struct cuba_ctx {
     double *h_obs;       // pinned staging for observables
     cudaStream_t cls_stream[kNumClasses] = {};   // the collision classes run concurrently, fenced into `stream`
     cudaEvent_t ev_fork = nullptr, ev_join[kNumClasses] = {};
+    uint32_t nmax_cur = 0;   // population of the fullest cell of the current store (variable time step, A23)
+    bool nmax_valid = false; // false after steps that did not read it back
+    uint32_t *h_u32 = nullptr;   // pinned word for that read-back
     bool fuse_hist = true;   // CUBA_OPT_FUSE_HIST
     double pre_dt = 0.0;     // > 0: cnt / carry already hold the histogram of the next step for this dt
     int prof_mode = 0;   // 0 off, 1 events per kernel (collision classes as one concurrent group), 2 classes serialised
@@ -252,6 +257,7 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
     ctx->h_obs = nullptr;
     auto fail = [&](int code) {
         if (ctx->h_obs) cudaFreeHost(ctx->h_obs);
+        if (ctx->h_u32) cudaFreeHost(ctx->h_u32);
         if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
         for (int k = 0; k < kNumClasses; ++k) {
             if (ctx->cls_stream[k]) cudaStreamDestroy(ctx->cls_stream[k]);
@@ -261,6 +267,7 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
         return code;
     };
     if (!cuda_ok(cudaMallocHost(&ctx->h_obs, (9 * kLrfMaxSlabs > 4 + kObsMaxSlabs ? 9 * kLrfMaxSlabs : 4 + kObsMaxSlabs) * sizeof(double)), "cudaMallocHost")) return fail(CUBA_ERR_CUDA);
+    if (!cuda_ok(cudaMallocHost(&ctx->h_u32, 64), "cudaMallocHost")) return fail(CUBA_ERR_CUDA);
     if (!cuda_ok(cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming), "cudaEventCreate")) return fail(CUBA_ERR_CUDA);
     for (int k = 0; k < kNumClasses; ++k) {
         if (!cuda_ok(cudaStreamCreateWithFlags(&ctx->cls_stream[k], cudaStreamNonBlocking), "cudaStreamCreate")) return fail(CUBA_ERR_CUDA);
@@ -319,7 +326,15 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
         double *to[6] = {x, y, z, px, py, pz};
         for (int k = 0; k < 6; ++k) CU(cudaMemcpyAsync(to[k], from[k], (size_t)n * 8, cudaMemcpyDeviceToDevice, st));
         CU(cudaMemcpyAsync(ctx->set[0].pid, ctx->set[1].pid, (size_t)n * 4, cudaMemcpyDeviceToDevice, st));
-        return sync_and_check(ctx);
+        int r = sync_and_check(ctx);
+        if (r != CUBA_OK) return r;
+        // fullest cell of the initial binning (start of a variable-dt run); init is synchronous anyway
+        std::vector<uint32_t> start((size_t)ncells + 1);
+        CU(cudaMemcpy(start.data(), ctx->at<uint32_t>(lay.cell_start), ((size_t)ncells + 1) * 4, cudaMemcpyDeviceToHost));
+        uint32_t m = 0;
+        for (int64_t c = 0; c < ncells; ++c) m = std::max(m, start[c + 1] - start[c]);
+        ctx->nmax_cur = m; ctx->nmax_valid = true;
+        return CUBA_OK;
     };
     rc = body();
     if (rc != CUBA_OK) return fail(rc);
@@ -332,6 +347,7 @@ void cuba_destroy(cuba_ctx *ctx)
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
     if (ctx->h_obs) cudaFreeHost(ctx->h_obs);
+    if (ctx->h_u32) cudaFreeHost(ctx->h_u32);
     for (int k = 0; k < kNumClasses; ++k) {
         if (ctx->cls_stream[k]) { cudaStreamSynchronize(ctx->cls_stream[k]); cudaStreamDestroy(ctx->cls_stream[k]); }
         if (ctx->ev_join[k]) cudaEventDestroy(ctx->ev_join[k]);
@@ -461,7 +477,7 @@ static int enqueue_bin(cuba_ctx *ctx, double dt, uint32_t *cell_of_pid)
     k_cell_start<<<(unsigned)lay.nblocks_cells, 256, 0, st>>>(ncells, ctx->at<uint32_t>(lay.count_new),
                                                               ctx->at<uint32_t>(lay.block_sum), ctx->at<uint32_t>(lay.cell_start),
                                                               ct, zero, ctx->at<uint4>(lay.class_list),
-                                                              ctx->at<unsigned long long>(lay.max_occ));
+                                                              ctx->at<unsigned long long>(lay.max_occ), zero + kStepMaxWord);
     LAUNCHED();
     prof_mark(ctx, G_CELL_START);
     if (!have_hist) {
@@ -501,7 +517,66 @@ int cuba_step(cuba_ctx *ctx, int nsteps, double dt, double sigma)
         ctx->pre_dt = next_dt;
         ctx->t += 1;
         ctx->steps += 1;
+        ctx->nmax_valid = false;
     }
+    return CUBA_OK;
+}
+
+// Variable time step, reading A23: the same fp64 expression, in the same order, as the oracle's.
+static double adaptive_dt(const cuba_ctx *ctx, uint32_t nmax, double dt_max, double sigma)
+{
+    if (nmax < 2u || !(sigma > 0.0)) return dt_max;
+    const double dx = ctx->box[0] / (double)ctx->g.nc[0];
+    const double dy = ctx->box[1] / (double)ctx->g.nc[1];
+    const double dz = ctx->box[2] / (double)ctx->g.nc[2];
+    const double V = (dx * dy) * dz;
+    const double cn = (nmax & 1u) ? (double)nmax : (double)(nmax - 1u);
+    const double g = sigma / (ctx->n_test * V);
+    const double lim = 0.9990234375 / ((2.0 * cn) * g);   // 1 - 2^-10
+    return lim < dt_max ? lim : dt_max;
+}
+
+static int read_step_max(cuba_ctx *ctx)
+{
+    CU(cudaMemcpyAsync(ctx->h_u32, ctx->at<uint32_t>(ctx->lay.zero) + kStepMaxWord, 4, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->nmax_cur = *ctx->h_u32;
+    ctx->nmax_valid = true;
+    return CUBA_OK;
+}
+
+int cuba_step_adaptive(cuba_ctx *ctx, int nsteps, double dt_max, double sigma, double *dt_used, double *elapsed)
+{
+    if (!ctx) return CUBA_ERR_NULL;
+    if (nsteps < 0) return CUBA_ERR_SIZE;
+    if (!(dt_max > 0.0) || !std::isfinite(dt_max) || !(sigma >= 0.0) || !std::isfinite(sigma)) return CUBA_ERR_VALUE;
+    double sum = 0.0;
+    int rc = CUBA_OK;
+    if (nsteps > 0 && !ctx->nmax_valid) {      // the last binning's value is still on the device
+        rc = read_step_max(ctx);
+        if (rc != CUBA_OK) return rc;
+    }
+    for (int s = 0; s < nsteps; ++s) {
+        const double dt = adaptive_dt(ctx, ctx->nmax_cur, dt_max, sigma);
+        double base;
+        rc = check_step_args(ctx, dt, sigma, &base);
+        if (rc != CUBA_OK) return rc;
+        rc = enqueue_bin(ctx, dt, nullptr);
+        if (rc != CUBA_OK) return rc;
+        // the fullest cell of the new binning fixes the NEXT step, whose histogram this step's
+        // collision kernel prepares: one 4-byte read-back per step between scatter and collide
+        rc = read_step_max(ctx);
+        if (rc != CUBA_OK) return rc;
+        const double next_dt = ctx->fuse_hist ? adaptive_dt(ctx, ctx->nmax_cur, dt_max, sigma) : 0.0;
+        rc = launch_collide<false>(ctx, base, nullptr, next_dt);
+        if (rc != CUBA_OK) return rc;
+        ctx->pre_dt = next_dt;
+        ctx->t += 1;
+        ctx->steps += 1;
+        if (dt_used) dt_used[s] = dt;
+        sum = sum + dt;
+    }
+    if (elapsed) *elapsed = sum;
     return CUBA_OK;
 }
 
@@ -555,6 +630,7 @@ int cuba_step_traced(cuba_ctx *ctx, double dt, double sigma, cuba_trace *out)
         if (r != CUBA_OK) return r;
         ctx->t += 1;
         ctx->steps += 1;
+        ctx->nmax_valid = false;
         r = sync_and_check(ctx);
         if (r != CUBA_OK) return r;
         if (run) {

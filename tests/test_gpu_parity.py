@@ -165,6 +165,41 @@ def test_lrf_observables_match_oracle(cuba, oracle_mod):
             g.observables_lrf(bad)
 
 
+def test_adaptive_time_step_matches_oracle(cuba, oracle_mod):
+    """the dt sequence (a function of the integer occupancy of the fullest
+    cell), the elapsed time and the state are the oracle's bit for bit -- where the rule binds
+    (dense box: dt far below dt_max), where it does not (riemann_small), with fixed steps in
+    between (the device-side occupancy must be fetched), with and without the fused histogram."""
+    dense = workloads.thermal_box(L=(3.0, 3.0, 3.0), ncell=(3, 3, 3), count=6000, seed=5, r_test=1.2,
+                                  sigma_gev2=10.0, dt=0.1)
+    loose = workloads.riemann_small()
+    loose.sigma *= 0.1                                  # the limit is ~0.75 fm/c: dt_max = 0.1 always wins
+    for w, binds in ((dense, True), (workloads.riemann_small(), True), (loose, False)):
+        for fuse in (1, 0):
+            g = cuba.Cuba.from_workload(w)
+            g.set_option(1, fuse)
+            o = oracle_mod.Oracle.from_workload(w)
+            ug, eg = g.step_adaptive(5, w.dt, w.sigma)
+            uo, eo = o.step_adaptive(5, w.dt, w.sigma)
+            assert np.array_equal(ug, uo) and eg == eo
+            assert bool(np.all(ug < w.dt)) == binds and bool(np.all(ug == w.dt)) == (not binds)
+            assert_state_equal(g.particles(), o.particles())
+            g.step(2, 0.5 * ug[-1], w.sigma)            # fixed steps: no occupancy read-back
+            o.step(2, 0.5 * uo[-1], w.sigma)
+            ug, eg = g.step_adaptive(3, w.dt, w.sigma)
+            uo, eo = o.step_adaptive(3, w.dt, w.sigma)
+            assert np.array_equal(ug, uo) and eg == eo
+            assert_state_equal(g.particles(), o.particles())
+            gc, oc = g.counters(), o.counters()
+            assert (gc.steps, gc.pairs, gc.collisions, gc.rounds) == (10, oc["pairs"], oc["collisions"], oc["rounds"])
+            assert gc.device_flags == 0
+    g = cuba.Cuba.from_workload(dense)
+    with pytest.raises(cuba.CubaError):
+        g.step_adaptive(1, -0.1, dense.sigma)
+    with pytest.raises(cuba.CubaError):
+        g.step_adaptive(1, 5.0, 0.0)                    # sigma = 0: dt = dt_max beyond the cell edge (PAPER.md:62)
+
+
 def test_k_steps_equal_k_single_steps_and_determinism(cuba):
     w = workloads.riemann_small()
     a, b, c = (cuba.Cuba.from_workload(w) for _ in range(3))
