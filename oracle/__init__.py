@@ -67,6 +67,10 @@ def lib():
         L.oracle_step.argtypes = [c_void_p, c_int, c_double, c_double]
         L.oracle_step.restype = c_int
         L.oracle_observables.argtypes = [c_void_p, dp, c_int, dp]
+        L.oracle_step_etas.argtypes = [c_void_p, c_int, c_double, c_double]
+        L.oracle_step_etas.restype = c_int
+        L.oracle_local_base.argtypes = [c_int64, dp, dp, dp, c_double, c_double]
+        L.oracle_local_base.restype = c_double
         L.oracle_step_adaptive.argtypes = [c_void_p, c_int, c_double, c_double, dp, dp]
         L.oracle_step_adaptive.restype = c_int
         L.oracle_observables_lrf.argtypes = [c_void_p, c_int, dp, dp]
@@ -165,6 +169,12 @@ def scatter(pa, pb, Ea, Eb, s, nhat):
     return qa, qb
 
 
+def local_base(px, py, pz, dt, etas):
+    """Eq. 3 without v_rel for one cell with the local cross section (A24)."""
+    px, py, pz = _f64(px), _f64(py), _f64(pz)
+    return float(lib().oracle_local_base(px.shape[0], _dp(px), _dp(py), _dp(pz), float(dt), float(etas)))
+
+
 def landau_match(T00, T0x, Txx, Tyy, Tzz):
     """(e, v, P_L, P_T) of one slab's tensor components."""
     o = np.zeros(4)
@@ -217,6 +227,12 @@ class Oracle:
 
     def step(self, nsteps, dt, sigma):
         rc = lib().oracle_step(self._h, int(nsteps), float(dt), float(sigma))
+        if rc != 0:
+            raise OracleError(rc)
+
+    def step_etas(self, nsteps, dt, etas):
+        """Local cross section for constant eta/s (reading A24)."""
+        rc = lib().oracle_step_etas(self._h, int(nsteps), float(dt), float(etas))
         if rc != 0:
             raise OracleError(rc)
 

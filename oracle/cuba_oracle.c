@@ -23,6 +23,7 @@
  *   66      total energy is conserved                                         -> observables
  *   62-72   energy density / flow of the Riemann problem, viscosity            -> LRF observables
  *   98      "implement the parameter dt as variable"                           -> oracle_step_adaptive
+ *   80,108  "local cross section" / constant eta/s of ref. [1]                 -> oracle_step_etas
  * Where the paper is silent (pair enumeration, shuffle, RNG, order inside a step, odd
  * cells, P > 1) the readings A1..A19 of DESIGN.md are followed; each is named at its use.
  *
@@ -35,7 +36,9 @@
  * Landau matching vs numpy's eigen-decomposition, hand-built slabs, tracelessness, and a
  * boosted thermal ensemble (e = 3 n T, v = beta); variable dt: reduces to the fixed step where
  * the rule does not bind, keeps every traced probability <= 1 without extra rounds, and leaves the
- * collision rate per unit time at the closed form.
+ * collision rate per unit time at the closed form; local cross section: traced probabilities
+ * against Eq. 3 assembled with math.fsum, collision rate per particle 0.3 T/(hbarc eta/s)
+ * independent of the density, independence of the array order.
  * Parity unpinned: the paper's Fig. 2-4 curves and the BAMPS overlay (images and BAMPS
  * are not available).
  */
@@ -454,8 +457,36 @@ static int collide_cell(oracle_state *st, uint32_t c, int64_t lo, int64_t hi, do
     return ORC_OK;
 }
 
-/* One step, reading A1 (Fig. 1 is missing): stream -> reflect -> bin -> pair -> collide. */
-static int step_once(oracle_state *st, double dt, double sigma)
+/* ------------------------------------------------------------------------------------
+ * Local ("per-cell") cross section for a constant shear viscosity to entropy density ratio
+ * (Fig. 3 caption "local cross section"; the constant-eta/s runs of ref. [1],
+ * PAPER.md:108; sigma_cell from the cell's n and <E>).  Reading A24
+ * (DESIGN.md): for an isotropic cross section and a massless Boltzmann gas eta = (6/5) T/sigma
+ * and s = 4 n, so eta/s fixes  sigma_cell = (3/10) T / (n (eta/s))  with, per cell,
+ * T = <E>/3 (in fm^-1: divided by hbar c = 0.197327 GeV fm) and n = n_cell/(r_test V_cell).
+ * Eq. 3 without v_rel then reads
+ *     base_cell = sigma_cell dt/(r_test V_cell) = ((0.1 S) dt) / (((hbarc (n n)) etas)),
+ * S = sum of the cell's energies at the start of S5.  So that S does not depend on the order of
+ * summation (R(n) and every P must be identical in any implementation), it is DEFINED as the
+ * exact fixed-point sum  S = (sum_i rint(E_i 2^40)) 2^-40  (64-bit integers; rint = to nearest,
+ * ties to even; E < 2^22 GeV).
+ * ---------------------------------------------------------------------------------- */
+#define ORC_HBARC 0.197327
+double oracle_local_base(int64_t n, const double *px, const double *py, const double *pz, double dt, double etas)
+{
+    int64_t acc = 0;
+    for (int64_t i = 0; i < n; ++i) acc += (int64_t)llrint(energy(px[i], py[i], pz[i]) * 1099511627776.0);
+    double S = (double)acc * (1.0 / 1099511627776.0);
+    double nn = (double)n * (double)n;
+    return ((0.1 * S) * dt) / ((ORC_HBARC * nn) * etas);
+}
+
+/* One step, reading A1 (Fig. 1 is missing): stream -> reflect -> bin -> pair -> collide.
+ * etas > 0 selects the local cross section (sigma is then ignored). */
+static int step_once_mode(oracle_state *st, double dt, double sigma, double etas);
+static int step_once(oracle_state *st, double dt, double sigma) { return step_once_mode(st, dt, sigma, 0.0); }
+
+static int step_once_mode(oracle_state *st, double dt, double sigma, double etas)
 {
     double dmin = st->box[0] / st->ncell[0];
     for (int k = 1; k < 3; ++k)
@@ -475,7 +506,9 @@ static int step_once(oracle_state *st, double dt, double sigma)
     for (int64_t c = 0; c < st->ncells; ++c) {
         int64_t lo = st->cell_start[c], hi = st->cell_start[c + 1];
         if ((uint32_t)(hi - lo) > st->max_occupancy) st->max_occupancy = (uint32_t)(hi - lo);
-        int r = collide_cell(st, (uint32_t)c, lo, hi, base);
+        double b = base;
+        if (etas > 0.0 && hi - lo >= 2) b = oracle_local_base(hi - lo, st->px + lo, st->py + lo, st->pz + lo, dt, etas);
+        int r = collide_cell(st, (uint32_t)c, lo, hi, b);
         if (r != ORC_OK) rc = r;
     }
     st->t += 1;
@@ -487,6 +520,16 @@ int oracle_step(oracle_state *st, int nsteps, double dt, double sigma)
 {
     for (int i = 0; i < nsteps; ++i) {
         int rc = step_once(st, dt, sigma);
+        if (rc != ORC_OK) return rc;
+    }
+    return ORC_OK;
+}
+
+int oracle_step_etas(oracle_state *st, int nsteps, double dt, double etas)
+{
+    if (!(etas > 0.0)) return ORC_ERR_ARG;
+    for (int i = 0; i < nsteps; ++i) {
+        int rc = step_once_mode(st, dt, 0.0, etas);
         if (rc != ORC_OK) return rc;
     }
     return ORC_OK;
