@@ -112,6 +112,16 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
  * surface at the next synchronising call. */
 int cuba_step(cuba_ctx *ctx, int nsteps, double dt, double sigma);
 
+/* Local ("per-cell") cross section for a constant shear viscosity to entropy density ratio
+ * ("local cross section", constant-eta/s runs of ref. [1] PAPER.md:108; DESIGN.md
+ * reading A24).  As cuba_step, but in every cell the total cross section of Eq. 3 is
+ *     sigma_cell = (3/10) T / (n * eta_over_s),  T = <E>/3 of the cell's particles (GeV / 0.197327
+ *     GeV fm), n = n_cell / (n_test * V_cell)
+ * (eta = (6/5) T/sigma and s = 4 n for an isotropic cross section and a massless Boltzmann gas);
+ * the cell's energy sum is the exact fixed-point sum (sum rint(E 2^40)) 2^-40, so the result does
+ * not depend on any summation order.  Errors as cuba_step; eta_over_s <= 0: CUBA_ERR_VALUE. */
+int cuba_step_local_sigma(cuba_ctx *ctx, int nsteps, double dt, double eta_over_s);
+
 /* Variable time step ("implement the parameter dt as variable"; DESIGN.md reading
  * A23).  Before each of the nsteps steps, with n_max the population of the fullest cell of the
  * current store and cn = n_max (odd) or n_max - 1 (even),

@@ -15,7 +15,7 @@ EXPORTS = ("cuba_workspace_bytes", "cuba_init", "cuba_step", "cuba_observables",
            "cuba_get_particles", "cuba_get_cells", "cuba_step_traced", "cuba_counters", "cuba_run_host", "cuba_destroy",
            "cuba_strerror", "cuba_last_cuda_error", "cuba_launch_count", "cuba_profile_enable",
            "cuba_profile_read", "cuba_profile_name", "cuba_set_option", "cuba_observables_lrf",
-           "cuba_step_adaptive")
+           "cuba_step_adaptive", "cuba_step_local_sigma")
 
 
 class CubaError(RuntimeError):
@@ -107,6 +107,7 @@ def lib():
         L.cuba_set_option.argtypes = [c_void_p, c_int, c_int]
         L.cuba_observables_lrf.argtypes = [c_void_p, c_int, dp, dp]
         L.cuba_step_adaptive.argtypes = [c_void_p, c_int, c_double, c_double, dp, dp]
+        L.cuba_step_local_sigma.argtypes = [c_void_p, c_int, c_double, c_double]
         L.cuba_profile_read.argtypes = [c_void_p, dp, POINTER(c_uint64)]
         L.cuba_profile_name.argtypes = [c_int]
         L.cuba_profile_name.restype = c_char_p
@@ -237,6 +238,10 @@ class Cuba:
         _check(lib().cuba_step_traced(self._h, float(dt), float(sigma), ctypes.byref(tr)))
         m = int(tr.n_pairs)
         return Trace(cell_of_pid, cell[:m], rnd[:m], pa[:m], pb[:m], P[:m], u[:m], dec[:m])
+
+    def step_local_sigma(self, nsteps, dt, eta_over_s):
+        """cuba_step_local_sigma: per-cell cross section for constant eta/s."""
+        _check(lib().cuba_step_local_sigma(self._h, int(nsteps), float(dt), float(eta_over_s)))
 
     def step_adaptive(self, nsteps, dt_max, sigma):
         """cuba_step_adaptive: returns (dt_used[nsteps], elapsed)."""

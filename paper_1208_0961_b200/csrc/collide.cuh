@@ -35,6 +35,9 @@ struct CollideParams {
     uint32_t *flags;
     // overflow class only: global scratch, 4 u32 per particle of the cell
     uint32_t *arena;
+    // local cross section for constant eta/s (etas > 0, A24): Eq. 3 without
+    // v_rel is computed per cell from the cell's population and energy sum instead of `base`
+    double etas, dt;
     // fused histogram of the NEXT step (next_dt > 0): the cell's CTA holds the final momenta on
     // chip, and the old cell of every particle is the cell itself, so S1-S3 of step t+1 are done
     // here and the (cell, direction) counts and the per-tile carries are written directly --
@@ -50,6 +53,40 @@ struct CollideParams {
     double *tr_P, *tr_u;
     uint8_t *tr_dec;
 };
+
+// Local cross section (A24): base_cell = ((0.1 S) dt) / ((hbarc (n n)) etas) with S the cell's
+// energy sum, DEFINED as the exact fixed-point sum (sum_i rint(E_i 2^40)) 2^-40 so that it does not
+// depend on the order in which threads add it up.
+constexpr double kHbarC = 0.197327;          // GeV fm (BASELINE.json:configs[0])
+constexpr double kFix40 = 1099511627776.0;   // 2^40
+
+__device__ __forceinline__ long long energy_fixed(double E) { return __double2ll_rn(E * kFix40); }
+
+__device__ __forceinline__ double local_base(long long acc, uint32_t n, double dt, double etas)
+{
+    const double S = (double)acc * (1.0 / kFix40);
+    const double nn = (double)n * (double)n;
+    return ((0.1 * S) * dt) / ((kHbarC * nn) * etas);
+}
+
+// Sum of one 64-bit integer per thread over the CTA (integer addition: any order gives the same
+// bits).  Call before a barrier, read with block_sum_ll_read after it.
+template <int THREADS>
+__device__ __forceinline__ void block_sum_ll_post(long long v, long long *s_slots)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+    if ((threadIdx.x & 31) == 0) s_slots[threadIdx.x >> 5] = v;
+}
+
+template <int THREADS>
+__device__ __forceinline__ long long block_sum_ll_read(const long long *s_slots)
+{
+    long long t = 0;
+#pragma unroll
+    for (int w = 0; w < THREADS / 32; ++w) t += s_slots[w];
+    return t;
+}
 
 // 53-bit uniform in [0,1)
 __device__ __forceinline__ double u53(uint32_t w0, uint32_t w1)
@@ -135,29 +172,33 @@ template <int THREADS, bool TRACE, typename IdxT>
 __device__ __forceinline__ void collide_cell(const CollideParams &P, uint32_t c, uint32_t lo, uint32_t n,
                                              double *sp0, double *sp1, double *sp2, double *sE,
                                              uint32_t *spid, uint32_t *skey, uint32_t *sbkt,
-                                             IdxT *sord, IdxT *stmp, uint32_t *s_warp,
+                                             IdxT *sord, IdxT *stmp, uint32_t *s_warp, long long *s_esum,
                                              unsigned long long &n_pairs, unsigned long long &n_coll,
                                              unsigned long long &n_near)
 {
     const int tid = threadIdx.x;
+    const uint32_t npairs = n >> 1;
+    long long esum = 0;
+    for (uint32_t j = tid; j < n; j += THREADS) {
+        const double a = P.px[lo + j], b = P.py[lo + j], cc = P.pz[lo + j];
+        sp0[j] = a; sp1[j] = b; sp2[j] = cc;
+        const double e = energy(a, b, cc);
+        sE[j] = e;
+        esum += energy_fixed(e);
+        spid[j] = P.pid[lo + j];
+    }
+    for (uint32_t j = tid; j <= n; j += THREADS) sbkt[j] = 0;
+    block_sum_ll_post<THREADS>(esum, s_esum);
+    __syncthreads();
     // rounds and scale (A5, A6): identical integer/fp64 results on every thread
+    const double base = (P.etas > 0.0) ? local_base(block_sum_ll_read<THREADS>(s_esum), n, P.dt, P.etas) : P.base;
     const double cn = (n & 1u) ? (double)n : (double)(n - 1u);
-    const double pmax = (2.0 * cn) * P.base;
+    const double pmax = (2.0 * cn) * base;
     int R;
     if (!(pmax <= 64.0)) { if (tid == 0) atomicOr(P.flags, kFlagRounds); R = 64; }
     else R = (pmax <= 1.0) ? 1 : (int)ceil(pmax);
     if (n < 2u) R = 0;
-    const double scale = (cn * P.base) / (double)R;
-    const uint32_t npairs = n >> 1;
-
-    for (uint32_t j = tid; j < n; j += THREADS) {
-        const double a = P.px[lo + j], b = P.py[lo + j], cc = P.pz[lo + j];
-        sp0[j] = a; sp1[j] = b; sp2[j] = cc;
-        sE[j] = energy(a, b, cc);
-        spid[j] = P.pid[lo + j];
-    }
-    for (uint32_t j = tid; j <= n; j += THREADS) sbkt[j] = 0;
-    __syncthreads();
+    const double scale = (cn * base) / (double)R;
 
     for (int rho = 0; rho < R; ++rho) {
         // (a) keys and bucket counts; the arrival slot only serves to park the element
@@ -500,28 +541,38 @@ struct ThreadStats {
     uint32_t hits;                       // uniform over a warp; lane 0 flushes
 };
 
-template <int THREADS, int ITEMS, int G, bool TRACE>
+template <int THREADS, int ITEMS, int G, bool TRACE, bool LOCAL>
 __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32_t c, uint32_t lo, uint32_t n,
                                                   double *sp0, double *sp1, double *sp2, double *sE,
                                                   uint32_t *spid, uint32_t *spark, uint32_t *sbkt,
                                                   uint16_t *sord, uint32_t *s_warp, CtaStats *stats,
-                                                  uint32_t *s_seg, ThreadStats &acc, uint32_t lo_next, uint32_t n_next)
+                                                  uint32_t *s_seg, long long *s_esum, ThreadStats &acc,
+                                                  uint32_t lo_next, uint32_t n_next)
 {
     static_assert(ITEMS % G == 0, "items are processed in groups of G");
     constexpr int NG = ITEMS / G;
     constexpr int PITEMS = (ITEMS + 1) / 2;          // pairs per thread
     constexpr int SCAN = ITEMS | 1;                  // words per thread in the scan (odd stride: no bank conflicts)
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const double cn = (n & 1u) ? (double)n : (double)(n - 1u);
-    const double pmax = (2.0 * cn) * P.base;
-    int R;
-    if (!(pmax <= 64.0)) { if (tid == 0) atomicOr(P.flags, kFlagRounds); R = 64; }
-    else R = (pmax <= 1.0) ? 1 : (int)ceil(pmax);
-    if (n < 2u) R = 0;          // a single particle has no partner; it is here for the fused histogram only
     const bool hist = P.next_dt > 0.0;
+    constexpr bool local = LOCAL;     // compile-time: the constant-sigma kernels carry none of its registers
+    // rounds and scale (A5, A6): identical integer/fp64 results on every thread.  With the local
+    // cross section the factor needs the cell's energy sum and is computed after staging.
+    double base = P.base;
+    const double cn = (n & 1u) ? (double)n : (double)(n - 1u);
+    int R = 0;
+    if (!local) {
+        const double pmax = (2.0 * cn) * base;
+        if (!(pmax <= 64.0)) { if (tid == 0) atomicOr(P.flags, kFlagRounds); R = 64; }
+        else R = (pmax <= 1.0) ? 1 : (int)ceil(pmax);
+        if (n < 2u) R = 0;          // a single particle has no partner; it is here for the fused histogram only
+    }
     if (tid == 0) {
-        const double scale = (cn * P.base) / (double)R;
-        stats->scale = scale; stats->hscale = 0.5 * scale; stats->lo = lo;
+        stats->lo = lo;
+        if (!local) {
+            const double scale = (cn * base) / (double)R;
+            stats->scale = scale; stats->hscale = 0.5 * scale;
+        }
         if (hist) hist_cell_setup(P.g, c, &stats->h);
     }
     const uint32_t npairs = n >> 1, nb = 2u * n, last = n - 1u;
@@ -530,6 +581,7 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
     uint32_t key[ITEMS], aux[ITEMS], keep[ITEMS];
 
     // ---- stage the cell: momenta, energies, pids; clear the bucket counters -----------------
+    long long esum = 0;
 #pragma unroll
     for (int g = 0; g < NG; ++g) {
         if ((uint32_t)(g * G * THREADS) >= n) break;
@@ -544,12 +596,27 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
         for (int i = 0; i < G; ++i) {
             const uint32_t j = tid + (g * G + i) * THREADS;
             const double e = energy(a[i], b[i], cc[i]);
-            if (j < n) { sp0[j] = a[i]; sp1[j] = b[i]; sp2[j] = cc[i]; sE[j] = e; spid[j] = id[i]; sbkt[j] = 0; }
+            if (j < n) {
+                sp0[j] = a[i]; sp1[j] = b[i]; sp2[j] = cc[i]; sE[j] = e; spid[j] = id[i]; sbkt[j] = 0;
+                if (local) esum += energy_fixed(e);
+            }
         }
     }
     if (hist)
         for (uint32_t e = tid; e < ((lo + n - 1u) / kTile - lo / kTile + 1u) * kDirs; e += THREADS) s_seg[e] = 0;
+    if (local) block_sum_ll_post<THREADS>(esum, s_esum);
     __syncthreads();
+    if (local) {
+        base = local_base(block_sum_ll_read<THREADS>(s_esum), n, P.dt, P.etas);
+        const double pmax = (2.0 * cn) * base;
+        if (!(pmax <= 64.0)) { if (tid == 0) atomicOr(P.flags, kFlagRounds); R = 64; }
+        else R = (pmax <= 1.0) ? 1 : (int)ceil(pmax);
+        if (n < 2u) R = 0;
+        if (tid == 0) {             // read in phase (e1), several barriers from here
+            const double scale = (cn * base) / (double)R;
+            stats->scale = scale; stats->hscale = 0.5 * scale;
+        }
+    }
     // the CTA's next cell goes to L2 while this one is processed, so its load phase does not wait on DRAM
     for (uint32_t l = tid * 16u; n_next && l < n_next + 16u; l += THREADS * 16u) {   // one 128 B line of doubles per thread
         const uint32_t e = lo_next + min(l, n_next - 1u);
@@ -852,7 +919,7 @@ __device__ __forceinline__ void flush_counters(const CollideParams &P, unsigned 
 // Shared-memory classes: CAP particles at most, 46 B of shared memory per particle.  The next
 // work item is fetched one cell ahead and its momenta / pids are prefetched into L2 while
 // the current cell is processed, so the load phase does not wait on DRAM.
-template <int THREADS, int ITEMS, int CAP, int MIN_BLOCKS, bool TRACE>
+template <int THREADS, int ITEMS, int CAP, int MIN_BLOCKS, bool TRACE, bool LOCAL>
 __global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
 k_collide(CollideParams P)
 {
@@ -871,6 +938,7 @@ k_collide(CollideParams P)
     __shared__ uint32_t s_warp[32];
     __shared__ CtaStats s_stats;
     __shared__ uint32_t s_seg[((CAP + kTile - 2) / kTile + 1) * kDirs];   // a cell of CAP particles spans at most this many tiles
+    __shared__ long long s_esum[32];
 
     // Dynamic work distribution, claimed one cell ahead so that the next cell can be prefetched
     // into L2.  (Measured alternatives, both slower because they lengthen the tail of the list:
@@ -890,8 +958,8 @@ k_collide(CollideParams P)
         item = s_item[(it + 1) & 1];
         uint4 nxt = make_uint4(0u, 0u, 0u, 0u);
         if (item < nlist) nxt = P.list[item];   // first used after the staging barrier
-        collide_cell_smem<THREADS, ITEMS, G, TRACE>(P, cur.x, cur.y, cur.z, sp0, sp1, sp2, sE, spid, spark, sbkt, sord,
-                                                    s_warp, &s_stats, s_seg, acc, nxt.y, nxt.z);
+        collide_cell_smem<THREADS, ITEMS, G, TRACE, LOCAL>(P, cur.x, cur.y, cur.z, sp0, sp1, sp2, sE, spid, spark, sbkt, sord,
+                                                    s_warp, &s_stats, s_seg, s_esum, acc, nxt.y, nxt.z);
         __syncthreads();
         cur = nxt;
     }
@@ -916,6 +984,7 @@ k_collide_overflow(CollideParams P, unsigned long long *arena_cursor, double *ar
     __shared__ uint32_t s_item;
     __shared__ unsigned long long s_base;
     __shared__ uint32_t s_run[32];
+    __shared__ long long s_esum[32];
     const uint32_t nlist = *P.list_count;
     unsigned long long n_pairs = 0, n_coll = 0, n_near = 0;
     for (;;) {
@@ -936,7 +1005,7 @@ k_collide_overflow(CollideParams P, unsigned long long *arena_cursor, double *ar
         // momenta in place: the "staging" copy is the particle store itself
         collide_cell<1024, TRACE, uint32_t>(P, c, lo, n, P.px + lo, P.py + lo, P.pz + lo, arena_E + b,
                                             const_cast<uint32_t *>(P.pid) + lo, skey, sbkt, sord, stmp,
-                                            s_warp, n_pairs, n_coll, n_near);
+                                            s_warp, s_esum, n_pairs, n_coll, n_near);
         __syncthreads();
         if (P.next_dt > 0.0) hist_cell_generic<1024>(P, c, lo, n, arena_E + b, s_run);
         __syncthreads();

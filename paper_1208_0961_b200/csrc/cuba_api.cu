@@ -275,8 +275,9 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
     }
 
 #define CUBA_OCC(K, T, I, C, MB)                                                                                          \
-    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, false>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]); \
-    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, true>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]);
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, true, false>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]); \
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, false, true>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]); \
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, false, false>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]);
     rc = CUBA_OK;
     CUBA_FOR_EACH_CLASS(CUBA_OCC)
 #undef CUBA_OCC
@@ -367,13 +368,14 @@ struct TraceDev {
 };
 
 template <bool TRACE>
-static int launch_collide(cuba_ctx *ctx, double base, const TraceDev *td, double next_dt)
+static int launch_collide(cuba_ctx *ctx, double base, const TraceDev *td, double next_dt, double etas = 0.0, double dt = 0.0)
 {
     const Layout &lay = ctx->lay;
     Soa &cur = ctx->set[ctx->cur];
     CollideParams P{};
     P.seed = ctx->seed; P.t = ctx->t; P.base = base;
     P.next_dt = next_dt; P.g = ctx->g;
+    P.etas = etas; P.dt = dt;
     P.x = cur.x; P.y = cur.y; P.z = cur.z;
     P.cnt = ctx->at<uint32_t>(lay.cnt); P.carry = ctx->at<uint32_t>(lay.carry);
     if (next_dt > 0.0) {      // the scatter of this step has consumed the offsets; empty cells must read as zero
@@ -407,7 +409,8 @@ static int launch_collide(cuba_ctx *ctx, double base, const TraceDev *td, double
         cudaStream_t st = serial ? main : ctx->cls_stream[K];                                    \
         if (!serial) CU(cudaStreamWaitEvent(st, ctx->ev_fork, 0));                               \
         cls(K);                                                                                  \
-        k_collide<T, I, C, MB, TRACE><<<ctx->grid_cls[K], T, collide_smem_bytes(C), st>>>(P);    \
+        if (!TRACE && etas > 0.0) k_collide<T, I, C, MB, false, true><<<ctx->grid_cls[K], T, collide_smem_bytes(C), st>>>(P); \
+        else k_collide<T, I, C, MB, TRACE, false><<<ctx->grid_cls[K], T, collide_smem_bytes(C), st>>>(P);    \
         LAUNCHED();                                                                              \
         if (serial) prof_mark(ctx, G_COLLIDE0 + K);                                              \
         else { CU(cudaEventRecord(ctx->ev_join[K], st)); CU(cudaStreamWaitEvent(main, ctx->ev_join[K], 0)); } \
@@ -501,7 +504,8 @@ static int enqueue_bin(cuba_ctx *ctx, double dt, uint32_t *cell_of_pid)
     return CUBA_OK;
 }
 
-int cuba_step(cuba_ctx *ctx, int nsteps, double dt, double sigma)
+// fixed time step; etas > 0 selects the local cross section (sigma is then unused)
+static int step_fixed(cuba_ctx *ctx, int nsteps, double dt, double sigma, double etas)
 {
     if (!ctx) return CUBA_ERR_NULL;
     if (nsteps < 0) return CUBA_ERR_SIZE;
@@ -512,7 +516,7 @@ int cuba_step(cuba_ctx *ctx, int nsteps, double dt, double sigma)
         rc = enqueue_bin(ctx, dt, nullptr);
         if (rc != CUBA_OK) return rc;
         const double next_dt = ctx->fuse_hist ? dt : 0.0;
-        rc = launch_collide<false>(ctx, base, nullptr, next_dt);
+        rc = launch_collide<false>(ctx, base, nullptr, next_dt, etas, dt);
         if (rc != CUBA_OK) return rc;
         ctx->pre_dt = next_dt;
         ctx->t += 1;
@@ -520,6 +524,17 @@ int cuba_step(cuba_ctx *ctx, int nsteps, double dt, double sigma)
         ctx->nmax_valid = false;
     }
     return CUBA_OK;
+}
+
+int cuba_step(cuba_ctx *ctx, int nsteps, double dt, double sigma)
+{
+    return step_fixed(ctx, nsteps, dt, sigma, 0.0);
+}
+
+int cuba_step_local_sigma(cuba_ctx *ctx, int nsteps, double dt, double eta_over_s)
+{
+    if (!(eta_over_s > 0.0) || !std::isfinite(eta_over_s)) return ctx ? CUBA_ERR_VALUE : CUBA_ERR_NULL;
+    return step_fixed(ctx, nsteps, dt, 0.0, eta_over_s);
 }
 
 // Variable time step, reading A23: the same fp64 expression, in the same order, as the oracle's.

@@ -165,6 +165,36 @@ def test_lrf_observables_match_oracle(cuba, oracle_mod):
             g.observables_lrf(bad)
 
 
+def test_local_cross_section_matches_oracle(cuba, oracle_mod):
+    """sigma per cell from the cell's n and <E> for constant eta/s.  The
+    per-cell factor comes from an order-free fixed-point energy sum, so rounds, decisions and the
+    state are the oracle's bit for bit: several size classes, many rounds (small eta/s), the
+    overflow kernel, both schedules, mixed with constant-sigma steps."""
+    cases = [(workloads.riemann_small(), 0.4), (workloads.riemann_small(), 0.02),
+             (workloads.riemann(L=(6.0, 3.0, 2.0), ncell=(12, 3, 2), r_test=90.0, dt=0.05, seed=13), 0.1),
+             (workloads.thermal_box(L=(1.0, 1.0, 1.0), ncell=(1, 1, 1), count=6000, seed=4, r_test=2000.0), 0.5)]
+    for w, etas in cases:
+        for fuse in (1, 0):
+            g = cuba.Cuba.from_workload(w)
+            g.set_option(1, fuse)
+            o = oracle_mod.Oracle.from_workload(w)
+            g.step_local_sigma(3, w.dt, etas)
+            o.step_etas(3, w.dt, etas)
+            assert_state_equal(g.particles(), o.particles())
+            g.step(1, w.dt, w.sigma)
+            o.step(1, w.dt, w.sigma)
+            g.step_local_sigma(2, w.dt, etas)
+            o.step_etas(2, w.dt, etas)
+            assert_state_equal(g.particles(), o.particles())
+            gc, oc = g.counters(), o.counters()
+            assert (gc.pairs, gc.collisions, gc.rounds) == (oc["pairs"], oc["collisions"], oc["rounds"])
+            assert gc.device_flags == 0 and oc["collisions"] > 0
+    assert oracle_mod.Oracle.from_workload(cases[1][0]) is not None
+    g = cuba.Cuba.from_workload(cases[0][0])
+    with pytest.raises(cuba.CubaError):
+        g.step_local_sigma(1, 0.1, 0.0)
+
+
 def test_adaptive_time_step_matches_oracle(cuba, oracle_mod):
     """the dt sequence (a function of the integer occupancy of the fullest
     cell), the elapsed time and the state are the oracle's bit for bit -- where the rule binds
