@@ -831,8 +831,17 @@ int cuba_run_host(const double box[3], const int ncell[3], int64_t n,
     cudaStream_t st = nullptr;
     auto body = [&]() -> int {
         CU(cudaStreamCreate(&st));
-        for (int k = 0; k < 6; ++k) CU(cudaMalloc(&dev[k], (size_t)n * 8));
-        CU(cudaMalloc(&ws, wsb));
+        // stream-ordered allocations from the device's default pool, which is told to keep what it
+        // has been given: a second call of the same size maps no new memory (cudaMalloc / cudaFree
+        // of 3.3 GB cost ~10 ms per call at 24.9M particles)
+        int dev_id = 0;
+        CU(cudaGetDevice(&dev_id));
+        cudaMemPool_t pool;
+        CU(cudaDeviceGetDefaultMemPool(&pool, dev_id));
+        uint64_t keep = UINT64_MAX;
+        CU(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+        for (int k = 0; k < 6; ++k) CU(cudaMallocAsync(reinterpret_cast<void **>(&dev[k]), (size_t)n * 8, st));
+        CU(cudaMallocAsync(&ws, wsb, st));
         for (int k = 0; k < 6; ++k) CU(cudaMemcpyAsync(dev[k], host[k], (size_t)n * 8, cudaMemcpyHostToDevice, st));
         int r = cuba_init(&ctx, box, ncell, n, dev[0], dev[1], dev[2], dev[3], dev[4], dev[5], n_test, seed, ws, wsb, st);
         if (r != CUBA_OK) return r;
@@ -851,9 +860,12 @@ int cuba_run_host(const double box[3], const int ncell[3], int64_t n,
     };
     const int rc = body();
     if (ctx) cuba_destroy(ctx);
-    for (int k = 0; k < 6; ++k) cudaFree(dev[k]);
-    cudaFree(ws);
-    if (st) cudaStreamDestroy(st);
+    if (st) {
+        for (int k = 0; k < 6; ++k) if (dev[k]) cudaFreeAsync(dev[k], st);
+        if (ws) cudaFreeAsync(ws, st);
+        cudaStreamSynchronize(st);
+        cudaStreamDestroy(st);
+    }
     return rc;
 }
 
