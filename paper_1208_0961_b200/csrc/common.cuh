@@ -9,7 +9,10 @@ namespace cuba {
 
 constexpr int kDirs = 27;           // (dix+1)*9 + (diy+1)*3 + (diz+1), each di in {-1,0,1}
 constexpr int kTileThreads = 256;
-constexpr int kTileItems = 2;
+#ifndef CUBA_TILE_ITEMS
+#define CUBA_TILE_ITEMS 2
+#endif
+constexpr int kTileItems = CUBA_TILE_ITEMS;
 constexpr int kTile = kTileThreads * kTileItems;   // particles per tile in the flat passes
 constexpr int kTileRows = kTile / 32;
 constexpr int kTileRec = 32;        // u32 words per tile record: 27 counts, cf, cl, pad
