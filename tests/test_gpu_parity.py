@@ -306,6 +306,67 @@ def test_edge_cases_match_oracle(cuba, oracle_mod, case):
         assert gc.pairs == 0
 
 
+@pytest.mark.parametrize("case", ["cfl_limit", "thin_axis", "anisotropic_cells", "sparse_grid", "odd_box"])
+def test_stress_geometries_match_oracle(cuba, oracle_mod, case):
+    """Geometries that stress the direction logic of the fused histogram and the placement:
+    dt just below the smallest cell edge (about half of the particles change cell,
+    many through edges and corners, reflections combined with cell changes), an axis one cell
+    thick (both faces of every cell are walls), strongly anisotropic cells, a grid where most
+    cells hold no or one particle, and a box with non-representable cell edges."""
+    if case == "cfl_limit":
+        w = workloads.thermal_box(L=(6.0, 5.0, 4.0), ncell=(6, 5, 4), count=40000, seed=61, r_test=30.0, dt=0.999)
+    elif case == "thin_axis":
+        w = workloads.thermal_box(L=(9.0, 1.0, 7.0), ncell=(9, 1, 7), count=30000, seed=62, r_test=40.0, dt=0.6)
+    elif case == "anisotropic_cells":
+        w = workloads.thermal_box(L=(4.0, 8.0, 2.0), ncell=(16, 4, 2), count=50000, seed=63, r_test=60.0, dt=0.24)
+    elif case == "sparse_grid":
+        w = workloads.thermal_box(L=(20.0, 20.0, 20.0), ncell=(40, 40, 40), count=30000, seed=64, r_test=2.0, dt=0.3)
+    else:
+        w = workloads.thermal_box(L=(3.3, 2.7, 1.9), ncell=(7, 3, 5), count=20000, seed=65, r_test=25.0, dt=0.3)
+    for fuse in (1, 0):
+        g = cuba.Cuba.from_workload(w)
+        g.set_option(1, fuse)
+        o = oracle_mod.Oracle.from_workload(w)
+        for _ in range(4):
+            g.step(2, w.dt, w.sigma)
+            o.step(2, w.dt, w.sigma)
+            assert_state_equal(g.particles(), o.particles())
+            assert np.array_equal(g.cell_start(), o.cells()[1])
+        gc, oc = g.counters(), o.counters()
+        assert (gc.pairs, gc.collisions, gc.rounds) == (oc["pairs"], oc["collisions"], oc["rounds"])
+        assert gc.device_flags == 0
+        if case != "sparse_grid":
+            assert oc["collisions"] > 100
+
+
+def test_config1_full_run_profiles_match_oracle(cuba, oracle_mod):
+    """Protocol (ii) of SURVEY 8(c) at BASELINE.json:configs[1] itself: 2.49M testparticles, 100
+    steps, 64-slab energy-density profiles every 10 steps.  Under the arithmetic contract A2 the
+    trajectories are identical, so the profiles agree to the summation-order tolerance and the
+    final store bit for bit (the oracle needs about a minute of one host core)."""
+    w = workloads.make(1)
+    g = cuba.Cuba.from_workload(w)
+    o = oracle_mod.Oracle.from_workload(w)
+    tot0, _ = g.observables(64)
+    for _ in range(10):
+        g.step(10, w.dt, w.sigma)
+        o.step(10, w.dt, w.sigma)
+        gt, ge = g.observables(64)
+        ot, oe = o.observables(64)
+        assert np.allclose(ge, oe, rtol=REL, atol=0)
+        assert gt[0] == pytest.approx(ot[0], rel=REL)
+    assert_state_equal(g.particles(), o.particles())
+    assert abs(gt[0] - tot0[0]) / tot0[0] < 1e-10                      # PAPER.md:66
+    T, lrf = g.observables_lrf(64)
+    assert_lrf_equal((T, lrf), o.observables_lrf(64))
+    # two waves leave the initial discontinuity at x = 16 (PAPER.md:70-72): the far ends are still
+    # at their initial energy densities, the middle lies in between, matter flows to the right
+    assert lrf[0, :8].mean() == pytest.approx(16.204, rel=0.02) and lrf[0, -8:].mean() == pytest.approx(1.0127, rel=0.03)
+    assert 1.5 < lrf[0, 30:36].mean() < 15.0 and lrf[1, 28:40].max() > 0.2
+    gc, oc = g.counters(), o.counters()
+    assert (gc.steps, gc.pairs, gc.collisions) == (100, oc["pairs"], oc["collisions"])
+
+
 def test_wall_reflection_on_device_preserves_energy_bits(cuba):
     """PAPER.md:44 with sigma = 0: after many wall hits every |p| is bit-identical."""
     import torch
