@@ -47,6 +47,23 @@ BYTES_STEP_FUSED = BYTES_SCATTER + BYTES_COLLIDE_FUSED           # 180: what the
 # `ncu --set full` capture (profiles/r01_v4_summary.md): (config, fused schedule, kernel group) -> bytes.
 # The group is the hot collision class (1.487 + 0.508 GB) plus the cold one (0.138 + 0.029 GB).
 NCU_TRAFFIC = {(2, True, "k_collide (all classes, concurrent)"): 2.162e9}
+# smsp__inst_executed.sum (warp instructions) per step of the same kernel group from the same capture:
+# the collision kernels are bound by instruction issue and latency, not by HBM, so the line also says
+# how far they are from the issue peak of 148 SMs x 4 schedulers x 1 warp instruction per clock.
+NCU_WARP_INST = {(2, True, "k_collide (all classes, concurrent)"): 645.1e6}
+ISSUE_SLOTS_PER_CLOCK = 148 * 4
+
+
+def issue_roofline(warp_inst, ms, clocks):
+    """Secondary roofline of an issue-bound kernel: recorded warp instructions per launch / measured
+    duration against 592 issue slots x the SM clock sampled during the run."""
+    mhz = (clocks or {}).get("sm_mhz") or (clocks or {}).get("sm_max_mhz")
+    if not warp_inst or not ms or not mhz:
+        return None
+    achieved = warp_inst / (ms * 1e-3) / 1e9
+    peak = ISSUE_SLOTS_PER_CLOCK * mhz * 1e6 / 1e9
+    return {"bound": "issue", "achieved": achieved, "peak": peak, "unit": "G warp-inst/s", "frac": achieved / peak,
+            "source": "smsp__inst_executed.sum from profiles/r01_v4_summary.md / CUDA-event duration of this run"}
 
 
 def peaks():
@@ -324,6 +341,7 @@ def main():
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((args.config, fused, dom)), "peak_source": peak_src,
                          "alg_bytes_per_launch": alg.get(dom, 0),
+                         "issue": issue_roofline(NCU_WARP_INST.get((args.config, fused, dom)), dom_ms, sampler.summary()),
                          "step": {"alg_bytes_per_particle": BYTES_STEP,
                                   "moved_bytes_per_particle": BYTES_STEP_FUSED if fused else BYTES_STEP,
                                   "achieved": BYTES_STEP * value / world / 1e9,
