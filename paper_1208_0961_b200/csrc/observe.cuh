@@ -15,32 +15,32 @@ constexpr int kObsMaxSlabs = 1024;
 constexpr int kLrfComp = 5;                     // T00, T0x, Txx, Tyy, Tzz
 constexpr int kLrfMaxSlabs = 256;               // kObsWarps * 5 * 256 doubles = 80 KB of shared memory
 
-// Every thread keeps a running sum for the slab of the particles it has seen last.  The store is
-// cell-sorted with x slowest and a CTA walks a contiguous range of tiles, so that slab changes a
-// handful of times per kernel; when it changes for any lane the whole warp reduces its running
-// sums (slab by slab, shuffle tree) into the warp's shared-memory bins and starts afresh.  When
-// and what is flushed depends on the data only, never on scheduling: the result is
-// bit-reproducible from run to run.
+// Every thread keeps running sums for two adjacent slabs, base and base + 1, with base uniform
+// over the warp.  The store is cell-sorted with x slowest and a CTA walks a contiguous range of
+// tiles, so consecutive particles lie in one layer of cells -- which spans one or two slabs when
+// nslab <= 2 nx (x is random inside a cell, so the two alternate from particle to particle).  Only
+// when some lane meets a slab outside {base, base + 1} does the warp reduce its sums (shuffle
+// trees) into its shared-memory bins and move the base.  When that happens depends on the data
+// only, never on scheduling: the result is bit-reproducible from run to run.  (More than two
+// slabs per cell layer still work, with a flush per change.)
 template <int NC>
-__device__ __forceinline__ void warp_flush(double (&acc)[NC], int &slab, double *bins, int nslab, int lane)
+__device__ __forceinline__ void warp_flush(double (&acc0)[NC], double (&acc1)[NC], int base, double *bins, int nslab, int lane)
 {
-    uint32_t todo = __ballot_sync(0xFFFFFFFFu, slab >= 0);
-    while (todo) {
-        const int leader = __ffs(todo) - 1;
-        const int s0 = __shfl_sync(0xFFFFFFFFu, slab, leader);
-        const bool mine = slab == s0;
+    if (base < 0) return;
 #pragma unroll
-        for (int q = 0; q < NC; ++q) {
-            double r = mine ? acc[q] : 0.0;
+    for (int q = 0; q < NC; ++q) {
+        double r0 = acc0[q], r1 = acc1[q];
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) r += __shfl_xor_sync(0xFFFFFFFFu, r, o);
-            if (lane == 0) bins[q * nslab + s0] += r;
+        for (int o = 16; o > 0; o >>= 1) {
+            r0 += __shfl_xor_sync(0xFFFFFFFFu, r0, o);
+            r1 += __shfl_xor_sync(0xFFFFFFFFu, r1, o);
         }
-        todo &= ~__ballot_sync(0xFFFFFFFFu, mine);
+        if (lane == 0) {
+            bins[q * nslab + base] += r0;
+            if (base + 1 < nslab) bins[q * nslab + base + 1] += r1;
+        }
+        acc0[q] = 0.0; acc1[q] = 0.0;
     }
-    slab = -1;
-#pragma unroll
-    for (int q = 0; q < NC; ++q) acc[q] = 0.0;
 }
 
 // LRF = false: energy density per slab (NC = 1) + totals (sum E, sum p); partial layout per
@@ -63,10 +63,10 @@ k_observe_partial(int64_t n, const double *__restrict__ x, const double *__restr
     for (int s = lane; s < NC * nslab; s += 32) bins[s] = 0.0;
     __syncwarp();
     double tE = 0.0, tx = 0.0, ty = 0.0, tz = 0.0;
-    double acc[NC];
+    double acc0[NC], acc1[NC];
 #pragma unroll
-    for (int q = 0; q < NC; ++q) acc[q] = 0.0;
-    int cur = -1;
+    for (int q = 0; q < NC; ++q) { acc0[q] = 0.0; acc1[q] = 0.0; }
+    int base = -1;                              // warp-uniform
     const int64_t ntiles = (n + kObsTile - 1) / kObsTile;
     const int64_t per = (ntiles + gridDim.x - 1) / gridDim.x;     // contiguous range of tiles per CTA
     const int64_t t0 = blockIdx.x * per, t1 = min(ntiles, t0 + per);
@@ -80,25 +80,63 @@ k_observe_partial(int64_t n, const double *__restrict__ x, const double *__restr
 #pragma unroll
         for (int k = 0; k < kObsItems; ++k) {
             const bool valid = tile * kObsTile + k * kObsThreads + tid < n;
-            const int slab = valid ? min(max(__double2int_rz(xx[k] * inv_w), 0), nslab - 1) : cur;
-            if (__any_sync(0xFFFFFFFFu, cur >= 0 && slab != cur)) warp_flush<NC>(acc, cur, bins, nslab, lane);
+            double v[NC];
+#pragma unroll
+            for (int q = 0; q < NC; ++q) v[q] = 0.0;
             if (valid) {
                 const double E = energy(a[k], b[k], c[k]);
-                cur = slab;
-                acc[0] += E;
+                v[0] = E;
                 if (LRF) {
                     const double w = 1.0 / E;
-                    acc[1 % NC] += a[k];
-                    acc[2 % NC] += (a[k] * a[k]) * w;
-                    acc[3 % NC] += (b[k] * b[k]) * w;
-                    acc[4 % NC] += (c[k] * c[k]) * w;
+                    v[1 % NC] = a[k];
+                    v[2 % NC] = (a[k] * a[k]) * w;
+                    v[3 % NC] = (b[k] * b[k]) * w;
+                    v[4 % NC] = (c[k] * c[k]) * w;
                 } else {
                     tE += E; tx += a[k]; ty += b[k]; tz += c[k];
                 }
             }
+            const int slab = valid ? min(max(__double2int_rz(xx[k] * inv_w), 0), nslab - 1) : -1;
+            bool keep = true;
+            if (__any_sync(0xFFFFFFFFu, valid && (base < 0 || slab < base || slab > base + 1))) {
+                warp_flush<NC>(acc0, acc1, base, bins, nslab, lane);
+                int m = valid ? slab : 0x7FFFFFFF;              // new base: the smallest slab present
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) m = min(m, __shfl_xor_sync(0xFFFFFFFFu, m, o));
+                base = m;
+                if (__any_sync(0xFFFFFFFFu, valid && slab > base + 1)) {
+                    // more than two slabs among these 32 particles (nslab > 2 nx): peel them off one
+                    // slab at a time straight into the bins; nothing is carried over
+                    uint32_t todo = __ballot_sync(0xFFFFFFFFu, valid);
+                    while (todo) {
+                        const int leader = __ffs(todo) - 1;
+                        const int s0 = __shfl_sync(0xFFFFFFFFu, slab, leader);
+                        const bool mine = valid && slab == s0;
+#pragma unroll
+                        for (int q = 0; q < NC; ++q) {
+                            double r = mine ? v[q] : 0.0;
+#pragma unroll
+                            for (int o = 16; o > 0; o >>= 1) r += __shfl_xor_sync(0xFFFFFFFFu, r, o);
+                            if (lane == 0) bins[q * nslab + s0] += r;
+                        }
+                        todo &= ~__ballot_sync(0xFFFFFFFFu, mine);
+                    }
+                    base = -1;
+                    keep = false;
+                }
+            }
+            if (keep && valid) {
+                if (slab == base) {
+#pragma unroll
+                    for (int q = 0; q < NC; ++q) acc0[q] += v[q];
+                } else {
+#pragma unroll
+                    for (int q = 0; q < NC; ++q) acc1[q] += v[q];
+                }
+            }
         }
     }
-    warp_flush<NC>(acc, cur, bins, nslab, lane);
+    warp_flush<NC>(acc0, acc1, base, bins, nslab, lane);
     if (!LRF) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
