@@ -4,7 +4,9 @@
 // the store is always cell-sorted (A19) and dt < cell edge, so a particle of
 // old cell c can only land in one of the 27 cells around c.  A counting sort keyed by
 // (old cell, direction d in 0..26) is therefore sparse:
-//   K_A  k_stream_hist   per particle: S1-S3, d; cnt[d][c_old] += 1   (order-free u32 adds)
+//   K_A  k_stream_hist   per particle: S1-S3, d; cnt[d][c_old] += 1   (order-free u32 adds).  In the
+//                        steady state this pass and K_carry do not run: the collision kernel of
+//                        the previous step has written cnt and carry (collide.cuh, fused histogram)
 //   K_B  k_gather        per new cell: the <= 27 (source cell, d) counts that feed it, taken
 //                        in ascending source-cell order = ascending previous array index,
 //                        turned into exclusive offsets in place; their sum is the new count
@@ -15,7 +17,7 @@
 //                        (c_old, d) group from warp votes, dest = cell_start[c_new] +
 //                        off[d][c_old] + rank.  No atomics touch the order: the placement is
 //                        the stable counting sort of north_star (3), deterministic by construction.
-// HBM traffic per particle-step: K_A reads 48 B, K_C reads 52 B and writes 52 B.
+// HBM traffic per particle-step: K_A reads 48 B (when it runs), K_C reads 52 B and writes 52 B.
 #pragma once
 #include "common.cuh"
 

@@ -4,7 +4,9 @@
 // One CTA per cell (persistent CTAs pull cells of their size class from a work list).
 // The cell's momenta, cached energies and pids are staged in shared memory once; all R(n)
 // rounds run on chip; momenta are written back once.  HBM traffic: 28 B read + 24 B written
-// per particle.
+// per particle, + 24 B read (x, y, z) when the kernel also prepares the counting-sort
+// histogram of the next step ("fused histogram" below).  Template switches: TRACE (parity
+// records per pair) and LOCAL (per-cell cross section for constant eta/s, A24).
 //
 // The shuffle is "sort by (Philox word, pid)" (A7).  Keys are uniform 32-bit
 // numbers, so the sort is a one-pass bucket sort: n buckets, bucket = floor(key * n / 2^32)
