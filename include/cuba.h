@@ -142,6 +142,12 @@ int cuba_step_adaptive(cuba_ctx *ctx, int nsteps, double dt_max, double sigma, d
  * one (or that follows cuba_init / cuba_step_traced) runs that pass.  value 0 always runs the
  * separate pass.  Errors: CUBA_ERR_NULL, CUBA_ERR_VALUE (unknown option or value). */
 #define CUBA_OPT_FUSE_HIST 1
+/* CUBA_OPT_GRAPH (default 1): for problems of up to 2^20 particles, whose step is bound by the host
+ * cost of its launches, cuba_step replays a CUDA graph of two steps (captured on first use for the
+ * given dt and sigma) instead of launching the kernels one by one -- provided the context's stream
+ * can be captured (not the legacy default stream or cudaStreamPerThread) and per-kernel profiling
+ * is off.  value 0: plain launches.  Results are identical either way. */
+#define CUBA_OPT_GRAPH 2
 int cuba_set_option(cuba_ctx *ctx, int option, int value);
 
 /* PAPER.md:66 (total energy) and PAPER.md:68-70 Fig. 2 (energy density along x).

@@ -180,10 +180,10 @@ class Cuba:
         self._h = h
 
     @classmethod
-    def from_workload(cls, w, device="cuda:0"):
+    def from_workload(cls, w, device="cuda:0", stream=None):
         import torch
         t = [torch.from_numpy(a).to(device) for a in w.arrays()]
-        return cls(w.box, w.ncell, *t, w.n_test, w.seed)
+        return cls(w.box, w.ncell, *t, w.n_test, w.seed, stream=stream)
 
     def close(self):
         if self._h:

@@ -26,6 +26,7 @@ struct CollideParams {
     uint64_t seed;
     uint32_t rk[20];      // Philox round keys: rk[2r] = seed_lo + r*0x9E3779B9, rk[2r+1] = seed_hi + r*0xBB67AE85
     uint32_t t;           // global step index
+    const uint32_t *t_dev; // GRAPH instantiations: the step index lives in device memory (a replayed graph cannot carry it)
     double base;          // sigma*dt/(r_test*V_cell): Eq. 3 without v_rel
     const uint32_t *cell_start;
     const uint4 *list;    // cells of this size class: {cell, first slot, population, -}
@@ -98,9 +99,9 @@ __device__ __forceinline__ double u53(uint32_t w0, uint32_t w1)
 
 // draw() with the key schedule taken from the kernel parameters (constant bank operands):
 // the same function of (seed, id, t, rho, tag, sub), without 18 key additions per call.
-__device__ __forceinline__ U4 drawk(const CollideParams &P, uint32_t id, uint32_t rho, uint32_t tag, uint32_t sub)
+__device__ __forceinline__ U4 drawk(const CollideParams &P, uint32_t t, uint32_t id, uint32_t rho, uint32_t tag, uint32_t sub)
 {
-    uint32_t c0 = id, c1 = P.t, c2 = rho, c3 = (tag << 16) | sub;
+    uint32_t c0 = id, c1 = t, c2 = rho, c3 = (tag << 16) | sub;
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
         const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
@@ -180,6 +181,7 @@ __device__ __forceinline__ void collide_cell(const CollideParams &P, uint32_t c,
 {
     const int tid = threadIdx.x;
     const uint32_t npairs = n >> 1;
+    const uint32_t tcur = P.t_dev ? *P.t_dev : P.t;
     long long esum = 0;
     for (uint32_t j = tid; j < n; j += THREADS) {
         const double a = P.px[lo + j], b = P.py[lo + j], cc = P.pz[lo + j];
@@ -205,7 +207,7 @@ __device__ __forceinline__ void collide_cell(const CollideParams &P, uint32_t c,
     for (int rho = 0; rho < R; ++rho) {
         // (a) keys and bucket counts; the arrival slot only serves to park the element
         for (uint32_t j = tid; j < n; j += THREADS) {
-            const uint32_t k = shuf_word(draw(P.seed, spid[j], P.t, (uint32_t)rho >> 2, kTagShuf, 0), rho);
+            const uint32_t k = shuf_word(draw(P.seed, spid[j], tcur, (uint32_t)rho >> 2, kTagShuf, 0), rho);
             skey[j] = k;
             sord[j] = (IdxT)atomicAdd(&sbkt[__umulhi(k, n)], 1u);
         }
@@ -253,7 +255,7 @@ __device__ __forceinline__ void collide_cell(const CollideParams &P, uint32_t c,
             const double vrel = 0.5 * (s / ee);                       // s/(2 E_a E_b)
             const double prob = vrel * scale;                         // Eq. 3 * cn/R
             const uint32_t ida = spid[a];
-            const U4 w = draw(P.seed, ida, P.t, (uint32_t)rho, kTagDec, 0);
+            const U4 w = draw(P.seed, ida, tcur, (uint32_t)rho, kTagDec, 0);
             const double u = u53(w.x, w.y);
             const bool hit = u < prob;
             n_pairs += 1;
@@ -265,7 +267,7 @@ __device__ __forceinline__ void collide_cell(const CollideParams &P, uint32_t c,
             }
             if (hit) {
                 double nx, ny, nz;
-                draw_direction(P.seed, ida, P.t, (uint32_t)rho, nx, ny, nz);
+                draw_direction(P.seed, ida, tcur, (uint32_t)rho, nx, ny, nz);
                 const double rs = sqrt(s);
                 const double Pvx = pax + pbx, Pvy = pay + pby, Pvz = paz + pbz;
                 const double Et = Ea + Eb;
@@ -426,11 +428,11 @@ __device__ __forceinline__ double u53_bits(uint32_t w0, uint32_t w1)
 }
 
 // Marsaglia disc rejection (A11) with the key schedule from the parameters.
-__device__ __forceinline__ void draw_direction_k(const CollideParams &P, uint32_t pid, uint32_t rho,
+__device__ __forceinline__ void draw_direction_k(const CollideParams &P, uint32_t t, uint32_t pid, uint32_t rho,
                                                  double &nx, double &ny, double &nz)
 {
     for (uint32_t call = 0; call < 65536u; ++call) {
-        const U4 w = drawk(P, pid, rho, kTagDir, call);
+        const U4 w = drawk(P, t, pid, rho, kTagDir, call);
 #pragma unroll
         for (int half = 0; half < 2; ++half) {
             const uint32_t wa = half ? w.z : w.x, wb = half ? w.w : w.y;
@@ -448,13 +450,13 @@ __device__ __forceinline__ void draw_direction_k(const CollideParams &P, uint32_
 }
 
 // Boost to the CM frame, isotropic direction, boost back (closed form A10).
-__device__ __forceinline__ void pair_scatter(const CollideParams &P, uint32_t ida, uint32_t rho, double s,
+__device__ __forceinline__ void pair_scatter(const CollideParams &P, uint32_t t, uint32_t ida, uint32_t rho, double s,
                                              double pax, double pay, double paz, double Ea,
                                              double pbx, double pby, double pbz, double Eb,
                                              double q[6])
 {
     double nx, ny, nz;
-    draw_direction_k(P, ida, rho, nx, ny, nz);
+    draw_direction_k(P, t, ida, rho, nx, ny, nz);
     const double rs = sqrt(s);
     const double Pvx = pax + pbx, Pvy = pay + pby, Pvz = paz + pbz;
     const double Et = Ea + Eb;
@@ -543,7 +545,7 @@ struct ThreadStats {
     uint32_t hits;                       // uniform over a warp; lane 0 flushes
 };
 
-template <int THREADS, int ITEMS, int G, bool TRACE, bool LOCAL>
+template <int THREADS, int ITEMS, int G, bool TRACE, bool LOCAL, bool GRAPH>
 __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32_t c, uint32_t lo, uint32_t n,
                                                   double *sp0, double *sp1, double *sp2, double *sE,
                                                   uint32_t *spid, uint32_t *spark, uint32_t *sbkt,
@@ -556,6 +558,9 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
     constexpr int PITEMS = (ITEMS + 1) / 2;          // pairs per thread
     constexpr int SCAN = ITEMS | 1;                  // words per thread in the scan (odd stride: no bank conflicts)
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    // step index: a constant-bank operand normally; a register loaded from device memory when the
+    // kernel is a node of a replayed CUDA graph (small problems only, where registers are plentiful)
+    const uint32_t tcur = GRAPH ? *P.t_dev : P.t;
     const bool hist = P.next_dt > 0.0;
     constexpr bool local = LOCAL;     // compile-time: the constant-sigma kernels carry none of its registers
     // rounds and scale (A5, A6): identical integer/fp64 results on every thread.  With the local
@@ -639,7 +644,7 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
                 for (int i = 0; i < G; ++i) {
                     const int it = g * G + i;
                     const uint32_t jc = min((uint32_t)(tid + it * THREADS), last);
-                    const U4 w = drawk(P, spid[jc], (uint32_t)rho >> 2, kTagShuf, 0);
+                    const U4 w = drawk(P, tcur, spid[jc], (uint32_t)rho >> 2, kTagShuf, 0);
                     key[it] = (rho & 2) ? w.z : w.x;
                     keep[it] = (rho & 2) ? w.w : w.y;
                 }
@@ -717,7 +722,7 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
             if (any) {
 #pragma unroll
                 for (int i = 0; i < G; ++i)
-                    if (slow[i]) rank[i] = slow_rank(P.seed, P.t, spark, spid, n, nb, tid + (g * G + i) * THREADS,
+                    if (slow[i]) rank[i] = slow_rank(P.seed, tcur, spark, spid, n, nb, tid + (g * G + i) * THREADS,
                                                      key[g * G + i], aux[g * G + i], rho);
             }
 #pragma unroll
@@ -752,7 +757,7 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
             }
 #pragma unroll
             for (int it = 0; it < PITEMS; ++it) {
-                const U4 w = drawk(P, ida[it], (uint32_t)rho, kTagDec, 0);
+                const U4 w = drawk(P, tcur, ida[it], (uint32_t)rho, kTagDec, 0);
                 u[it] = u53_bits(w.x, w.y);
             }
 #pragma unroll
@@ -803,7 +808,7 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
             const double dz = Eb * paz - Ea * pbz;
             const double s = ((dx * dx + dy * dy) + dz * dz) / ee;
             double q[6];
-            pair_scatter(P, spid[a], (uint32_t)rho, s, pax, pay, paz, Ea, pbx, pby, pbz, Eb, q);
+            pair_scatter(P, tcur, spid[a], (uint32_t)rho, s, pax, pay, paz, Ea, pbx, pby, pbz, Eb, q);
             sp0[a] = q[0]; sp1[a] = q[1]; sp2[a] = q[2];
             sp0[b] = q[3]; sp1[b] = q[4]; sp2[b] = q[5];
             if (rho + 1 < R || hist) { sE[a] = energy(q[0], q[1], q[2]); sE[b] = energy(q[3], q[4], q[5]); }
@@ -921,7 +926,7 @@ __device__ __forceinline__ void flush_counters(const CollideParams &P, unsigned 
 // Shared-memory classes: CAP particles at most, 46 B of shared memory per particle.  The next
 // work item is fetched one cell ahead and its momenta / pids are prefetched into L2 while
 // the current cell is processed, so the load phase does not wait on DRAM.
-template <int THREADS, int ITEMS, int CAP, int MIN_BLOCKS, bool TRACE, bool LOCAL>
+template <int THREADS, int ITEMS, int CAP, int MIN_BLOCKS, bool TRACE, bool LOCAL, bool GRAPH>
 __global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
 k_collide(CollideParams P)
 {
@@ -960,7 +965,7 @@ k_collide(CollideParams P)
         item = s_item[(it + 1) & 1];
         uint4 nxt = make_uint4(0u, 0u, 0u, 0u);
         if (item < nlist) nxt = P.list[item];   // first used after the staging barrier
-        collide_cell_smem<THREADS, ITEMS, G, TRACE, LOCAL>(P, cur.x, cur.y, cur.z, sp0, sp1, sp2, sE, spid, spark, sbkt, sord,
+        collide_cell_smem<THREADS, ITEMS, G, TRACE, LOCAL, GRAPH>(P, cur.x, cur.y, cur.z, sp0, sp1, sp2, sE, spid, spark, sbkt, sord,
                                                     s_warp, &s_stats, s_seg, s_esum, acc, nxt.y, nxt.z);
         __syncthreads();
         cur = nxt;
@@ -972,6 +977,10 @@ k_collide(CollideParams P)
         if (s_stats.near) atomicAdd(&P.counters[3], (unsigned long long)s_stats.near);
     }
 }
+
+// step index in device memory for graph replays
+__global__ void k_set_t(uint32_t *t_dev, uint32_t v) { *t_dev = v; }
+__global__ void k_bump_t(uint32_t *t_dev) { *t_dev += 1u; }
 
 constexpr size_t collide_smem_bytes(int cap) { return (size_t)cap * 46 + 64; }
 

@@ -59,7 +59,7 @@ size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 struct Layout {
     size_t setB[6], pidA, pidB, cnt, count_new, cell_start, block_sum, tile_rec, carry, class_list,
-        zero, counters, flags, max_occ, obs_partial, obs_result, arena32, arenaE, rsH, total;
+        zero, counters, flags, tdev, max_occ, obs_partial, obs_result, arena32, arenaE, rsH, total;
     int64_t ntiles, nblocks_cells, rs_blocks, arena_entries;
 };
 
@@ -89,6 +89,7 @@ Layout make_layout(int64_t n, int64_t ncells)
     L.zero = take(kZeroWords * 4);
     L.counters = take(8 * 8);
     L.flags = take(4);
+    L.tdev = take(4);
     L.max_occ = take(8);
     constexpr size_t obs_words = (4 + kObsMaxSlabs) > kLrfComp * kLrfMaxSlabs ? (4 + kObsMaxSlabs) : kLrfComp * kLrfMaxSlabs;
     constexpr size_t res_words = (4 + kObsMaxSlabs) > 9 * kLrfMaxSlabs ? (4 + kObsMaxSlabs) : 9 * kLrfMaxSlabs;
@@ -123,6 +124,11 @@ struct cuba_ctx {
     uint32_t nmax_cur = 0;   // population of the fullest cell of the current store (variable time step, A23)
     bool nmax_valid = false; // false after steps that did not read it back
     uint32_t *h_u32 = nullptr;   // pinned word for that read-back
+    bool use_graph = true;   // CUBA_OPT_GRAPH
+    bool capturing = false;  // launches go into a stream capture: GRAPH kernel instantiations, no profiling marks
+    cudaGraphExec_t graph_exec = nullptr;   // two steps (the store alternates between its two copies) for (graph_dt, graph_sigma)
+    double graph_dt = 0.0, graph_sigma = -1.0;
+    uint64_t graph_kernels = 0;             // kernel launches one replay stands for (cuba_launch_count)
     bool fuse_hist = true;   // CUBA_OPT_FUSE_HIST
     double pre_dt = 0.0;     // > 0: cnt / carry already hold the histogram of the next step for this dt
     int prof_mode = 0;   // 0 off, 1 events per kernel (collision classes as one concurrent group), 2 classes serialised
@@ -195,7 +201,7 @@ static_assert(G_COLLIDE0 + kNumClasses == CUBA_PROFILE_GROUPS, "profile groups")
 
 static void prof_mark(cuba_ctx *ctx, int group)
 {
-    if (!ctx->prof_on) return;
+    if (!ctx->prof_on || ctx->capturing) return;
     cudaEvent_t e;
     if (ctx->prof_pool.empty()) { if (cudaEventCreate(&e) != cudaSuccess) return; }
     else { e = ctx->prof_pool.back(); ctx->prof_pool.pop_back(); }
@@ -275,9 +281,10 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
     }
 
 #define CUBA_OCC(K, T, I, C, MB)                                                                                          \
-    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, true, false>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]); \
-    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, false, true>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]); \
-    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, false, false>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]);
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, true, false, false>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]); \
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, false, true, false>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]); \
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, false, false, true>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]); \
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, false, false, false>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]);
     rc = CUBA_OK;
     CUBA_FOR_EACH_CLASS(CUBA_OCC)
 #undef CUBA_OCC
@@ -347,6 +354,7 @@ void cuba_destroy(cuba_ctx *ctx)
 {
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
+    if (ctx->graph_exec) cudaGraphExecDestroy(ctx->graph_exec);
     if (ctx->h_obs) cudaFreeHost(ctx->h_obs);
     if (ctx->h_u32) cudaFreeHost(ctx->h_u32);
     for (int k = 0; k < kNumClasses; ++k) {
@@ -376,6 +384,7 @@ static int launch_collide(cuba_ctx *ctx, double base, const TraceDev *td, double
     P.seed = ctx->seed; P.t = ctx->t; P.base = base;
     P.next_dt = next_dt; P.g = ctx->g;
     P.etas = etas; P.dt = dt;
+    P.t_dev = ctx->capturing ? ctx->at<uint32_t>(lay.tdev) : nullptr;
     P.x = cur.x; P.y = cur.y; P.z = cur.z;
     P.cnt = ctx->at<uint32_t>(lay.cnt); P.carry = ctx->at<uint32_t>(lay.carry);
     if (next_dt > 0.0) {      // the scatter of this step has consumed the offsets; empty cells must read as zero
@@ -409,8 +418,9 @@ static int launch_collide(cuba_ctx *ctx, double base, const TraceDev *td, double
         cudaStream_t st = serial ? main : ctx->cls_stream[K];                                    \
         if (!serial) CU(cudaStreamWaitEvent(st, ctx->ev_fork, 0));                               \
         cls(K);                                                                                  \
-        if (!TRACE && etas > 0.0) k_collide<T, I, C, MB, false, true><<<ctx->grid_cls[K], T, collide_smem_bytes(C), st>>>(P); \
-        else k_collide<T, I, C, MB, TRACE, false><<<ctx->grid_cls[K], T, collide_smem_bytes(C), st>>>(P);    \
+        if (!TRACE && ctx->capturing) k_collide<T, I, C, MB, false, false, true><<<ctx->grid_cls[K], T, collide_smem_bytes(C), st>>>(P); \
+        else if (!TRACE && etas > 0.0) k_collide<T, I, C, MB, false, true, false><<<ctx->grid_cls[K], T, collide_smem_bytes(C), st>>>(P); \
+        else k_collide<T, I, C, MB, TRACE, false, false><<<ctx->grid_cls[K], T, collide_smem_bytes(C), st>>>(P);    \
         LAUNCHED();                                                                              \
         if (serial) prof_mark(ctx, G_COLLIDE0 + K);                                              \
         else { CU(cudaEventRecord(ctx->ev_join[K], st)); CU(cudaStreamWaitEvent(main, ctx->ev_join[K], 0)); } \
@@ -505,6 +515,64 @@ static int enqueue_bin(cuba_ctx *ctx, double dt, uint32_t *cell_of_pid)
 }
 
 // fixed time step; etas > 0 selects the local cross section (sigma is then unused)
+// one step by plain launches (also what a stream capture records)
+static int step_once(cuba_ctx *ctx, double dt, double base, double etas)
+{
+    int rc = enqueue_bin(ctx, dt, nullptr);
+    if (rc != CUBA_OK) return rc;
+    const double next_dt = ctx->fuse_hist ? dt : 0.0;
+    rc = launch_collide<false>(ctx, base, nullptr, next_dt, etas, dt);
+    if (rc != CUBA_OK) return rc;
+    ctx->pre_dt = next_dt;
+    return CUBA_OK;
+}
+
+static void graph_drop(cuba_ctx *ctx)
+{
+    if (ctx->graph_exec) cudaGraphExecDestroy(ctx->graph_exec);
+    ctx->graph_exec = nullptr;
+    ctx->graph_sigma = -1.0;
+}
+
+// Small problems are bound by the host cost of the ~13 launches and the stream fork/join of a
+// step, not by device time (78 us per step at 13.8k particles).  In the steady state of the fused
+// schedule two consecutive steps differ only in which copy of the store is read and in the step
+// index, so TWO steps are captured once into a CUDA graph (step index read from device memory and
+// bumped by a one-thread kernel after each step) and replayed.
+constexpr int64_t kGraphMaxParticles = 1 << 20;
+
+static int graph_capture(cuba_ctx *ctx, double dt, double sigma, double base)
+{
+    graph_drop(ctx);
+    const int cur0 = ctx->cur;
+    const double pre0 = ctx->pre_dt;
+    const uint64_t l0 = g_launches.load();
+    cudaGraph_t graph = nullptr;
+    uint32_t *t_dev = ctx->at<uint32_t>(ctx->lay.tdev);
+    CU(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+    ctx->capturing = true;
+    int rc = CUBA_OK;
+    for (int k = 0; k < 2 && rc == CUBA_OK; ++k) {
+        rc = step_once(ctx, dt, base, 0.0);
+        if (rc == CUBA_OK) { k_bump_t<<<1, 1, 0, ctx->stream>>>(t_dev); g_launches.fetch_add(1, std::memory_order_relaxed); }
+    }
+    ctx->capturing = false;
+    const cudaError_t e = cudaStreamEndCapture(ctx->stream, &graph);
+    ctx->graph_kernels = g_launches.load() - l0;
+    g_launches.store(l0);                       // nothing has run yet
+    ctx->cur = cur0; ctx->pre_dt = pre0;        // two steps bring both back to where they were
+    if (rc != CUBA_OK || !cuda_ok(e, "cudaStreamEndCapture")) {
+        if (graph) cudaGraphDestroy(graph);
+        return rc != CUBA_OK ? rc : CUBA_ERR_CUDA;
+    }
+    const bool ok = cuda_ok(cudaGraphInstantiate(&ctx->graph_exec, graph, 0), "cudaGraphInstantiate");
+    cudaGraphDestroy(graph);
+    if (!ok) { ctx->graph_exec = nullptr; return CUBA_ERR_CUDA; }
+    ctx->graph_dt = dt; ctx->graph_sigma = sigma;
+    return CUBA_OK;
+}
+
+// fixed time step; etas > 0 selects the local cross section (sigma is then unused)
 static int step_fixed(cuba_ctx *ctx, int nsteps, double dt, double sigma, double etas)
 {
     if (!ctx) return CUBA_ERR_NULL;
@@ -512,17 +580,35 @@ static int step_fixed(cuba_ctx *ctx, int nsteps, double dt, double sigma, double
     double base;
     int rc = check_step_args(ctx, dt, sigma, &base);
     if (rc != CUBA_OK) return rc;
-    for (int s = 0; s < nsteps; ++s) {
-        rc = enqueue_bin(ctx, dt, nullptr);
-        if (rc != CUBA_OK) return rc;
-        const double next_dt = ctx->fuse_hist ? dt : 0.0;
-        rc = launch_collide<false>(ctx, base, nullptr, next_dt, etas, dt);
-        if (rc != CUBA_OK) return rc;
-        ctx->pre_dt = next_dt;
-        ctx->t += 1;
-        ctx->steps += 1;
-        ctx->nmax_valid = false;
+    int s = 0;
+    auto plain = [&]() -> int {
+        const int r = step_once(ctx, dt, base, etas);
+        if (r != CUBA_OK) return r;
+        ctx->t += 1; ctx->steps += 1; ctx->nmax_valid = false; ++s;
+        return CUBA_OK;
+    };
+    // the legacy default stream (0, cudaStreamLegacy) and cudaStreamPerThread cannot be captured
+    const bool graphable = ctx->use_graph && ctx->fuse_hist && !ctx->prof_on && etas == 0.0 && ctx->n <= kGraphMaxParticles &&
+                           reinterpret_cast<uintptr_t>(ctx->stream) > 2;
+    if (graphable && nsteps >= 4) {
+        // reach the steady state the graph was captured in: histogram prepared for this dt, store in copy 0
+        while (s < nsteps && !(ctx->pre_dt == dt && ctx->cur == 0)) { rc = plain(); if (rc != CUBA_OK) return rc; }
+        if (nsteps - s >= 2) {
+            if (!ctx->graph_exec || ctx->graph_dt != dt || ctx->graph_sigma != sigma) {
+                rc = graph_capture(ctx, dt, sigma, base);
+                if (rc != CUBA_OK) return rc;
+            }
+            k_set_t<<<1, 1, 0, ctx->stream>>>(ctx->at<uint32_t>(ctx->lay.tdev), ctx->t);
+            LAUNCHED();
+            for (; nsteps - s >= 2; s += 2) {
+                CU(cudaGraphLaunch(ctx->graph_exec, ctx->stream));
+                g_launches.fetch_add(ctx->graph_kernels, std::memory_order_relaxed);
+                ctx->t += 2; ctx->steps += 2;
+            }
+            ctx->nmax_valid = false;
+        }
     }
+    while (s < nsteps) { rc = plain(); if (rc != CUBA_OK) return rc; }
     return CUBA_OK;
 }
 
@@ -667,7 +753,8 @@ int cuba_step_traced(cuba_ctx *ctx, double dt, double sigma, cuba_trace *out)
 int cuba_set_option(cuba_ctx *ctx, int option, int value)
 {
     if (!ctx) return CUBA_ERR_NULL;
-    if (option != CUBA_OPT_FUSE_HIST || (value != 0 && value != 1)) return CUBA_ERR_VALUE;
+    if ((option != CUBA_OPT_FUSE_HIST && option != CUBA_OPT_GRAPH) || (value != 0 && value != 1)) return CUBA_ERR_VALUE;
+    if (option == CUBA_OPT_GRAPH) { ctx->use_graph = value != 0; return CUBA_OK; }
     ctx->fuse_hist = value != 0;
     if (!ctx->fuse_hist) ctx->pre_dt = 0.0;
     return CUBA_OK;

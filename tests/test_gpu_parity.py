@@ -165,6 +165,44 @@ def test_lrf_observables_match_oracle(cuba, oracle_mod):
             g.observables_lrf(bad)
 
 
+def test_cuda_graph_replay_is_bit_identical(cuba, oracle_mod):
+    """CUBA_OPT_GRAPH: on a capturable stream, small problems replay a two-step CUDA graph (step
+    index in device memory).  Same bits as plain launches and as the oracle: even and odd step
+    counts, a start from either copy of the store, a change of dt (re-capture), single steps in
+    between, and the launch counter keeps counting the kernels a replay stands for."""
+    import torch
+    w = workloads.riemann(L=(6.0, 3.0, 2.0), ncell=(12, 3, 2), r_test=90.0, sigma_gev2=50.0, dt=0.05, seed=23)
+    st = torch.cuda.Stream()
+    graph = cuba.Cuba.from_workload(w, stream=st)
+    plain = cuba.Cuba.from_workload(w, stream=torch.cuda.Stream())
+    plain.set_option(2, 0)
+    o = oracle_mod.Oracle.from_workload(w)
+    l0 = cuba.launch_count()
+    graph.step(8, w.dt, w.sigma)
+    lg = cuba.launch_count() - l0
+    l0 = cuba.launch_count()
+    plain.step(8, w.dt, w.sigma)
+    lp = cuba.launch_count() - l0
+    assert lp - 8 <= lg <= lp + 8                        # + k_set_t / k_bump_t, - nothing hidden
+    o.step(8, w.dt, w.sigma)
+    for k, dt in ((7, w.dt), (1, w.dt), (5, 0.5 * w.dt), (6, 0.5 * w.dt), (3, w.dt), (9, w.dt)):
+        graph.step(k, dt, w.sigma)
+        plain.step(k, dt, w.sigma)
+        o.step(k, dt, w.sigma)
+        for a, b, c in zip(graph.particles(), plain.particles(), o.particles()):
+            assert np.array_equal(a, b) and np.array_equal(a, c)
+    cg, co = graph.counters(), o.counters()
+    assert (cg.steps, cg.pairs, cg.collisions, cg.rounds) == (39, co["pairs"], co["collisions"], co["rounds"])
+    assert cg.device_flags == 0
+    # configs[0], the PR1 reference config, through the graph: 50 steps in one call
+    w0 = workloads.make(0)
+    g0 = cuba.Cuba.from_workload(w0, stream=st)
+    o0 = oracle_mod.Oracle.from_workload(w0)
+    g0.step(w0.steps, w0.dt, w0.sigma)
+    o0.step(w0.steps, w0.dt, w0.sigma)
+    assert_state_equal(g0.particles(), o0.particles())
+
+
 def test_local_cross_section_matches_oracle(cuba, oracle_mod):
     """sigma per cell from the cell's n and <E> for constant eta/s.  The
     per-cell factor comes from an order-free fixed-point energy sum, so rounds, decisions and the
