@@ -59,7 +59,7 @@ size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 struct Layout {
     size_t setB[6], pidA, pidB, cnt, count_new, cell_start, block_sum, tile_rec, carry, class_list,
-        zero, counters, flags, tdev, max_occ, obs_partial, obs_result, arena32, arenaE, rsH, total;
+        zero, counters, flags, tdev, max_occ, obs_partial, obs_result, arena32, arenaE, rsH, rsSums, total;
     int64_t ntiles, nblocks_cells, rs_blocks, arena_entries;
 };
 
@@ -98,6 +98,7 @@ Layout make_layout(int64_t n, int64_t ncells)
     L.arena32 = take((size_t)L.arena_entries * 16);   // also the init sort's key/value double buffers
     L.arenaE = take((size_t)L.arena_entries * 8);
     L.rsH = take((size_t)256 * L.rs_blocks * 4);
+    L.rsSums = take(((size_t)256 * L.rs_blocks / kScanChunk + 2) * 4);
     L.total = o;
     return L;
 }
@@ -319,8 +320,17 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
         for (int p = 0; p < passes; ++p) {
             k_rs_hist<<<nb, kRsThreads, 0, st>>>(keys[src], n, 8 * p, nb, H);
             LAUNCHED();
-            k_scan_blocks<<<1, 1024, 0, st>>>(H, (int)(256 * nb), nullptr, 0);
-            LAUNCHED();
+            {
+                const int64_t total = (int64_t)256 * nb;
+                const unsigned nchunks = (unsigned)((total + kScanChunk - 1) / kScanChunk);
+                uint32_t *sums = ctx->at<uint32_t>(lay.rsSums);
+                k_chunk_sums<<<nchunks, kScanThreads, 0, st>>>(H, total, sums);
+                LAUNCHED();
+                k_scan_blocks<<<1, 1024, 0, st>>>(sums, (int)nchunks, nullptr, 0);
+                LAUNCHED();
+                k_chunk_scan<<<nchunks, kScanThreads, 0, st>>>(H, total, sums);
+                LAUNCHED();
+            }
             k_rs_scatter<<<nb, kRsThreads, 0, st>>>(keys[src], vals[src], keys[1 - src], vals[1 - src], n, 8 * p, nb, H);
             LAUNCHED();
             src = 1 - src;

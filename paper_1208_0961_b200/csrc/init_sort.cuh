@@ -44,6 +44,69 @@ k_rs_hist(const uint32_t *__restrict__ keys, int64_t n, int shift, uint32_t nblo
     H[(size_t)threadIdx.x * nblocks + blockIdx.x] = s_h[threadIdx.x];
 }
 
+// Exclusive scan of the digit-major histogram table H (256 * nblocks entries, millions for tens
+// of millions of particles) in three launches: per-chunk sums, a one-CTA scan of those sums
+// (k_scan_blocks), and a per-chunk scan on top of its offset.
+constexpr int kScanThreads = 1024;
+constexpr int kScanItems = 4;
+constexpr int kScanChunk = kScanThreads * kScanItems;
+
+__global__ void __launch_bounds__(kScanThreads)
+k_chunk_sums(const uint32_t *__restrict__ H, int64_t total, uint32_t *__restrict__ sums)
+{
+    __shared__ uint32_t s_warp[32];
+    const int64_t base = (int64_t)blockIdx.x * kScanChunk + (int64_t)threadIdx.x * kScanItems;
+    uint32_t v = 0;
+#pragma unroll
+    for (int q = 0; q < kScanItems; ++q) v += (base + q < total) ? H[base + q] : 0u;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+    if ((threadIdx.x & 31) == 0) s_warp[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        uint32_t w = s_warp[threadIdx.x];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xFFFFFFFFu, w, o);
+        if (threadIdx.x == 0) sums[blockIdx.x] = w;
+    }
+}
+
+__global__ void __launch_bounds__(kScanThreads)
+k_chunk_scan(uint32_t *__restrict__ H, int64_t total, const uint32_t *__restrict__ chunk_prefix)
+{
+    __shared__ uint32_t s_warp[32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int64_t base = (int64_t)blockIdx.x * kScanChunk + (int64_t)threadIdx.x * kScanItems;
+    uint32_t v[kScanItems], sum = 0;
+#pragma unroll
+    for (int q = 0; q < kScanItems; ++q) { v[q] = (base + q < total) ? H[base + q] : 0u; sum += v[q]; }
+    uint32_t inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) s_warp[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        const uint32_t w = s_warp[lane];
+        uint32_t winc = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, winc, o);
+            if (lane >= o) winc += t;
+        }
+        s_warp[lane] = winc - w;
+    }
+    __syncthreads();
+    uint32_t run = chunk_prefix[blockIdx.x] + s_warp[wid] + inc - sum;
+#pragma unroll
+    for (int q = 0; q < kScanItems; ++q) {
+        if (base + q < total) H[base + q] = run;
+        run += v[q];
+    }
+}
+
 // stable scatter: order inside a block is (warp, row, lane) = ascending input index
 __global__ void __launch_bounds__(kRsThreads)
 k_rs_scatter(const uint32_t *__restrict__ keys, const uint32_t *__restrict__ vals,
