@@ -377,6 +377,65 @@ def test_stress_geometries_match_oracle(cuba, oracle_mod, case):
             assert oc["collisions"] > 100
 
 
+@pytest.mark.parametrize("seed", range(16))
+def test_random_configurations_match_oracle(cuba, oracle_mod, seed):
+    """Seeded fuzz over the parameter space: box shape, grid, density, cross section (from no
+    collisions to several rounds), dt up to the CFL limit, step mix (fixed / traced / adaptive /
+    local cross section), schedule options, capturable or default stream.  State, cell table and
+    counters must be the oracle's bit for bit after every call."""
+    import torch
+    rng = np.random.default_rng(1000 + seed)
+    ncell = tuple(int(v) for v in rng.integers(1, 9, 3))
+    d = rng.uniform(0.3, 1.5, 3)
+    L = tuple(float(a * b) for a, b in zip(ncell, d))
+    ncells = ncell[0] * ncell[1] * ncell[2]
+    per_cell = float(rng.choice([0.3, 3.0, 30.0, 300.0]))
+    count = int(min(60000, max(2, per_cell * ncells)))
+    dmin = float(d.min())
+    dt = float(rng.uniform(0.05, 0.98)) * dmin
+    V = float(np.prod(d))
+    target = float(rng.choice([0.0, 0.2, 0.9, 2.5, 6.0]))              # 2 cn base in a typical cell
+    mean_n = max(count / ncells, 2.0)
+    sigma_fm2 = 0.389379
+    r_test = max(2.0 * mean_n * sigma_fm2 * dt / V / target, 1e-3) if target > 0 else 1.0
+    w = workloads.thermal_box(L=L, ncell=ncell, count=count, seed=500 + seed, r_test=r_test,
+                              sigma_gev2=(10.0 if target > 0 else 0.0), dt=dt, T=float(rng.uniform(0.1, 0.6)))
+    stream = torch.cuda.Stream() if seed % 2 else None
+    g = cuba.Cuba.from_workload(w, stream=stream)
+    g.set_option(1, int(rng.integers(0, 2)))
+    g.set_option(2, int(rng.integers(0, 2)))
+    o = oracle_mod.Oracle.from_workload(w)
+
+    def check():
+        assert_state_equal(g.particles(), o.particles())
+        assert np.array_equal(g.cell_start(), o.cells()[1])
+        gc, oc = g.counters(), o.counters()
+        assert (gc.steps, gc.pairs, gc.collisions, gc.rounds) == (oc["steps"], oc["pairs"], oc["collisions"], oc["rounds"])
+        assert gc.device_flags == 0
+
+    check()
+    for _ in range(5):
+        kind = rng.choice(["fixed", "fixed", "traced", "adaptive", "local", "halfdt"])
+        k = int(rng.integers(1, 8))
+        if kind == "fixed":
+            g.step(k, w.dt, w.sigma); o.step(k, w.dt, w.sigma)
+        elif kind == "halfdt":
+            g.step(k, 0.5 * w.dt, w.sigma); o.step(k, 0.5 * w.dt, w.sigma)
+        elif kind == "traced":
+            g.step_traced(w.dt, w.sigma); o.step(1, w.dt, w.sigma)
+        elif kind == "adaptive":
+            ug, eg = g.step_adaptive(k, w.dt, w.sigma)
+            uo, eo = o.step_adaptive(k, w.dt, w.sigma)
+            assert np.array_equal(ug, uo) and eg == eo
+        else:
+            etas = float(rng.uniform(0.05, 1.0)) * max(1.0, 40.0 / mean_n)   # keeps the rounds below the cap of 64
+            g.step_local_sigma(k, w.dt, etas); o.step_etas(k, w.dt, etas)
+        check()
+    gt, ge = g.observables(7)
+    ot, oe = o.observables(7)
+    assert np.allclose(ge, oe, rtol=REL, atol=0) and gt[0] == pytest.approx(ot[0], rel=REL)
+
+
 def test_config1_full_run_profiles_match_oracle(cuba, oracle_mod):
     """Protocol (ii) of SURVEY 8(c) at BASELINE.json:configs[1] itself: 2.49M testparticles, 100
     steps, 64-slab energy-density profiles every 10 steps.  Under the arithmetic contract A2 the
