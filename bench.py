@@ -355,7 +355,7 @@ def main():
                                    % e2e["steps"], "seconds": e2e["s"]}
         if not args.no_cpu_baseline:
             ow, sample = oracle_sample_workload(args.config)
-            osteps = max(2, min(10, int(12e6 // max(ow.n, 1)) + 1))
+            osteps = max(2, min(60, int(60e6 // max(ow.n, 1)) + 1))   # about 10-30 s of one host core
             odt, oc = time_oracle(ow, osteps, 0)
             line["cpu_baseline"] = {"value": ow.n * osteps / odt, "unit": UNIT, "cores": 1, "kind": "oracle",
                                     "sample": "%s, N=%d, %d steps, %.1f s" % (sample, ow.n, osteps, odt),
