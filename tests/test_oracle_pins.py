@@ -338,12 +338,75 @@ def test_pairings_are_uniform_over_perfect_matchings(oracle_mod, n, count):
     hist = {}
     trials = 6000
     for t in range(trials):
-        order = oracle_mod.shuffle_order(1234, t, t % 3, pids)
+        order = oracle_mod.shuffle_order(1234, t, t % 8, pids)   # all four words of both Philox calls
         assert sorted(order) == sorted(pids)
         hist[matching_id(order)] = hist.get(matching_id(order), 0) + 1
     assert len(hist) == count
     chi2 = sum((v - trials / count) ** 2 / (trials / count) for v in hist.values())
     assert stats.chi2.sf(chi2, count - 1) > 1e-3
+
+
+
+def _keys_from_philox(oracle_mod, seed, t, rho, pids):
+    """A7 assembled in the test from the cuRAND-pinned Philox routine: key = word (rho mod 4) of the
+    call with counter {pid, t, rho div 4, SHUF << 16 | 0}, key {seed lo, seed hi}; << 32 | pid."""
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    out = []
+    for pid in pids:
+        w = oracle_mod.philox4x32_10([int(pid), t, rho >> 2, 0], key)
+        out.append((int(w[rho & 3]) << 32) | int(pid))
+    return out
+
+
+def test_shuffle_key_is_word_rho_mod_4_of_call_rho_div_4(oracle_mod):
+    """A7 for every round of two Philox calls (rho = 0..7) and beyond: the order is the argsort of
+    keys assembled here; the eight orders differ pairwise (a dropped `>> 2` would repeat rounds
+    0-3 in 4-7, a dropped `& 3` would read the wrong word)."""
+    pids = np.array([5, 900001, 17, 3, 250, 9, 1000003, 42, 77, 123456, 31, 64, 65, 66, 4000000000], dtype=np.uint32)
+    seed, t = (0x9ABCDEF0 << 32) | 0x12345678, 11
+    orders = []
+    for rho in list(range(8)) + [8, 13, 63]:
+        keys = _keys_from_philox(oracle_mod, seed, t, rho, pids)
+        expect = pids[np.argsort(np.array(keys, dtype=np.uint64), kind="stable")]
+        got = oracle_mod.shuffle_order(seed, t, rho, pids)
+        assert np.array_equal(got, expect), rho
+        orders.append(tuple(int(v) for v in got))
+    assert len(set(orders)) == len(orders)
+
+
+def test_step_pairs_follow_the_key_layout_in_every_round(oracle_mod):
+    """The same pin on the step itself (collide_cell, not the stand-alone shuffle): a dense
+    single-layer box that needs R = 7 rounds; in every round the traced (pid_a, pid_b) list of a
+    cell is its pids ordered by the keys assembled in the test from Philox, paired 2k with 2k+1."""
+    n_per_cell, A = 23, 3
+    arrs = one_cell_ensemble(n_per_cell, A, seed=7)
+    dt, r, seed = 1e-9, 2.0, 0xDEADBEEF12345
+    base = 6.5 / (2.0 * n_per_cell)          # pmax = 6.5 -> R = 7 (uses words 0-3 of call 0, 0-2 of call 1)
+    sigma = base * r / dt
+    o = oracle_mod.Oracle([A, A, A], [A, A, A], *arrs, r, seed)
+    o.set_trace(True)
+    o.step(2, dt, sigma)                     # the traced step is the second one: t = 1
+    tr = o.trace()
+    assert int(tr["round"].max()) == 6 and o.counters()["rounds"] == 2 * 7 * A ** 3
+    cell, start = o.cells()
+    pid = o.particles()[0]
+    seen = set()
+    for c in range(A ** 3):
+        ids = pid[start[c]:start[c + 1]]
+        for rho in range(7):
+            keys = _keys_from_philox(oracle_mod, seed, 1, rho, ids)
+            order = ids[np.argsort(np.array(keys, dtype=np.uint64), kind="stable")]
+            m = (tr["cell"] == c) & (tr["round"] == rho)
+            assert np.array_equal(tr["pid_a"][m], order[0:2 * (n_per_cell // 2):2]), (c, rho)
+            assert np.array_equal(tr["pid_b"][m], order[1:2 * (n_per_cell // 2):2]), (c, rho)
+            if c == 0:
+                seen.add(tuple(int(v) for v in order))
+    assert len(seen) == 7                    # no round repeats another round's pairing
+    # the decision uniform of round rho is keyed by rho itself (not rho div 4): A20
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    for i in np.random.default_rng(3).integers(0, tr["u"].size, 40):
+        w = oracle_mod.philox4x32_10([int(tr["pid_a"][i]), 1, int(tr["round"][i]), 1 << 16], key)
+        assert tr["u"][i] == oracle_mod.u53(w[0], w[1])
 
 
 def test_shuffle_does_not_depend_on_arrival_order(oracle_mod):
@@ -429,7 +492,7 @@ def one_cell_ensemble(n_per_cell, ncell_axis, seed):
 
 
 @pytest.mark.parametrize("n_per_cell,target_pmax", [(2, 0.5), (3, 0.6), (4, 0.6), (5, 0.8), (27, 0.9),
-                                                     (40, 2.6), (41, 3.3)])
+                                                     (40, 2.6), (41, 3.3), (26, 5.4), (31, 7.7)])
 def test_collision_rate_matches_all_pairs_expectation(oracle_mod, n_per_cell, target_pmax):
     """north_star: rate = n^2 <v_rel> sigma / (2 N_test).  Exactly: sum over all n(n-1)/2 pairs of
     Eq. 3 with <v_rel> = 1 for an isotropic massless gas, i.e. n(n-1)/2 * base per cell per step,
