@@ -85,6 +85,9 @@ def lib():
         L.oracle_dirlog_len.restype = c_int64
         L.oracle_dirlog_copy.argtypes = [c_void_p, dp]
         L.oracle_shuffle_order.argtypes = [c_uint64, c_uint32, c_uint32, c_int64, u32p, u32p]
+        L.oracle_collide_cells.argtypes = [c_uint64, c_uint32, c_double, c_int64, POINTER(c_int64), POINTER(c_int64),
+                                           u32p, u32p, dp, dp, dp, POINTER(c_uint64)]
+        L.oracle_collide_cells.restype = c_int
         _lib = L
     return _lib
 
@@ -187,6 +190,24 @@ def shuffle_order(seed, t, rho, pids):
     out = np.zeros_like(pids)
     lib().oracle_shuffle_order(int(seed), int(t), int(rho), pids.shape[0], _u32p(pids), _u32p(out))
     return out
+
+
+def collide_cells(seed, t, base, lo, hi, pid, px, py, pz, cell_id=None):
+    """S5 of the oracle on the cells [lo[k], hi[k]) of a cell-sorted state (copies are collided);
+    returns (px, py, pz, dict(pairs, collisions, rounds))."""
+    lo = np.ascontiguousarray(lo, dtype=np.int64)
+    hi = np.ascontiguousarray(hi, dtype=np.int64)
+    pid = np.ascontiguousarray(pid, dtype=np.uint32)
+    p = [_f64(a).copy() for a in (px, py, pz)]
+    cid = None if cell_id is None else np.ascontiguousarray(cell_id, dtype=np.uint32)
+    cnt = np.zeros(3, dtype=np.uint64)
+    i64p = POINTER(c_int64)
+    rc = lib().oracle_collide_cells(int(seed), int(t), float(base), lo.shape[0], lo.ctypes.data_as(i64p),
+                                    hi.ctypes.data_as(i64p), None if cid is None else _u32p(cid), _u32p(pid),
+                                    _dp(p[0]), _dp(p[1]), _dp(p[2]), cnt.ctypes.data_as(POINTER(c_uint64)))
+    if rc != 0:
+        raise OracleError(rc)
+    return p[0], p[1], p[2], dict(pairs=int(cnt[0]), collisions=int(cnt[1]), rounds=int(cnt[2]))
 
 
 # ---- a run -----------------------------------------------------------------------------

@@ -458,6 +458,30 @@ static int collide_cell(oracle_state *st, uint32_t c, int64_t lo, int64_t hi, do
 }
 
 /* ------------------------------------------------------------------------------------
+ * S5 on selected cells of a caller-supplied, cell-sorted state: an entry point
+ * to collide_cell() above for parity checks at sizes where only some cells can be re-collided
+ * (tests/test_gpu_large.py).  pid/px/py/pz are whole arrays in array order; cell k of the
+ * selection holds slots [lo[k], hi[k]) and is collided in place with step index t and the Eq. 3
+ * factor `base`.  counters (may be NULL) receives {pairs, collisions, rounds}.  No arithmetic of
+ * its own.
+ * ---------------------------------------------------------------------------------- */
+int oracle_collide_cells(uint64_t seed, uint32_t t, double base, int64_t ncell_sel,
+                         const int64_t *lo, const int64_t *hi, const uint32_t *cell_id,
+                         uint32_t *pid, double *px, double *py, double *pz, uint64_t counters[3])
+{
+    oracle_state st;
+    memset(&st, 0, sizeof(st));
+    st.seed = seed; st.t = t; st.pid = pid; st.px = px; st.py = py; st.pz = pz;
+    int rc = ORC_OK;
+    for (int64_t k = 0; k < ncell_sel; ++k) {
+        int r = collide_cell(&st, cell_id ? cell_id[k] : (uint32_t)k, lo[k], hi[k], base);
+        if (r != ORC_OK) rc = r;
+    }
+    if (counters) { counters[0] = st.pairs; counters[1] = st.collisions; counters[2] = st.rounds; }
+    return rc;
+}
+
+/* ------------------------------------------------------------------------------------
  * Local ("per-cell") cross section for a constant shear viscosity to entropy density ratio
  * (Fig. 3 caption "local cross section"; the constant-eta/s runs of ref. [1],
  * PAPER.md:108; sigma_cell from the cell's n and <E>).  Reading A24

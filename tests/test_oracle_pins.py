@@ -649,3 +649,28 @@ def test_k_steps_equal_k_single_steps(oracle_mod):
         b.step(1, w.dt, w.sigma)
     for u, v in zip(a.particles(), b.particles()):
         assert np.array_equal(u, v)
+
+
+def test_collide_cells_entry_point_is_the_steps_s5(oracle_mod):
+    """oracle_collide_cells (used by the full-size GPU checks) is S5 of oracle_step: colliding every
+    cell of the streamed, binned state reproduces the step's momenta and counters bit for bit."""
+    w = workloads.riemann_small()
+    a = oracle_mod.Oracle.from_workload(w)
+    a.step(2, w.dt, w.sigma)                       # t = 2 afterwards
+    b = oracle_mod.Oracle.from_workload(w)
+    b.step(2, w.dt, w.sigma)
+    b.step(1, w.dt, 0.0)                           # S1-S4 of the third step only
+    cb = a.counters()
+    a.step(1, w.dt, w.sigma)
+    pid, x, y, z, px, py, pz = b.particles()
+    _, start = b.cells()
+    V = float(np.prod(np.array(w.box) / np.array(w.ncell)))
+    base = (w.sigma * w.dt) / (w.n_test * V)
+    lo, hi = start[:-1].astype(np.int64), start[1:].astype(np.int64)
+    qx, qy, qz, cnt = oracle_mod.collide_cells(w.seed, 2, base, lo, hi, pid, px, py, pz)
+    ref = a.particles()
+    assert np.array_equal(ref[0], pid)
+    assert np.array_equal(qx, ref[4]) and np.array_equal(qy, ref[5]) and np.array_equal(qz, ref[6])
+    ca = a.counters()
+    assert cnt["collisions"] == ca["collisions"] - cb["collisions"] > 100
+    assert cnt["pairs"] == ca["pairs"] - cb["pairs"] and cnt["rounds"] == ca["rounds"] - cb["rounds"]
