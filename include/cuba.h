@@ -22,7 +22,9 @@
  * in Eq. 3, A3).
  *
  * Memory: every pointer is labelled DEVICE or HOST.  The caller (PyTorch in the shipped
- * binding) allocates all device memory; the library allocates none on the cuba_step path.
+ * binding) allocates all device memory; the library allocates no device memory on the cuba_step
+ * path (for problems of up to 2^20 particles the first cuba_step of a given (dt, sigma) instantiates
+ * a CUDA graph of two steps once -- a driver-side allocation; CUBA_OPT_GRAPH = 0 avoids it).
  * Errors: every call returns 0 or a negative CUBA_ERR_* code; nothing throws or aborts.
  * There is no CPU fallback: without a CUDA device every call fails with CUBA_ERR_CUDA.
  */
@@ -178,7 +180,10 @@ int cuba_get_particles(cuba_ctx *ctx, uint32_t *pid, double *x, double *y, doubl
 int cuba_get_cells(cuba_ctx *ctx, uint32_t *cell_start);
 
 /* One step with the parity trace filled (slow path: allocates temporary device memory,
- * synchronises).  The state advances exactly as with cuba_step(ctx, 1, dt, sigma). */
+ * synchronises).  The state advances exactly as with cuba_step(ctx, 1, dt, sigma) -- also when
+ * the records cannot be taken: with CUBA_ERR_TRACE (out->n_pairs then holds the capacity that
+ * was needed; cell_of_pid is filled) or after a failed temporary allocation the step is completed
+ * without records, so the context stays valid and one step further; a retry traces the NEXT step. */
 int cuba_step_traced(cuba_ctx *ctx, double dt, double sigma, cuba_trace *out);
 
 /* Counters since cuba_init.  Synchronises. */
@@ -187,7 +192,9 @@ int cuba_counters(cuba_ctx *ctx, cuba_counters_t *out);
 /* End-to-end convenience for HOST-resident data: allocates device memory, uploads the six
  * HOST arrays (n doubles each), runs cuba_init + cuba_step(nsteps) + cuba_observables,
  * optionally downloads the final state into the same HOST arrays (pid_out may be null;
- * download != 0 to copy back), frees everything.  Used for the bench's e2e number. */
+ * download != 0 to copy back), frees everything.  Device memory comes from a memory pool owned
+ * by the library (kept between calls so that a second call of the same size maps nothing new;
+ * the process-wide default pool is not touched).  Used for the bench's e2e number. */
 int cuba_run_host(const double box[3], const int ncell[3], int64_t n,
                   double *x, double *y, double *z, double *px, double *py, double *pz,
                   double n_test, uint64_t seed, int nsteps, double dt, double sigma,

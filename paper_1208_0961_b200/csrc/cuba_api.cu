@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <utility>
 #include <vector>
@@ -611,17 +612,25 @@ static int step_fixed(cuba_ctx *ctx, int nsteps, double dt, double sigma, double
         while (s < nsteps && !(ctx->pre_dt == dt && ctx->cur == 0)) { rc = plain(); if (rc != CUBA_OK) return rc; }
         if (nsteps - s >= 2) {
             if (!ctx->graph_exec || ctx->graph_dt != dt || ctx->graph_sigma != sigma) {
-                rc = graph_capture(ctx, dt, sigma, base);
-                if (rc != CUBA_OK) return rc;
+                // a stream that is already being captured by the caller cannot host a second capture
+                cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+                if (cudaStreamIsCapturing(ctx->stream, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone ||
+                    graph_capture(ctx, dt, sigma, base) != CUBA_OK) {
+                    cudaGetLastError();          // not an error of the step: fall back to plain launches for good
+                    graph_drop(ctx);
+                    ctx->use_graph = false;
+                }
             }
-            k_set_t<<<1, 1, 0, ctx->stream>>>(ctx->at<uint32_t>(ctx->lay.tdev), ctx->t);
-            LAUNCHED();
-            for (; nsteps - s >= 2; s += 2) {
-                CU(cudaGraphLaunch(ctx->graph_exec, ctx->stream));
-                g_launches.fetch_add(ctx->graph_kernels, std::memory_order_relaxed);
-                ctx->t += 2; ctx->steps += 2;
+            if (ctx->graph_exec) {
+                k_set_t<<<1, 1, 0, ctx->stream>>>(ctx->at<uint32_t>(ctx->lay.tdev), ctx->t);
+                LAUNCHED();
+                for (; nsteps - s >= 2; s += 2) {
+                    CU(cudaGraphLaunch(ctx->graph_exec, ctx->stream));
+                    g_launches.fetch_add(ctx->graph_kernels, std::memory_order_relaxed);
+                    ctx->t += 2; ctx->steps += 2;
+                }
+                ctx->nmax_valid = false;
             }
-            ctx->nmax_valid = false;
         }
     }
     while (s < nsteps) { rc = plain(); if (rc != CUBA_OK) return rc; }
@@ -673,28 +682,31 @@ int cuba_step_adaptive(cuba_ctx *ctx, int nsteps, double dt_max, double sigma, d
         rc = read_step_max(ctx);
         if (rc != CUBA_OK) return rc;
     }
+    // *elapsed is written on every return path: the time covered by the steps that completed
+    auto done = [&](int code) { if (elapsed) *elapsed = sum; return code; };
     for (int s = 0; s < nsteps; ++s) {
         const double dt = adaptive_dt(ctx, ctx->nmax_cur, dt_max, sigma);
         double base;
         rc = check_step_args(ctx, dt, sigma, &base);
-        if (rc != CUBA_OK) return rc;
+        if (rc != CUBA_OK) return done(rc);
         rc = enqueue_bin(ctx, dt, nullptr);
-        if (rc != CUBA_OK) return rc;
+        if (rc != CUBA_OK) return done(rc);
         // the fullest cell of the new binning fixes the NEXT step, whose histogram this step's
         // collision kernel prepares: one 4-byte read-back per step between scatter and collide
-        rc = read_step_max(ctx);
-        if (rc != CUBA_OK) return rc;
-        const double next_dt = ctx->fuse_hist ? adaptive_dt(ctx, ctx->nmax_cur, dt_max, sigma) : 0.0;
-        rc = launch_collide<false>(ctx, base, nullptr, next_dt);
-        if (rc != CUBA_OK) return rc;
+        const int rm = read_step_max(ctx);
+        double next_dt = (ctx->fuse_hist && rm == CUBA_OK) ? adaptive_dt(ctx, ctx->nmax_cur, dt_max, sigma) : 0.0;
+        double nbase;
+        if (next_dt > 0.0 && check_step_args(ctx, next_dt, sigma, &nbase) != CUBA_OK) next_dt = 0.0;   // the next call reports it
+        rc = launch_collide<false>(ctx, base, nullptr, next_dt);   // the store is binned: always finish the step
+        if (rc != CUBA_OK) return done(rc);
         ctx->pre_dt = next_dt;
         ctx->t += 1;
         ctx->steps += 1;
         if (dt_used) dt_used[s] = dt;
         sum = sum + dt;
+        if (rm != CUBA_OK) return done(rm);
     }
-    if (elapsed) *elapsed = sum;
-    return CUBA_OK;
+    return done(CUBA_OK);
 }
 
 int cuba_step_traced(cuba_ctx *ctx, double dt, double sigma, cuba_trace *out)
@@ -712,10 +724,15 @@ int cuba_step_traced(cuba_ctx *ctx, double dt, double sigma, cuba_trace *out)
         cudaFree(td.off); cudaFree(td.cell); cudaFree(td.round); cudaFree(td.pa); cudaFree(td.pb);
         cudaFree(td.cell_of_pid); cudaFree(td.P); cudaFree(td.u); cudaFree(td.dec);
     };
+    // After enqueue_bin the store has been streamed and re-sorted: from there on the step is always
+    // completed (untraced if the records cannot be taken), so that an error never leaves the context
+    // half-stepped -- a retry with a larger capacity would otherwise stream a second time.
+    bool binned = false, collided = false;
     auto body = [&]() -> int {
         CU(cudaMalloc(&td.cell_of_pid, (size_t)n * 4));
         int r = enqueue_bin(ctx, dt, td.cell_of_pid);
         if (r != CUBA_OK) return r;
+        binned = true;
         r = sync_and_check(ctx);
         if (r != CUBA_OK) return r;
         // per-cell record offsets: R(n) * floor(n/2), the same fp64 expressions as the kernel
@@ -743,6 +760,7 @@ int cuba_step_traced(cuba_ctx *ctx, double dt, double sigma, cuba_trace *out)
         CU(cudaMalloc(&td.pa, m * 4)); CU(cudaMalloc(&td.pb, m * 4));
         CU(cudaMalloc(&td.P, m * 8)); CU(cudaMalloc(&td.u, m * 8)); CU(cudaMalloc(&td.dec, m));
         CU(cudaMemcpy(td.off, off.data(), ((size_t)ncells + 1) * 8, cudaMemcpyHostToDevice));
+        collided = true;
         r = launch_collide<true>(ctx, base, &td, 0.0);
         if (r != CUBA_OK) return r;
         ctx->t += 1;
@@ -762,8 +780,17 @@ int cuba_step_traced(cuba_ctx *ctx, double dt, double sigma, cuba_trace *out)
         return CUBA_OK;
     };
     rc = body();
+    if (rc != CUBA_OK && binned && !collided) {
+        // finish the step without records (a short capacity, a failed allocation)
+        cudaGetLastError();
+        if (launch_collide<false>(ctx, base, nullptr, 0.0) == CUBA_OK) {
+            ctx->t += 1; ctx->steps += 1; ctx->nmax_valid = false;
+            cudaStreamSynchronize(ctx->stream);
+        }
+    }
     release();
     return rc;
+
 }
 
 int cuba_set_option(cuba_ctx *ctx, int option, int value)
@@ -919,6 +946,28 @@ int cuba_counters(cuba_ctx *ctx, cuba_counters_t *out)
     return CUBA_OK;
 }
 
+// Memory pool of cuba_run_host, one per device, created on first use and kept for the life of the
+// process (release threshold: keep everything).
+static int run_host_pool(int dev_id, cudaMemPool_t *out)
+{
+    static std::mutex mu;
+    static cudaMemPool_t pools[64] = {};
+    if (dev_id < 0 || dev_id >= 64) return CUBA_ERR_CUDA;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!pools[dev_id]) {
+        cudaMemPoolProps props{};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev_id;
+        CU(cudaMemPoolCreate(&pools[dev_id], &props));
+        uint64_t keep = UINT64_MAX;
+        CU(cudaMemPoolSetAttribute(pools[dev_id], cudaMemPoolAttrReleaseThreshold, &keep));
+    }
+    *out = pools[dev_id];
+    return CUBA_OK;
+}
+
 int cuba_run_host(const double box[3], const int ncell[3], int64_t n,
                   double *x, double *y, double *z, double *px, double *py, double *pz,
                   double n_test, uint64_t seed, int nsteps, double dt, double sigma,
@@ -934,17 +983,16 @@ int cuba_run_host(const double box[3], const int ncell[3], int64_t n,
     cudaStream_t st = nullptr;
     auto body = [&]() -> int {
         CU(cudaStreamCreate(&st));
-        // stream-ordered allocations from the device's default pool, which is told to keep what it
-        // has been given: a second call of the same size maps no new memory (cudaMalloc / cudaFree
-        // of 3.3 GB cost ~10 ms per call at 24.9M particles)
+        // stream-ordered allocations from a pool owned by the library, which keeps what it has been
+        // given: a second call of the same size maps no new memory (cudaMalloc / cudaFree of 3.3 GB
+        // cost ~10 ms per call at 24.9M particles).  The process-wide default pool is left alone.
         int dev_id = 0;
         CU(cudaGetDevice(&dev_id));
-        cudaMemPool_t pool;
-        CU(cudaDeviceGetDefaultMemPool(&pool, dev_id));
-        uint64_t keep = UINT64_MAX;
-        CU(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
-        for (int k = 0; k < 6; ++k) CU(cudaMallocAsync(reinterpret_cast<void **>(&dev[k]), (size_t)n * 8, st));
-        CU(cudaMallocAsync(&ws, wsb, st));
+        cudaMemPool_t pool = nullptr;
+        int rp = run_host_pool(dev_id, &pool);
+        if (rp != CUBA_OK) return rp;
+        for (int k = 0; k < 6; ++k) CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&dev[k]), (size_t)n * 8, pool, st));
+        CU(cudaMallocFromPoolAsync(&ws, wsb, pool, st));
         for (int k = 0; k < 6; ++k) CU(cudaMemcpyAsync(dev[k], host[k], (size_t)n * 8, cudaMemcpyHostToDevice, st));
         int r = cuba_init(&ctx, box, ncell, n, dev[0], dev[1], dev[2], dev[3], dev[4], dev[5], n_test, seed, ws, wsb, st);
         if (r != CUBA_OK) return r;

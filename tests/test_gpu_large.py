@@ -86,41 +86,58 @@ def test_full_size_step_sampled_against_oracle(cuba, oracle_mod, config):
     slot_b[pidb] = np.arange(w.n)
     hot = np.argsort(counts)[-3:]
     sample = np.concatenate([hot, rng.integers(0, ncells, 12)])
-    for c in sample:
-        lo, hi = int(starta[c]), int(starta[c + 1])
-        if hi - lo < 2:
-            continue
-        ids = pida[lo:hi]
-        before = slot_b[ids]
-        got = np.stack([sa[3][lo:hi], sa[4][lo:hi], sa[5][lo:hi]])
-        # momenta before S5 of this step = post-binning momenta reflected by this step's walls:
-        # take them from a replay of S1-S2 on the "before" state
-        (rx, ry, rz, rpx, rpy, rpz), _ = oracle_mod.stream_reflect(*[a[before] for a in sb], w.dt, w.box)
-        ref = oracle_collide_cell(oracle_mod, w, ids, np.stack([rpx, rpy, rpz]), t_index, base)
-        assert np.array_equal(got, ref), "cell %d" % c
+    sample = np.array([c for c in sample if starta[c + 1] - starta[c] >= 2])
+    # momenta before S5 of this step = S1-S2 of the oracle on the state before the step, in the new array order
+    (rx, ry, rz, rpx, rpy, rpz), _ = oracle_mod.stream_reflect(*[a[slot_b[pida]] for a in sb], w.dt, w.box)
+    lo, hi = starta[sample].astype(np.int64), starta[sample + 1].astype(np.int64)
+    qx, qy, qz, cnt = oracle_mod.collide_cells(w.seed, t_index, base, lo, hi, pida, rpx, rpy, rpz, cell_id=sample)
+    for c, l, h in zip(sample, lo, hi):
+        for name, got, ref in (("px", sa[3], qx), ("py", sa[4], qy), ("pz", sa[5], qz)):
+            assert np.array_equal(got[l:h], ref[l:h]), "cell %d %s" % (c, name)
+    assert cnt["collisions"] > 0
 
 
-def oracle_collide_cell(oracle_mod, w, ids, p, t, base):
-    """S5 of one cell done with the oracle's own pieces (shuffle_order, pair_kinematics, the
-    DEC uniform via philox + u53, direction, scatter), in the order of oracle/cuba_oracle.c."""
-    n = ids.shape[0]
-    cn = float(n if n % 2 else n - 1)
-    pmax = (2.0 * cn) * base
-    R = 1 if pmax <= 1.0 else int(math.ceil(pmax))
-    scale = (cn * base) / float(R)
-    p = p.copy()
-    index_of = {int(v): k for k, v in enumerate(ids)}
-    key = [w.seed & 0xFFFFFFFF, w.seed >> 32]
-    for rho in range(R):
-        order = oracle_mod.shuffle_order(w.seed, t, rho, ids)
-        for k in range(n // 2):
-            a, b = index_of[int(order[2 * k])], index_of[int(order[2 * k + 1])]
-            Ea, Eb, s, vrel = oracle_mod.pair_kinematics(p[:, a], p[:, b])
-            P = vrel * scale
-            wds = oracle_mod.philox4x32_10([int(ids[a]), t, rho, 1 << 16], key)
-            u = oracle_mod.u53(wds[0], wds[1])
-            if u < P:
-                nhat, _ = oracle_mod.direction(w.seed, int(ids[a]), t, rho)
-                qa, qb = oracle_mod.scatter(p[:, a], p[:, b], Ea, Eb, s, nhat)
-                p[:, a], p[:, b] = qa, qb
-    return p
+def test_config2_whole_state_against_oracle(cuba, oracle_mod):
+    """north_star's target size itself (BASELINE.json:configs[2], 24,889,326 testparticles; run
+    parameters of PAPER.md:66): one traced step from the identical state -- every cell index, all
+    ~23M pair records, probabilities, uniforms and decisions, and the whole store compared with the
+    oracle -- then three plain steps (fused schedule, the launch configuration bench.py times),
+    the whole store again, and the 64-slab energy-density profile."""
+    w = workloads.make(2)
+    g = cuba.Cuba.from_workload(w)
+    o = oracle_mod.Oracle.from_workload(w)
+
+    def same_state():
+        gp, op = g.particles(), o.particles()
+        for name, a, b in zip("pid x y z px py pz".split(), gp, op):
+            assert np.array_equal(a, b), name
+        assert np.array_equal(g.cell_start(), o.cells()[1])
+
+    same_state()                                                   # A19: init sort
+    o.set_trace(True)
+    o.step(1, w.dt, w.sigma)
+    tg = g.step_traced(w.dt, w.sigma, pair_capacity=w.n + 64)
+    to = o.trace()
+    o.set_trace(False)
+    ocell, _ = o.cells()
+    ocell_of_pid = np.empty(w.n, dtype=np.uint32)
+    ocell_of_pid[o.particles()[0]] = ocell
+    assert np.array_equal(tg.cell_of_pid, ocell_of_pid)
+    assert tg.cell.shape[0] == to["cell"].shape[0] > 20_000_000
+    for k, a in (("cell", tg.cell), ("round", tg.round), ("pid_a", tg.pid_a), ("pid_b", tg.pid_b),
+                 ("P", tg.P), ("u", tg.u), ("decided", tg.decided)):
+        assert np.array_equal(a, to[k]), k
+    assert int((np.abs(to["u"] - to["P"]) <= 1e-12).sum()) == 0    # A16: nothing to exclude
+    assert int(to["round"].max()) == 1                             # the ~1350-particle cells need two rounds
+    del tg, to
+    same_state()
+    g.step(3, w.dt, w.sigma)
+    o.step(3, w.dt, w.sigma)
+    same_state()
+    gt, ge = g.observables(64)
+    ot, oe = o.observables(64)
+    assert np.allclose(ge, oe, rtol=1e-12, atol=0) and gt[0] == pytest.approx(ot[0], rel=1e-12)
+    gc, oc = g.counters(), o.counters()
+    assert (gc.steps, gc.pairs, gc.collisions, gc.rounds, gc.near_threshold) == \
+           (4, oc["pairs"], oc["collisions"], oc["rounds"], 0)
+    assert gc.device_flags == 0 and gc.overflow_cells == 0

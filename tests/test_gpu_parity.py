@@ -90,6 +90,29 @@ def test_one_step_bit_exact_many_rounds_and_size_classes(cuba, oracle_mod):
     assert o.counters()["max_occupancy"] > 512
 
 
+@pytest.mark.parametrize("n", [128, 129, 256, 257, 512, 513, 896, 897, 1536, 1537, 2048, 2049, 4544, 4545])
+def test_one_step_bit_exact_at_every_size_class_boundary(cuba, oracle_mod, n):
+    """One cell holding exactly n particles (the capacities of the collision classes and one more,
+    up to the global-memory overflow kernel) next to a small one; three rounds (A6)."""
+    base_w = workloads.thermal_box(L=(2.0, 1.0, 1.0), ncell=(2, 1, 1), count=n + 77, seed=100 + n)
+    rng = np.random.default_rng(n)
+    pos = rng.uniform(0.3, 0.7, (3, n + 77))          # dt = 0.1 moves nobody across a face
+    pos[0, n:] += 1.0
+    r_test, dt = 2.0, 0.1
+    cn = n if n % 2 else n - 1
+    sigma = (2.5 / (2.0 * cn)) * r_test * 1.0 / dt    # pmax = 2.5 in the big cell: R = 3
+    w = workloads.Workload("class_boundary_%d" % n, (2.0, 1.0, 1.0), (2, 1, 1), r_test, sigma, dt, 1, 100 + n, 2,
+                           pos[0].copy(), pos[1].copy(), pos[2].copy(), base_w.px, base_w.py, base_w.pz)
+    g, o = run_traced_step(cuba, oracle_mod, w)
+    base = (sigma * dt) / (r_test * 1.0)
+    assert o.counters()["max_occupancy"] == n
+    assert o.counters()["rounds"] == 3 + max(1, math.ceil((2.0 * 77) * base))
+    assert g.counters().overflow_cells == (1 if n > 4544 else 0)
+    g.step(2, w.dt, w.sigma)                           # fused schedule on the same cells
+    o.step(2, w.dt, w.sigma)
+    assert_state_equal(g.particles(), o.particles())
+
+
 def test_config0_full_run_matches_oracle(cuba, oracle_mod):
     """BASELINE.json:configs[0]: 50 steps, state bit-identical, totals and profile to 1e-12."""
     w = workloads.make(0)
@@ -518,3 +541,25 @@ def test_run_host_end_to_end_matches_oracle(cuba, oracle_mod):
     assert np.allclose(ed, oe, rtol=REL, atol=0) and tot[0] == pytest.approx(ot[0], rel=REL)
     assert_state_equal((pid, *host), o.particles())
     assert cuba.launch_count() > 0
+
+
+def test_short_trace_capacity_completes_the_step(cuba, oracle_mod):
+    """cuba_step_traced with too little room reports CUBA_ERR_TRACE but still takes the step (untraced):
+    the context is never left streamed-but-not-collided, and a retry traces the next step."""
+    w = workloads.riemann_small()
+    g = cuba.Cuba.from_workload(w)
+    o = oracle_mod.Oracle.from_workload(w)
+    with pytest.raises(cuba.CubaError) as e:
+        g.step_traced(w.dt, w.sigma, pair_capacity=5)
+    assert e.value.code == -10
+    o.step(1, w.dt, w.sigma)
+    assert_state_equal(g.particles(), o.particles())
+    assert g.counters().steps == 1
+    o.set_trace(True)
+    o.step(1, w.dt, w.sigma)
+    tg = g.step_traced(w.dt, w.sigma)
+    to = o.trace()
+    assert np.array_equal(tg.pid_a, to["pid_a"]) and np.array_equal(tg.decided, to["decided"])
+    g.step(3, w.dt, w.sigma)
+    o.step(3, w.dt, w.sigma)
+    assert_state_equal(g.particles(), o.particles())
