@@ -319,24 +319,30 @@ __device__ __forceinline__ int next_direction(const Geom &g, double dt, int ix0,
     return ((unsigned)dx <= 2u && (unsigned)dy <= 2u && (unsigned)dz <= 2u) ? (dx * 9 + dy * 3 + dz) : -1;
 }
 
-// Per-cell constants of the fused histogram, written by thread 0 when the cell is set up.
+// Per-cell constants of the fused histogram, written when the cell is set up.
 struct HistCell {
     int i0[3];            // cell coordinates (x slowest)
     double i0d[3];        // the same as doubles
-    int lo_code[3];       // per-axis direction component of a particle that leaves through the lower face:
-    int hi_code[3];       //   0 / 2, or 1 where that face is a wall (elastic reflection back into the cell, A12)
+    uint32_t map[kDirs];  // raw direction code (floor of the estimated position, per axis 0/1/2) -> direction code:
+                          // a component that leaves through a wall face becomes 1 (elastic reflection back
+                          // into the cell, A12; dt < cell edge keeps the mirror image inside it)
 };
 
-__device__ __forceinline__ void hist_cell_setup(const Geom &g, uint32_t c, HistCell *h)
+__device__ __forceinline__ void hist_cell_setup(const Geom &g, uint32_t c, HistCell *h, int tid)
 {
-    h->i0[2] = (int)(c % (uint32_t)g.nc[2]);
-    h->i0[1] = (int)((c / (uint32_t)g.nc[2]) % (uint32_t)g.nc[1]);
-    h->i0[0] = (int)(c / ((uint32_t)g.nc[2] * (uint32_t)g.nc[1]));
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        h->i0d[k] = (double)h->i0[k];
-        h->lo_code[k] = h->i0[k] == 0 ? 1 : 0;
-        h->hi_code[k] = h->i0[k] == g.nc[k] - 1 ? 1 : 2;
+    const int i2 = (int)(c % (uint32_t)g.nc[2]);
+    const int i1 = (int)((c / (uint32_t)g.nc[2]) % (uint32_t)g.nc[1]);
+    const int i0 = (int)(c / ((uint32_t)g.nc[2] * (uint32_t)g.nc[1]));
+    if (tid == 0) {
+        h->i0[0] = i0; h->i0[1] = i1; h->i0[2] = i2;
+        h->i0d[0] = (double)i0; h->i0d[1] = (double)i1; h->i0d[2] = (double)i2;
+    }
+    if (tid < kDirs) {
+        int dx = tid / 9, dy = (tid / 3) % 3, dz = tid % 3;
+        if ((dx == 0 && i0 == 0) || (dx == 2 && i0 == g.nc[0] - 1)) dx = 1;
+        if ((dy == 0 && i1 == 0) || (dy == 2 && i1 == g.nc[1] - 1)) dy = 1;
+        if ((dz == 0 && i2 == 0) || (dz == 2 && i2 == g.nc[2] - 1)) dz = 1;
+        h->map[tid] = (uint32_t)(dx * 9 + dy * 3 + dz);
     }
 }
 
@@ -347,38 +353,39 @@ __device__ __forceinline__ double rcp_approx(double a)
     return r;
 }
 
-// One axis of the guarded estimate: t = position after the move in units of the cell edge,
-// relative to the cell's lower face (the cell is [0,1)).  Away from the faces (and dt < cell edge
-// means |t - 0.5| < 1.5) the direction component follows from t alone: inside -> 1; beyond the
-// upper face -> 2, beyond the lower -> 0, or 1 if that face is a wall (the reflected position lies
-// in the same cell).  Within kHistEps of a face -- or anything unexpected, NaN included -- the
-// caller redoes the particle with the exact operation order.
-constexpr double kHistEps = 1e-4;   // the estimate is good to ~1e-9; the band is generous
+// Guarded estimate of the direction code.  t = position after the move in units of the cell edge,
+// relative to the cell's lower face (the cell is [0,1); dt < cell edge means -1 < t < 2), computed
+// without the fp64 division (hardware reciprocal + one Newton step, explicit FMAs: good to ~1e-9).
+// Adding 1.5*2^32 leaves round(t*2^20) in the low word of the sum (two's complement) and a fixed high
+// word: the integer part of (t+1) is the raw component 0/1/2 and the 20 fraction bits say how close
+// the particle is to a face.  Within kHistBand/2^20 = 1.2e-4 cell edges of a face -- or for anything
+// unexpected (NaN, a high word that is not the constant's) -- the caller redoes the particle with the
+// exact operation order of S1-S3; the scatter always uses the exact arithmetic.
+constexpr double kHistMagic = 6442450944.0;        // 1.5 * 2^32
+constexpr int kHistMagicHi = 0x41F80000;           // its high word; 0x41F7FFFF just below
+constexpr uint32_t kHistOne = 1u << 20;
+constexpr uint32_t kHistBand = 128u;
 
-__device__ __forceinline__ int axis_code(double t, int lo_code, int hi_code, bool &safe)
-{
-    const double a = fabs(t - 0.5);
-    const bool inside = a < 0.5 - kHistEps;
-    const bool outside = a > 0.5 + kHistEps && a < 1.5 - kHistEps;
-    safe = safe && (inside || outside);
-    return inside ? 1 : (t > 0.5 ? hi_code : lo_code);
-}
-
-// Direction code of a particle: the same value as next_direction(), computed without the fp64
-// division (hardware reciprocal estimate + one Newton step, fused multiply-adds) wherever the
-// outcome is not within kHistEps of changing.
 __device__ __forceinline__ int next_direction_guarded(const Geom &g, double dt, const HistCell &h,
                                                       double x, double y, double z, double px, double py, double pz, double E)
 {
     double r = rcp_approx(E);
     r = __fma_rn(r, __fma_rn(-E, r, 1.0), r);
     const double w = dt * r;
-    bool safe = true;
-    const int dx = axis_code(__fma_rn(__fma_rn(px, w, x), g.inv_d[0], -h.i0d[0]), h.lo_code[0], h.hi_code[0], safe);
-    const int dy = axis_code(__fma_rn(__fma_rn(py, w, y), g.inv_d[1], -h.i0d[1]), h.lo_code[1], h.hi_code[1], safe);
-    const int dz = axis_code(__fma_rn(__fma_rn(pz, w, z), g.inv_d[2], -h.i0d[2]), h.lo_code[2], h.hi_code[2], safe);
+    const double yx = __dadd_rn(__fma_rn(__fma_rn(px, w, x), g.inv_d[0], -h.i0d[0]), kHistMagic);
+    const double yy = __dadd_rn(__fma_rn(__fma_rn(py, w, y), g.inv_d[1], -h.i0d[1]), kHistMagic);
+    const double yz = __dadd_rn(__fma_rn(__fma_rn(pz, w, z), g.inv_d[2], -h.i0d[2]), kHistMagic);
+    const uint32_t ux = (uint32_t)__double2loint(yx) + kHistOne;     // (t + 1) * 2^20 for -1 <= t < 2
+    const uint32_t uy = (uint32_t)__double2loint(yy) + kHistOne;
+    const uint32_t uz = (uint32_t)__double2loint(yz) + kHistOne;
+    const uint32_t hi = ((uint32_t)__double2hiint(yx) - (uint32_t)(kHistMagicHi - 1)) |
+                        ((uint32_t)__double2hiint(yy) - (uint32_t)(kHistMagicHi - 1)) |
+                        ((uint32_t)__double2hiint(yz) - (uint32_t)(kHistMagicHi - 1));
+    const uint32_t gx = (ux & (kHistOne - 1u)) - kHistBand, gy = (uy & (kHistOne - 1u)) - kHistBand,
+                   gz = (uz & (kHistOne - 1u)) - kHistBand;
+    const bool safe = hi <= 1u && max(ux, max(uy, uz)) < 3u * kHistOne && max(gx, max(gy, gz)) < kHistOne - 2u * kHistBand;
     if (CUBA_FORCE_SLOW_PATHS || !safe) return next_direction(g, dt, h.i0[0], h.i0[1], h.i0[2], x, y, z, px, py, pz, E);
-    return dx * 9 + dy * 3 + dz;
+    return (int)h.map[(ux >> 20) * 9u + (uy >> 20) * 3u + (uz >> 20)];
 }
 
 // Tile segments of a cell: the flat passes work on tiles of kTile consecutive slots; segment k of
@@ -388,6 +395,24 @@ __device__ __forceinline__ int next_direction_guarded(const Geom &g, double dt, 
 //   carry[tile T0+k][d]    = sum over segments before k, k >= 1         (what k_carry derives)
 //   carry[tile T0][d]      = 0 if the cell starts exactly at the tile start
 // Every tile start lies in exactly one non-empty cell, so every carry row is written once.
+// Only the particles that leave the cell are counted one by one; the count of the direction "stays"
+// (code 13) of a segment is its size minus the others (hist_fill_stay, between two barriers).
+constexpr uint32_t kDirStay = 13u;
+
+template <int THREADS>
+__device__ __forceinline__ void hist_fill_stay(uint32_t lo, uint32_t n, uint32_t *s_seg)
+{
+    const uint32_t T0 = lo / kTile, nseg = (lo + n - 1u) / kTile - T0 + 1u;
+    if (threadIdx.x < nseg) {
+        const uint32_t k = threadIdx.x;
+        const uint32_t a = max(lo, (T0 + k) * (uint32_t)kTile), b = min(lo + n, (T0 + k + 1u) * (uint32_t)kTile);
+        uint32_t others = 0;
+#pragma unroll
+        for (uint32_t d = 0; d < (uint32_t)kDirs; ++d) others += (d == kDirStay) ? 0u : s_seg[k * kDirs + d];
+        s_seg[k * kDirs + kDirStay] = (b - a) - others;
+    }
+}
+
 template <int THREADS>
 __device__ __forceinline__ void hist_publish(const CollideParams &P, uint32_t c, uint32_t lo, uint32_t n,
                                              const uint32_t *s_seg)
@@ -403,20 +428,31 @@ __device__ __forceinline__ void hist_publish(const CollideParams &P, uint32_t c,
 }
 
 // ---- shared-memory classes ------------------------------------------------------------
-// Same results as the generic routine above, organised for issue efficiency on sm_100a:
-//   * every phase works on groups of G items per thread with clamped, unguarded loads so
-//     that the G Philox / fp64 chains of a thread interleave (only stores are predicated);
-//   * 2n buckets with 16-bit counters packed two per word; the keys themselves are parked in
-//     bucket order, so an element ranks itself from five consecutive words (no indirection)
-//     and buckets with more than four elements or equal 32-bit keys take a rare slow path;
-//   * the Eq. 3 decision compares u*(EaEb)^2 with |d|^2*scale/2 (no division); only a
-//     decision inside a 4e-9 band around the threshold is redone with the exact operation
-//     order of the oracle, so the decisions (and the near-threshold counter, A16) are the
-//     oracle's bit for bit; the division for s is paid by the pairs that collide;
-//   * hits are compacted per warp, and a warp scatters its own hits right away: pairs are
-//     disjoint, so no block barrier separates decision and scatter;
-//   * the energy of an outgoing momentum is only recomputed when another round will read it.
-// Five block barriers per round.
+// Same results as the generic routine above, organised for instruction count and issue efficiency on
+// sm_100a.  The momentum-independent part of TWO consecutive rounds (the two shuffles) is done in one
+// sweep, then the two rounds' pair phases follow:
+//
+//   rank by bitmap.  The keys are uniform 32-bit numbers, so a cell of n particles gets a bitmap of
+//     M = 32 n bits (n words): bit b = floor(key * M / 2^32), monotone in the key.  Phase A: one
+//     atomicOr per element and round; an element that finds its bit already set adds one to the
+//     word's duplicate counter.  Phase B: an exclusive scan over the words of popc(word) +
+//     duplicates, both rounds packed into one 32-bit scan.  Phase C: rank = prefix of the word +
+//     popc(bits below mine) -- two loads and a popc, no parked keys, no comparisons.  The ~5 % of the
+//     elements whose word holds a duplicate ("dirty" words) put (key, word, index) on a short list
+//     in phase B and rank themselves inside the word by scanning that list, with the pid deciding
+//     between equal 32-bit keys (A7); if the list overflows (never with uniform keys; forced in the
+//     slow-paths test build) a brute-force count over recomputed keys takes over.  The result depends
+//     on keys and pids only, never on the order in which threads arrived.
+//   pair phases.  Energies are not staged: the first pair phase of a sweep computes E = |p| of both
+//     partners for its Eq. 3 decision anyway and leaves them in shared memory -- in the space of the
+//     two bitmaps, which are dead by then -- for the second round, the scatters and the fused
+//     histogram.  The decision compares u*(EaEb)^2 with |d|^2*scale/2 (no division); only a decision
+//     inside a 4e-9 band around the threshold is redone with the exact operation order of the
+//     oracle, so the decisions (and the near-threshold counter, A16) are the oracle's bit for bit.
+//     Hits are compacted per warp and a warp scatters its own hits right away (pairs are disjoint).
+//
+// Shared memory: 44 B per particle (p_x,p_y as one 16-byte element, p_z, pid, two bitmaps | E,
+// packed duplicate counters | prefixes, two 16-bit orders).  Block barriers per sweep of two rounds: 7.
 
 // 53-bit uniform from two Philox words, same value as u53(): both halves are exact integers
 // below 2^27 placed in the mantissa of 2^52, so every operation below is exact.
@@ -427,26 +463,36 @@ __device__ __forceinline__ double u53_bits(uint32_t w0, uint32_t w1)
     return (hi * 67108864.0 + lo) * (1.0 / 9007199254740992.0);
 }
 
-// Marsaglia disc rejection (A11) with the key schedule from the parameters.
+// Marsaglia disc rejection (A11) with the key schedule from the parameters.  Both attempts of the
+// first call are evaluated without a branch (95 % of the draws end there) so that a warp stays
+// converged; later calls are a rare loop.
+__device__ __forceinline__ void disc_point(uint32_t wa, uint32_t wb, double &a, double &b, double &q)
+{
+    a = ((double)wa + 0.5) * (1.0 / 2147483648.0) - 1.0;
+    b = ((double)wb + 0.5) * (1.0 / 2147483648.0) - 1.0;
+    q = a * a + b * b;
+}
+
 __device__ __forceinline__ void draw_direction_k(const CollideParams &P, uint32_t t, uint32_t pid, uint32_t rho,
                                                  double &nx, double &ny, double &nz)
 {
-    for (uint32_t call = 0; call < 65536u; ++call) {
-        const U4 w = drawk(P, t, pid, rho, kTagDir, call);
-#pragma unroll
-        for (int half = 0; half < 2; ++half) {
-            const uint32_t wa = half ? w.z : w.x, wb = half ? w.w : w.y;
-            const double a = ((double)wa + 0.5) * (1.0 / 2147483648.0) - 1.0;
-            const double b = ((double)wb + 0.5) * (1.0 / 2147483648.0) - 1.0;
-            const double q = a * a + b * b;
-            if (q < 1.0) {
-                const double h = sqrt(1.0 - q);
-                nx = (2.0 * a) * h; ny = (2.0 * b) * h; nz = 1.0 - 2.0 * q;
-                return;
-            }
+    const U4 w0 = drawk(P, t, pid, rho, kTagDir, 0);
+    double a, b, q, a2, b2, q2;
+    disc_point(w0.x, w0.y, a, b, q);
+    disc_point(w0.z, w0.w, a2, b2, q2);
+    bool ok = q < 1.0;
+    if (!ok) { a = a2; b = b2; q = q2; ok = q2 < 1.0; }
+    if (!ok) {
+        for (uint32_t call = 1; call < 65536u && !ok; ++call) {
+            const U4 w = drawk(P, t, pid, rho, kTagDir, call);
+            disc_point(w.x, w.y, a, b, q);
+            ok = q < 1.0;
+            if (!ok) { disc_point(w.z, w.w, a, b, q); ok = q < 1.0; }
         }
+        if (!ok) { nx = 0.0; ny = 0.0; nz = 1.0; return; }
     }
-    nx = 0.0; ny = 0.0; nz = 1.0;
+    const double h = sqrt(1.0 - q);
+    nx = (2.0 * a) * h; ny = (2.0 * b) * h; nz = 1.0 - 2.0 * q;
 }
 
 // Boost to the CM frame, isotropic direction, boost back (closed form A10).
@@ -471,7 +517,7 @@ __device__ __forceinline__ void pair_scatter(const CollideParams &P, uint32_t t,
     q[5] = 0.5 * (Pvz * f2 - rs * nz);
 }
 
-// Exclusive block scan with one barrier; s_warp is next written a round (several barriers) later.
+// Exclusive block scan with one barrier; s_warp is next written a sweep (several barriers) later.
 template <int THREADS>
 __device__ __forceinline__ uint32_t block_exclusive_scan_1b(uint32_t v, uint32_t *s_warp)
 {
@@ -495,28 +541,19 @@ __device__ __forceinline__ uint32_t block_exclusive_scan_1b(uint32_t v, uint32_t
     return __shfl_sync(0xFFFFFFFFu, winc - w, wid) + inc - v;
 }
 
-
-// Rare path of the in-bucket ranking: buckets with more than four elements, or equal 32-bit
-// keys (then the pid decides, A7; the keys of the other particles are recomputed).
-__device__ __noinline__ uint32_t slow_rank(uint64_t seed, uint32_t t, const uint32_t *spark, const uint32_t *spid,
-                                           uint32_t n, uint32_t nb, uint32_t j, uint32_t k, uint32_t beg, int rho)
+// Last resort of the ranking inside a dirty word (the list of dirty elements overflowed): count
+// the cell's elements of the same word with a smaller (key, pid), keys recomputed.
+// (Scalars only: a reference to the kernel parameters would force a copy of them onto the stack.)
+__device__ __noinline__ uint32_t brute_rank(uint64_t seed, uint32_t t, const uint32_t *spid, uint32_t n,
+                                            uint32_t M, uint32_t word, uint32_t k, uint32_t id, int rho)
 {
-    const uint32_t b = __umulhi(k, nb);
-    uint32_t rank = beg, same = 0;
-    for (uint32_t q = beg; q < n; ++q) {
-        const uint32_t kk = spark[q];
-        if (__umulhi(kk, nb) != b) break;
-        rank += kk < k ? 1u : 0u;
-        same += kk == k ? 1u : 0u;
+    uint32_t cnt = 0;
+    for (uint32_t i = 0; i < n; ++i) {
+        const uint32_t id2 = spid[i];
+        const uint32_t k2 = shuf_word(draw(seed, id2, t, (uint32_t)rho >> 2, kTagShuf, 0), rho);
+        if ((__umulhi(k2, M) >> 5) == word && (k2 < k || (k2 == k && id2 < id))) cnt += 1u;
     }
-    if (CUBA_FORCE_SLOW_PATHS || same > 1u) {
-        const uint32_t id = spid[j];
-        for (uint32_t i = 0; i < n; ++i) {
-            const uint32_t id2 = spid[i];
-            if (id2 < id && shuf_word(draw(seed, id2, t, (uint32_t)rho >> 2, kTagShuf, 0), rho) == k) rank += 1u;
-        }
-    }
-    return rank;
+    return cnt;
 }
 
 // Rare path of the Eq. 3 decision: the exact operation order of the oracle.
@@ -529,13 +566,17 @@ __device__ __noinline__ uint32_t exact_decision(double dd, double ee, double u, 
     return (u < prob ? 1u : 0u) | (fabs(u - prob) <= 1e-12 ? 2u : 0u);
 }
 
-// Per-CTA statistics in shared memory: [0] pairs, [1] collisions, [2] near-threshold decisions;
-// and the constants of the current cell that are only needed at a few places (kept out of
-// registers across the register-hungry phases).
+constexpr int kChains = 64;
+constexpr uint32_t kNil = 0xFFFFu;
+
+// Per-CTA state in static shared memory: constants of the current cell that are only needed at a
+// few places (kept out of registers across the register-hungry phases) and small counters.
 struct CtaStats {
     double scale, hscale;     // Eq. 3 factor cn*base/R of the current cell, and half of it
     uint32_t lo;              // first slot of the current cell
     uint32_t near;            // near-threshold decisions of this CTA (A16; rare)
+    uint32_t nlist[2];        // entries on the two dirty-element lists of the current sweep
+    uint32_t head[2][kChains]; // first entry of the chain of the words with (word mod kChains) equal, per list
     HistCell h;               // fused histogram: constants of the current cell
 };
 
@@ -545,11 +586,207 @@ struct ThreadStats {
     uint32_t hits;                       // uniform over a warp; lane 0 flushes
 };
 
-template <int THREADS, int ITEMS, int G, bool TRACE, bool LOCAL, bool GRAPH>
+// Shared-memory arrays of one CTA: fixed offsets into the dynamic shared memory, so that every
+// access is a shared-memory instruction with an immediate offset (no pointer registers).
+extern __shared__ __align__(128) unsigned char cuba_smem[];
+
+template <int CAP, int LCAP>
+struct CellSmem {
+    // (p_x, p_y) [CAP]
+    static __device__ __forceinline__ double2 *pxy() { return reinterpret_cast<double2 *>(cuba_smem); }
+    // p_z [CAP]
+    static __device__ __forceinline__ double *pz() { return reinterpret_cast<double *>(cuba_smem + 16 * CAP); }
+    // [2 CAP] bitmap of round A, bitmap of round B; as doubles: E[CAP] from the first pair phase on
+    static __device__ __forceinline__ uint32_t *bm() { return reinterpret_cast<uint32_t *>(cuba_smem + 24 * CAP); }
+    static __device__ __forceinline__ double *E() { return reinterpret_cast<double *>(cuba_smem + 24 * CAP); }
+    static __device__ __forceinline__ uint32_t *pid() { return reinterpret_cast<uint32_t *>(cuba_smem + 32 * CAP); }
+    // [CAP] per word: duplicates of round A | round B << 16; after the scan (prefix << 1 | dirty), packed alike
+    static __device__ __forceinline__ uint32_t *cnt() { return reinterpret_cast<uint32_t *>(cuba_smem + 36 * CAP); }
+    // [CAP] each: the order of round A / B
+    static __device__ __forceinline__ uint16_t *ord(int slot) { return reinterpret_cast<uint16_t *>(cuba_smem + 40 * CAP) + slot * CAP; }
+    // [LCAP] each, per round: dirty elements: key; word << 13 | index; prefix of the word | next entry of the chain << 16
+    static __device__ __forceinline__ uint32_t *lkey(int slot) { return reinterpret_cast<uint32_t *>(cuba_smem + 44 * CAP) + 3 * LCAP * slot; }
+    static __device__ __forceinline__ uint32_t *lwj(int slot) { return lkey(slot) + LCAP; }
+    static __device__ __forceinline__ uint32_t *lpn(int slot) { return lkey(slot) + 2 * LCAP; }
+    // [warps][PITEMS * 32] this warp's colliding pairs
+    static __device__ __forceinline__ uint16_t *hits() { return reinterpret_cast<uint16_t *>(cuba_smem + 44 * CAP + 24 * LCAP); }
+};
+
+__host__ __device__ constexpr int collide_list_cap(int cap) { return cap / 8 > 64 ? cap / 8 : 64; }
+__host__ __device__ constexpr size_t collide_smem_bytes(int cap, int threads, int items)
+{
+    return (size_t)cap * 44 + 2 * (size_t)collide_list_cap(cap) * 12 + (size_t)threads * ((items + 1) / 2) * 2 + 64;
+}
+
+// One pair phase (one round): Eq. 3 decision for the pairs order[2k], order[2k+1], then this warp's
+// hits are scattered.  first: the energies are computed here and left in sE (see above).  The pairs
+// are dealt to the warps in equal contiguous shares (the hits, and with them the scatter work, are
+// then spread evenly: a warp rarely has more than 32).
+template <typename S, int THREADS, int PITEMS, bool TRACE>
+__device__ __forceinline__ uint32_t pair_phase(const CollideParams &P, uint32_t c, uint32_t n, uint32_t tcur, int rho,
+                                            int slot, bool first, bool keepE, CtaStats *stats)
+{
+    const uint16_t *sord = S::ord(slot);
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const uint32_t npairs = n >> 1;
+    const uint32_t share = (npairs + THREADS / 32 - 1) / (THREADS / 32);        // pairs per warp
+    const uint32_t k0 = wid * share, k1 = min(npairs, k0 + share);              // this warp's pairs [k0, k1)
+    double *sE = S::E();
+    uint16_t *shit = S::hits() + wid * (PITEMS * 32);
+    if (first && tid == 0 && (n & 1u)) {          // the particle left over by the pairing: nobody else computes its energy
+        const uint32_t i = sord[n - 1u];
+        const double2 xy = S::pxy()[i];
+        sE[i] = energy(xy.x, xy.y, S::pz()[i]);
+    }
+    uint32_t nh = 0;
+    {
+        const double scale = *reinterpret_cast<volatile double *>(&stats->scale);
+        const double hscale = *reinterpret_cast<volatile double *>(&stats->hscale);
+        double dd[PITEMS], ee[PITEMS], u[PITEMS];
+        uint32_t ida[PITEMS];
+#pragma unroll
+        for (int it = 0; it < PITEMS; ++it) {
+            const uint32_t k = k0 + it * 32 + lane;
+            const uint32_t kc = min(k, npairs - 1u);
+            const uint32_t ab = *reinterpret_cast<const uint32_t *>(sord + 2 * kc);
+            const uint32_t a = ab & 0xFFFFu, b = ab >> 16;
+            const double2 pa = S::pxy()[a], pb = S::pxy()[b];
+            const double paz = S::pz()[a], pbz = S::pz()[b];
+            double Ea, Eb;
+            if (first) {
+                Ea = energy(pa.x, pa.y, paz); Eb = energy(pb.x, pb.y, pbz);
+                if (k < k1) { sE[a] = Ea; sE[b] = Eb; }
+            } else {
+                Ea = sE[a]; Eb = sE[b];
+            }
+            const double dx = Eb * pa.x - Ea * pb.x;
+            const double dy = Eb * pa.y - Ea * pb.y;
+            const double dz = Eb * paz - Ea * pbz;
+            ida[it] = S::pid()[a];
+            ee[it] = Ea * Eb;
+            dd[it] = (dx * dx + dy * dy) + dz * dz;
+        }
+#pragma unroll
+        for (int it = 0; it < PITEMS; ++it) {
+            const U4 w = drawk(P, tcur, ida[it], (uint32_t)rho, kTagDec, 0);
+            u[it] = u53_bits(w.x, w.y);
+        }
+#pragma unroll
+        for (int it = 0; it < PITEMS; ++it) {
+            const uint32_t k = k0 + it * 32 + lane;
+            bool hit;
+            if (TRACE) {
+                const double s = dd[it] / ee[it];         // (p_a+p_b)^2, A9
+                const double vrel = 0.5 * (s / ee[it]);   // s/(2 E_a E_b)
+                const double prob = vrel * scale;         // Eq. 3 * cn/R
+                hit = u[it] < prob;
+                if (k < k1) {
+                    if (fabs(u[it] - prob) <= 1e-12) atomicAdd(&stats->near, 1u);
+                    const uint32_t ab = *reinterpret_cast<const uint32_t *>(sord + 2 * k);
+                    const unsigned long long e = P.trace_off[c] + (unsigned long long)rho * npairs + k;
+                    P.tr_cell[e] = c; P.tr_round[e] = (uint32_t)rho; P.tr_pa[e] = ida[it]; P.tr_pb[e] = S::pid()[ab >> 16];
+                    P.tr_P[e] = prob; P.tr_u[e] = u[it]; P.tr_dec[e] = hit ? 1 : 0;
+                }
+            } else {
+                // sign(u - P) from u*(EaEb)^2 - |d|^2*scale/2; the exact form only inside a band
+                // far wider than the rounding error (it also catches NaN, inf and underflow)
+                const double ee2 = ee[it] * ee[it];
+                const double diff = u[it] * ee2 - dd[it] * hscale;
+                hit = diff < 0.0;
+                if (CUBA_FORCE_SLOW_PATHS || !(fabs(diff) > 4e-9 * ee2) || !(ee2 > 1e-280)) {
+                    const uint32_t r = exact_decision(dd[it], ee[it], u[it], scale);
+                    hit = (r & 1u) != 0;
+                    if ((r & 2u) && k < k1) atomicAdd(&stats->near, 1u);
+                }
+            }
+            hit = hit && k < k1;
+            const uint32_t hm = __ballot_sync(0xFFFFFFFFu, hit);
+            if (hit) shit[nh + __popc(hm & lanemask_lt())] = (uint16_t)k;
+            nh += __popc(hm);
+        }
+    }
+    __syncwarp();
+    // scatter this warp's colliding pairs, densely
+    for (uint32_t h = lane; h < nh; h += 32) {
+        const uint32_t k = shit[h];
+        const uint32_t ab = *reinterpret_cast<const uint32_t *>(sord + 2 * k);
+        const uint32_t a = ab & 0xFFFFu, b = ab >> 16;
+        const double2 pa = S::pxy()[a], pb = S::pxy()[b];
+        const double paz = S::pz()[a], pbz = S::pz()[b];
+        const double Ea = sE[a], Eb = sE[b];
+        const double ee = Ea * Eb;
+        const double dx = Eb * pa.x - Ea * pb.x;
+        const double dy = Eb * pa.y - Ea * pb.y;
+        const double dz = Eb * paz - Ea * pbz;
+        const double s = ((dx * dx + dy * dy) + dz * dz) / ee;
+        double q[6];
+        pair_scatter(P, tcur, S::pid()[a], (uint32_t)rho, s, pa.x, pa.y, paz, Ea, pb.x, pb.y, pbz, Eb, q);
+        S::pxy()[a] = make_double2(q[0], q[1]); S::pz()[a] = q[2];
+        S::pxy()[b] = make_double2(q[3], q[4]); S::pz()[b] = q[5];
+        if (keepE) { sE[a] = energy(q[0], q[1], q[2]); sE[b] = energy(q[3], q[4], q[5]); }
+    }
+    __syncwarp();   // the hit list is rewritten in the next pair phase
+    return nh;
+}
+
+// Phase C1 for one element and one of the two rounds of a sweep (slot 0 / 1): the rank of an element of
+// a clean word; an element of a dirty word goes onto the round's list, chained by word mod kChains.
+template <typename S, int LCAP>
+__device__ __forceinline__ void rank_clean(const CollideParams &P, CtaStats *stats, int slot,
+                                           uint32_t k, uint32_t j, uint32_t n, uint32_t M,
+                                           uint32_t tcur, int rho)
+{
+    const uint32_t b = __umulhi(k, M), word = b >> 5, below = (1u << (b & 31u)) - 1u;
+    const uint32_t pw = (S::cnt()[word] >> (16 * slot)) & 0xFFFFu;
+    uint32_t rank = (pw >> 1) + __popc((S::bm() + slot * n)[word] & below);
+    if (j < n) {
+        if (CUBA_FORCE_SLOW_PATHS || (pw & 1u)) {
+            const uint32_t at = atomicAdd(&stats->nlist[slot], 1u);
+            if (at < (uint32_t)LCAP) {
+                const uint32_t next = atomicExch(&stats->head[slot][word % kChains], at);
+                S::lkey(slot)[at] = k;
+                S::lwj(slot)[at] = (word << 13) | j;
+                S::lpn(slot)[at] = (pw >> 1) | (next << 16);
+                return;
+            }
+            rank = (pw >> 1) + brute_rank(P.seed, tcur, S::pid(), n, M, word, k, S::pid()[j], rho);   // the list is full
+        }
+        S::ord(slot)[rank] = (uint16_t)j;
+    }
+}
+
+// Phase C2, one thread per list entry (the two lists side by side, each on its own half of the CTA): rank
+// inside the dirty word = entries of the same word with a smaller (key, pid), found on the word's chain.
+template <typename S, int LCAP, int THREADS>
+__device__ __forceinline__ void rank_dirty(const CollideParams &P, const CtaStats *stats, uint32_t n, uint32_t M,
+                                           uint32_t tcur, int rho0, bool two)
+{
+    constexpr int HALF = THREADS >= 64 ? THREADS / 2 : THREADS;
+    const int slot = (THREADS >= 64 && (int)threadIdx.x >= HALF) ? 1 : 0;
+    for (int pass = 0; pass < (THREADS >= 64 ? 1 : 2); ++pass) {
+        const int sl = THREADS >= 64 ? slot : pass;
+        if (sl == 1 && !two) break;
+        const uint32_t nl = stats->nlist[sl];
+        for (uint32_t i = threadIdx.x - (THREADS >= 64 ? sl * HALF : 0); i < min(nl, (uint32_t)LCAP); i += HALF) {
+            const uint32_t k = S::lkey(sl)[i], wj = S::lwj(sl)[i];
+            const uint32_t word = wj >> 13, j = wj & 0x1FFFu, id = S::pid()[j];
+            uint32_t cnt = 0;
+            if (nl <= (uint32_t)LCAP) {
+                for (uint32_t q = stats->head[sl][word % kChains]; q != kNil; q = S::lpn(sl)[q] >> 16) {
+                    const uint32_t wj2 = S::lwj(sl)[q], k2 = S::lkey(sl)[q];
+                    if ((wj2 >> 13) == word && (k2 < k || (k2 == k && S::pid()[wj2 & 0x1FFFu] < id))) cnt += 1u;
+                }
+            } else {
+                cnt = brute_rank(P.seed, tcur, S::pid(), n, M, word, k, id, rho0 + sl);   // some elements of the word may be missing from the list
+            }
+            S::ord(sl)[(S::lpn(sl)[i] & 0xFFFFu) + cnt] = (uint16_t)j;
+        }
+    }
+}
+
+template <int THREADS, int ITEMS, int G, int CAP, int LCAP, bool TRACE, bool LOCAL, bool GRAPH>
 __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32_t c, uint32_t lo, uint32_t n,
-                                                  double *sp0, double *sp1, double *sp2, double *sE,
-                                                  uint32_t *spid, uint32_t *spark, uint32_t *sbkt,
-                                                  uint16_t *sord, uint32_t *s_warp, CtaStats *stats,
+                                                  uint32_t *s_warp, CtaStats *stats,
                                                   uint32_t *s_seg, long long *s_esum, ThreadStats &acc,
                                                   uint32_t lo_next, uint32_t n_next)
 {
@@ -557,7 +794,8 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
     constexpr int NG = ITEMS / G;
     constexpr int PITEMS = (ITEMS + 1) / 2;          // pairs per thread
     constexpr int SCAN = ITEMS | 1;                  // words per thread in the scan (odd stride: no bank conflicts)
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    using S = CellSmem<CAP, LCAP>;
+    const int tid = threadIdx.x;
     // step index: a constant-bank operand normally; a register loaded from device memory when the
     // kernel is a node of a replayed CUDA graph (small problems only, where registers are plentiful)
     const uint32_t tcur = GRAPH ? *P.t_dev : P.t;
@@ -574,20 +812,22 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
         else R = (pmax <= 1.0) ? 1 : (int)ceil(pmax);
         if (n < 2u) R = 0;          // a single particle has no partner; it is here for the fused histogram only
     }
+    for (int e = tid; e < 2 * kChains; e += THREADS) (&stats->head[0][0])[e] = kNil;
     if (tid == 0) {
         stats->lo = lo;
+        stats->nlist[0] = 0; stats->nlist[1] = 0;
         if (!local) {
             const double scale = (cn * base) / (double)R;
             stats->scale = scale; stats->hscale = 0.5 * scale;
         }
-        if (hist) hist_cell_setup(P.g, c, &stats->h);
     }
-    const uint32_t npairs = n >> 1, nb = 2u * n, last = n - 1u;
-    uint16_t *sb16 = reinterpret_cast<uint16_t *>(sbkt);
-    uint16_t *shit = reinterpret_cast<uint16_t *>(spark) + wid * (PITEMS * 32);   // this warp's hit list
-    uint32_t key[ITEMS], aux[ITEMS], keep[ITEMS];
+    if (hist && tid < 32) hist_cell_setup(P.g, c, &stats->h, tid);
+    const uint32_t last = n - 1u;
+    const uint32_t M = 32u * n;                      // bits of a bitmap: word = bit >> 5 < n
+    uint32_t *bmA = S::bm(), *bmB = S::bm() + n;
+    double *sE = S::E();   // E[n] covers exactly the two bitmaps (2 n words)
 
-    // ---- stage the cell: momenta, energies, pids; clear the bucket counters -----------------
+    // ---- stage the cell: momenta and pids; clear the bitmaps and the duplicate counters ---------
     long long esum = 0;
 #pragma unroll
     for (int g = 0; g < NG; ++g) {
@@ -602,10 +842,10 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
 #pragma unroll
         for (int i = 0; i < G; ++i) {
             const uint32_t j = tid + (g * G + i) * THREADS;
-            const double e = energy(a[i], b[i], cc[i]);
             if (j < n) {
-                sp0[j] = a[i]; sp1[j] = b[i]; sp2[j] = cc[i]; sE[j] = e; spid[j] = id[i]; sbkt[j] = 0;
-                if (local) esum += energy_fixed(e);
+                S::pxy()[j] = make_double2(a[i], b[i]); S::pz()[j] = cc[i]; S::pid()[j] = id[i];
+                *reinterpret_cast<uint2 *>(S::bm() + 2 * j) = make_uint2(0u, 0u); S::cnt()[j] = 0;
+                if (local) esum += energy_fixed(energy(a[i], b[i], cc[i]));
             }
         }
     }
@@ -619,7 +859,7 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
         if (!(pmax <= 64.0)) { if (tid == 0) atomicOr(P.flags, kFlagRounds); R = 64; }
         else R = (pmax <= 1.0) ? 1 : (int)ceil(pmax);
         if (n < 2u) R = 0;
-        if (tid == 0) {             // read in phase (e1), several barriers from here
+        if (tid == 0) {             // read in the pair phases, several barriers from here
             const double scale = (cn * base) / (double)R;
             stats->scale = scale; stats->hscale = 0.5 * scale;
         }
@@ -633,246 +873,138 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
     }
 
     uint32_t warp_hits = 0;
-    for (int rho = 0; rho < R; ++rho) {
-        // (a) shuffle keys (A7: word rho mod 4 of the call for rounds 4*(rho div 4)..+3; one call
-        // serves two rounds, the second word is kept) and bucket counts
+    for (int rho0 = 0; rho0 < R; rho0 += 2) {
+        const bool two = rho0 + 1 < R;
+        if (rho0 > 0) {
+            // later sweeps: the energies (in the bitmaps' space) are dead again until the next pair phase
+            __syncthreads();
+#pragma unroll
+            for (int it = 0; it < ITEMS; ++it) {
+                const uint32_t j = tid + it * THREADS;
+                if (j < n) { *reinterpret_cast<uint2 *>(S::bm() + 2 * j) = make_uint2(0u, 0u); S::cnt()[j] = 0; }
+            }
+            for (int e = tid; e < 2 * kChains; e += THREADS) (&stats->head[0][0])[e] = kNil;
+            if (tid == 0) { stats->nlist[0] = 0; stats->nlist[1] = 0; }
+            __syncthreads();
+        }
+        uint32_t keyA[ITEMS], keyB[ITEMS];
+        // (A) shuffle keys of the two rounds (A7: words 2*(sweep mod 2), +1 of the call for rounds
+        // 4*(rho div 4)..+3) and one atomicOr per element and round
 #pragma unroll
         for (int g = 0; g < NG; ++g) {
             if ((uint32_t)(g * G * THREADS) >= n) break;
-            if ((rho & 1) == 0) {
 #pragma unroll
-                for (int i = 0; i < G; ++i) {
-                    const int it = g * G + i;
-                    const uint32_t jc = min((uint32_t)(tid + it * THREADS), last);
-                    const U4 w = drawk(P, tcur, spid[jc], (uint32_t)rho >> 2, kTagShuf, 0);
-                    key[it] = (rho & 2) ? w.z : w.x;
-                    keep[it] = (rho & 2) ? w.w : w.y;
-                }
-            } else {
-#pragma unroll
-                for (int i = 0; i < G; ++i) key[g * G + i] = keep[g * G + i];
+            for (int i = 0; i < G; ++i) {
+                const int it = g * G + i;
+                const uint32_t jc = min((uint32_t)(tid + it * THREADS), last);
+                const U4 w = drawk(P, tcur, S::pid()[jc], (uint32_t)rho0 >> 2, kTagShuf, 0);
+                keyA[it] = (rho0 & 2) ? w.z : w.x;
+                keyB[it] = (rho0 & 2) ? w.w : w.y;
             }
 #pragma unroll
             for (int i = 0; i < G; ++i) {
                 const int it = g * G + i;
                 const uint32_t j = tid + it * THREADS;
-                const uint32_t b = __umulhi(key[it], nb);
-                const uint32_t sh = (b & 1u) * 16u;
-                aux[it] = 0;
-                if (j < n) aux[it] = (atomicAdd(&sbkt[b >> 1], 1u << sh) >> sh) & 0xFFFFu;   // arrival slot
+                if (j < n) {
+                    const uint32_t bA = __umulhi(keyA[it], M), mA = 1u << (bA & 31u);
+                    if (atomicOr(&bmA[bA >> 5], mA) & mA) atomicAdd(&S::cnt()[bA >> 5], 1u);
+                    if (two) {
+                        const uint32_t bB = __umulhi(keyB[it], M), mB = 1u << (bB & 31u);
+                        if (atomicOr(&bmB[bB >> 5], mB) & mB) atomicAdd(&S::cnt()[bB >> 5], 0x10000u);
+                    }
+                }
             }
         }
         __syncthreads();
-        // (b) exclusive scan of the 2n counters (n words), a contiguous chunk of words per thread
+        // (B) per word: elements = popc + duplicates, both rounds packed in one word; exclusive scan
         {
             const uint32_t chunk = ((n + THREADS - 1) / THREADS) | 1u;
             const uint32_t w0 = min(n, tid * chunk), w1 = min(n, w0 + chunk);
-            uint32_t v[SCAN], sum = 0;
+            uint32_t v[SCAN], sum = 0, dirty = 0;
 #pragma unroll
             for (int q = 0; q < SCAN; ++q) {
-                v[q] = (w0 + q < w1) ? sbkt[w0 + q] : 0u;
-                sum += (v[q] & 0xFFFFu) + (v[q] >> 16);
+                v[q] = 0;
+                if (w0 + q < w1) {
+                    const uint32_t cw = S::cnt()[w0 + q];
+                    v[q] = (__popc(bmA[w0 + q]) + (cw & 0xFFFFu)) + ((__popc(bmB[w0 + q]) + (cw >> 16)) << 16);
+                    dirty |= (((cw & 0xFFFFu) ? 1u : 0u) | ((cw >> 16) ? 2u : 0u)) << (2 * q);
+                }
+                sum += v[q];
             }
-            uint32_t run = block_exclusive_scan_1b<THREADS>(sum, s_warp);
+            uint32_t run = block_exclusive_scan_1b<THREADS>(sum, s_warp);   // its barrier separates the reads of cnt above from the writes below
+            if (THREADS == 32) __syncwarp();
 #pragma unroll
             for (int q = 0; q < SCAN; ++q) {
-                const uint32_t mid = run + (v[q] & 0xFFFFu);
-                if (w0 + q < w1) sbkt[w0 + q] = run | (mid << 16);
-                run = mid + (v[q] >> 16);
-            }
-        }
-        __syncthreads();
-        // (c) park the key at bucket start + arrival slot; four sentinels behind the last key
-#pragma unroll
-        for (int g = 0; g < NG; ++g) {
-            if ((uint32_t)(g * G * THREADS) >= n) break;
-#pragma unroll
-            for (int i = 0; i < G; ++i) {
-                const int it = g * G + i;
-                const uint32_t j = tid + it * THREADS;
-                const uint32_t beg = sb16[__umulhi(key[it], nb)];
-                if (j < n) spark[beg + aux[it]] = key[it];
-                aux[it] = (j < n) ? beg : 0u;
-            }
-        }
-        if (tid < 4) spark[n + tid] = 0xFFFFFFFFu;
-        __syncthreads();
-        // (d) rank = bucket start + number of bucket mates with a smaller key.  Keys beyond the
-        // bucket are larger (the bucket index is monotone in the key), so four words decide a
-        // bucket of up to four; the fifth tells whether the bucket is bigger.
-#pragma unroll
-        for (int g = 0; g < NG; ++g) {
-            if ((uint32_t)(g * G * THREADS) >= n) break;
-            uint32_t rank[G];
-            bool slow[G];
-#pragma unroll
-            for (int i = 0; i < G; ++i) {
-                const int it = g * G + i;
-                const uint32_t k = key[it], beg = aux[it];
-                const uint32_t k0 = spark[beg], k1 = spark[beg + 1], k2 = spark[beg + 2], k3 = spark[beg + 3],
-                               k4 = spark[beg + 4];
-                rank[i] = beg + (k0 < k ? 1u : 0u) + (k1 < k ? 1u : 0u) + (k2 < k ? 1u : 0u) + (k3 < k ? 1u : 0u);
-                const uint32_t same = (k0 == k ? 1u : 0u) + (k1 == k ? 1u : 0u) + (k2 == k ? 1u : 0u) + (k3 == k ? 1u : 0u);
-                slow[i] = (tid + it * THREADS < n) &&
-                          (CUBA_FORCE_SLOW_PATHS || same != 1u || __umulhi(k4, nb) == __umulhi(k, nb));
-            }
-            bool any = false;
-#pragma unroll
-            for (int i = 0; i < G; ++i) any = any || slow[i];
-            if (any) {
-#pragma unroll
-                for (int i = 0; i < G; ++i)
-                    if (slow[i]) rank[i] = slow_rank(P.seed, tcur, spark, spid, n, nb, tid + (g * G + i) * THREADS,
-                                                     key[g * G + i], aux[g * G + i], rho);
-            }
-#pragma unroll
-            for (int i = 0; i < G; ++i) {
-                const uint32_t j = tid + (g * G + i) * THREADS;
-                if (j < n) {
-                    sord[rank[i]] = (uint16_t)j;
-                    sbkt[j] = 0;                 // the counters are free: clear them for the next round
+                if (w0 + q < w1) {
+                    const uint32_t d = (dirty >> (2 * q)) & 3u;
+                    S::cnt()[w0 + q] = (((run & 0xFFFFu) << 1) | (d & 1u)) | ((((run >> 16) << 1) | (d >> 1)) << 16);
                 }
+                run += v[q];
             }
         }
         __syncthreads();
-        // (e1) pair order[2k] with order[2k+1]: Eq. 3 decision; this warp's hits go to its list
-        uint32_t nh = 0;
-        {
-            const double scale = *reinterpret_cast<volatile double *>(&stats->scale);
-            const double hscale = *reinterpret_cast<volatile double *>(&stats->hscale);
-            double dd[PITEMS], ee[PITEMS], u[PITEMS];
-            uint32_t ida[PITEMS];
+        // (C1) rank = prefix of the word + occupied bits below mine; elements of dirty words go onto a list
 #pragma unroll
-            for (int it = 0; it < PITEMS; ++it) {
-                const uint32_t kc = min((uint32_t)(tid + it * THREADS), npairs - 1u);
-                const uint32_t ab = *reinterpret_cast<const uint32_t *>(sord + 2 * kc);
-                const uint32_t a = ab & 0xFFFFu, b = ab >> 16;
-                const double Ea = sE[a], Eb = sE[b];
-                const double dx = Eb * sp0[a] - Ea * sp0[b];
-                const double dy = Eb * sp1[a] - Ea * sp1[b];
-                const double dz = Eb * sp2[a] - Ea * sp2[b];
-                ida[it] = spid[a];
-                ee[it] = Ea * Eb;
-                dd[it] = (dx * dx + dy * dy) + dz * dz;
-            }
-#pragma unroll
-            for (int it = 0; it < PITEMS; ++it) {
-                const U4 w = drawk(P, tcur, ida[it], (uint32_t)rho, kTagDec, 0);
-                u[it] = u53_bits(w.x, w.y);
-            }
-#pragma unroll
-            for (int it = 0; it < PITEMS; ++it) {
-                const uint32_t k = tid + it * THREADS;
-                bool hit;
-                if (TRACE) {
-                    const double s = dd[it] / ee[it];         // (p_a+p_b)^2, A9
-                    const double vrel = 0.5 * (s / ee[it]);   // s/(2 E_a E_b)
-                    const double prob = vrel * scale;         // Eq. 3 * cn/R
-                    hit = u[it] < prob;
-                    if (k < npairs) {
-                        if (fabs(u[it] - prob) <= 1e-12) atomicAdd(&stats->near, 1u);
-                        const uint32_t ab = *reinterpret_cast<const uint32_t *>(sord + 2 * k);
-                        const unsigned long long e = P.trace_off[c] + (unsigned long long)rho * npairs + k;
-                        P.tr_cell[e] = c; P.tr_round[e] = (uint32_t)rho; P.tr_pa[e] = ida[it]; P.tr_pb[e] = spid[ab >> 16];
-                        P.tr_P[e] = prob; P.tr_u[e] = u[it]; P.tr_dec[e] = hit ? 1 : 0;
-                    }
-                } else {
-                    // sign(u - P) from u*(EaEb)^2 - |d|^2*scale/2; the exact form only inside a band
-                    // far wider than the rounding error (it also catches NaN, inf and underflow)
-                    const double ee2 = ee[it] * ee[it];
-                    const double diff = u[it] * ee2 - dd[it] * hscale;
-                    hit = diff < 0.0;
-                    if (CUBA_FORCE_SLOW_PATHS || !(fabs(diff) > 4e-9 * ee2) || !(ee2 > 1e-280)) {
-                        const uint32_t r = exact_decision(dd[it], ee[it], u[it], scale);
-                        hit = (r & 1u) != 0;
-                        if ((r & 2u) && k < npairs) atomicAdd(&stats->near, 1u);
-                    }
-                }
-                hit = hit && k < npairs;
-                const uint32_t hm = __ballot_sync(0xFFFFFFFFu, hit);
-                if (hit) shit[nh + __popc(hm & lanemask_lt())] = (uint16_t)k;
-                nh += __popc(hm);
-            }
+        for (int it = 0; it < ITEMS; ++it) {
+            if ((uint32_t)(it * THREADS) >= n) break;
+            const uint32_t j = tid + it * THREADS;
+#pragma unroll 1
+            for (int sl = 0; sl < (two ? 2 : 1); ++sl)
+                rank_clean<S, LCAP>(P, stats, sl, sl ? keyB[it] : keyA[it], j, n, M, tcur, rho0 + sl);
         }
-        __syncwarp();
-        // (e2) scatter this warp's colliding pairs, densely
-        for (uint32_t h = lane; h < nh; h += 32) {
-            const uint32_t k = shit[h];
-            const uint32_t ab = *reinterpret_cast<const uint32_t *>(sord + 2 * k);
-            const uint32_t a = ab & 0xFFFFu, b = ab >> 16;
-            const double pax = sp0[a], pay = sp1[a], paz = sp2[a], Ea = sE[a];
-            const double pbx = sp0[b], pby = sp1[b], pbz = sp2[b], Eb = sE[b];
-            const double ee = Ea * Eb;
-            const double dx = Eb * pax - Ea * pbx;
-            const double dy = Eb * pay - Ea * pby;
-            const double dz = Eb * paz - Ea * pbz;
-            const double s = ((dx * dx + dy * dy) + dz * dz) / ee;
-            double q[6];
-            pair_scatter(P, tcur, spid[a], (uint32_t)rho, s, pax, pay, paz, Ea, pbx, pby, pbz, Eb, q);
-            sp0[a] = q[0]; sp1[a] = q[1]; sp2[a] = q[2];
-            sp0[b] = q[3]; sp1[b] = q[4]; sp2[b] = q[5];
-            if (rho + 1 < R || hist) { sE[a] = energy(q[0], q[1], q[2]); sE[b] = energy(q[3], q[4], q[5]); }
+        __syncthreads();
+        // (C2) the listed elements, one thread each
+        rank_dirty<S, LCAP, THREADS>(P, stats, n, M, tcur, rho0, two);
+        __syncthreads();
+        // pair phases of the two rounds; energies appear in the first one
+#pragma unroll 1
+        for (int sl = 0; sl < (two ? 2 : 1); ++sl) {
+            if (sl) __syncthreads();
+            warp_hits += pair_phase<S, THREADS, PITEMS, TRACE>(P, c, n, tcur, rho0 + sl, sl, sl == 0, sl == 0 ? (two || hist) : hist, stats);
         }
-        warp_hits += nh;
-        __syncwarp();   // the hit list is rewritten in the next round
+    }
+    if (R == 0 && hist && tid == 0) {     // a lone particle: no pair phase has computed its energy
+        const double2 xy = S::pxy()[0];
+        sE[0] = energy(xy.x, xy.y, S::pz()[0]);
     }
     __syncthreads();
     const uint32_t lo_w = *reinterpret_cast<volatile uint32_t *>(&stats->lo);
-    // positions for the fused histogram: all loads of a thread in flight before anything waits on them
-#ifndef CUBA_HB6
-#define CUBA_HB6 2
-#endif
-    constexpr int HB = (ITEMS == 6) ? CUBA_HB6 : ((ITEMS % 2 == 0) ? 2 : 1);
-    double xx[HB], yy[HB], zz[HB];
-    if (hist && HB == ITEMS) {
-#pragma unroll
-        for (int it = 0; it < HB; ++it) {
-            const uint32_t jc = lo_w + min((uint32_t)(tid + it * THREADS), last);
-            xx[it] = P.x[jc]; yy[it] = P.y[jc]; zz[it] = P.z[jc];
-        }
-    }
-#pragma unroll
-    for (int g = 0; g < NG; ++g) {
-        if ((uint32_t)(g * G * THREADS) >= n) break;
-#pragma unroll
-        for (int i = 0; i < G; ++i) {
-            const uint32_t j = tid + (g * G + i) * THREADS;
-            if (j < n) { P.px[lo_w + j] = sp0[j]; P.py[lo_w + j] = sp1[j]; P.pz[lo_w + j] = sp2[j]; }
-        }
+    constexpr int HB = (ITEMS % 2 == 0) ? 2 : 1;
+#pragma unroll 1
+    for (uint32_t j = tid; j < n; j += THREADS) {
+        const double2 xy = S::pxy()[j];
+        P.px[lo_w + j] = xy.x; P.py[lo_w + j] = xy.y; P.pz[lo_w + j] = S::pz()[j];
     }
     acc.hits += warp_hits;
-    acc.pairs += (unsigned long long)R * npairs;
+    acc.pairs += (unsigned long long)R * (n >> 1);
     acc.rounds += (unsigned long long)R;
 
     // ---- fused histogram of the next step (S1-S3 of step t+1 on the final momenta) ----------
     if (hist) {
         const uint32_t T0 = lo_w / kTile;
         const HistCell &hc = stats->h;
-#pragma unroll
+#pragma unroll 1
         for (int g = 0; g < ITEMS / HB; ++g) {
             if ((uint32_t)(g * HB * THREADS) >= n) break;
-            if (HB != ITEMS) {
+            double xx[HB], yy[HB], zz[HB];
 #pragma unroll
-                for (int i = 0; i < HB; ++i) {
-                    const uint32_t jc = lo_w + min((uint32_t)(tid + (g * HB + i) * THREADS), last);
-                    xx[i] = P.x[jc]; yy[i] = P.y[jc]; zz[i] = P.z[jc];
-                }
+            for (int i = 0; i < HB; ++i) {
+                const uint32_t jc = lo_w + min((uint32_t)(tid + (g * HB + i) * THREADS), last);
+                xx[i] = P.x[jc]; yy[i] = P.y[jc]; zz[i] = P.z[jc];
             }
 #pragma unroll
             for (int i = 0; i < HB; ++i) {
                 const uint32_t j = tid + (g * HB + i) * THREADS, jj = min(j, last);
-                const int d = next_direction_guarded(P.g, P.next_dt, hc, xx[i], yy[i], zz[i],
-                                                     sp0[jj], sp1[jj], sp2[jj], sE[jj]);
-                const bool valid = j < n;
-                if (valid && d < 0) atomicOr(P.flags, kFlagMoved);
-                const uint32_t key = ((lo_w + jj) / kTile - T0) * kDirs + (uint32_t)max(d, 0);
-                const uint32_t active = __ballot_sync(0xFFFFFFFFu, valid);
-                if (valid) {
-                    const uint32_t peers = __match_any_sync(active, key);
-                    if ((peers & lanemask_lt()) == 0) atomicAdd(&s_seg[key], (uint32_t)__popc(peers));
+                const double2 xy = S::pxy()[jj];
+                const int d = next_direction_guarded(P.g, P.next_dt, hc, xx[i], yy[i], zz[i], xy.x, xy.y, S::pz()[jj], sE[jj]);
+                if (j < n && d != (int)kDirStay) {
+                    if (d < 0) atomicOr(P.flags, kFlagMoved);
+                    atomicAdd(&s_seg[((lo_w + j) / kTile - T0) * kDirs + (uint32_t)max(d, 0)], 1u);
                 }
             }
         }
+        __syncthreads();
+        hist_fill_stay<THREADS>(lo_w, n, s_seg);
         __syncthreads();
         hist_publish<THREADS>(P, c, lo_w, n, s_seg);
     }
@@ -923,25 +1055,21 @@ __device__ __forceinline__ void flush_counters(const CollideParams &P, unsigned 
     }
 }
 
-// Shared-memory classes: CAP particles at most, 46 B of shared memory per particle.  The next
+// Shared-memory classes: CAP particles at most, 44 B of shared memory per particle.  The next
 // work item is fetched one cell ahead and its momenta / pids are prefetched into L2 while
 // the current cell is processed, so the load phase does not wait on DRAM.
 template <int THREADS, int ITEMS, int CAP, int MIN_BLOCKS, bool TRACE, bool LOCAL, bool GRAPH>
 __global__ void __launch_bounds__(THREADS, MIN_BLOCKS)
 k_collide(CollideParams P)
 {
-    static_assert(CAP <= THREADS * ITEMS && CAP < 65536, "class capacity");
+    static_assert(CAP <= THREADS * ITEMS && CAP < 8192 && CAP % 32 == 0, "class capacity");
 #ifndef CUBA_G6
 #define CUBA_G6 3
 #endif
     constexpr int G = (ITEMS == 6) ? CUBA_G6 : ((ITEMS % 2 == 0) ? 2 : ITEMS);
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    double *sp0 = reinterpret_cast<double *>(smem_raw);
-    double *sp1 = sp0 + CAP, *sp2 = sp1 + CAP, *sE = sp2 + CAP;
-    uint32_t *spid = reinterpret_cast<uint32_t *>(sE + CAP);
-    uint32_t *spark = spid + CAP;                // CAP keys + 4 sentinels (+ pad); hit lists between (d) and (c)
-    uint32_t *sbkt = spark + CAP + 8;            // CAP words = 2 CAP packed 16-bit counters
-    uint16_t *sord = reinterpret_cast<uint16_t *>(sbkt + CAP + 8);
+    constexpr int LCAP = collide_list_cap(CAP);
+    constexpr int PITEMS = (ITEMS + 1) / 2;
+    static_assert(collide_smem_bytes(CAP, THREADS, ITEMS) >= (size_t)CAP * 44 + 24 * (size_t)LCAP + (size_t)THREADS * PITEMS * 2, "carve");
     __shared__ uint32_t s_warp[32];
     __shared__ CtaStats s_stats;
     __shared__ uint32_t s_seg[((CAP + kTile - 2) / kTile + 1) * kDirs];   // a cell of CAP particles spans at most this many tiles
@@ -965,8 +1093,8 @@ k_collide(CollideParams P)
         item = s_item[(it + 1) & 1];
         uint4 nxt = make_uint4(0u, 0u, 0u, 0u);
         if (item < nlist) nxt = P.list[item];   // first used after the staging barrier
-        collide_cell_smem<THREADS, ITEMS, G, TRACE, LOCAL, GRAPH>(P, cur.x, cur.y, cur.z, sp0, sp1, sp2, sE, spid, spark, sbkt, sord,
-                                                    s_warp, &s_stats, s_seg, s_esum, acc, nxt.y, nxt.z);
+        collide_cell_smem<THREADS, ITEMS, G, CAP, LCAP, TRACE, LOCAL, GRAPH>(P, cur.x, cur.y, cur.z, s_warp, &s_stats, s_seg, s_esum,
+                                                                        acc, nxt.y, nxt.z);
         __syncthreads();
         cur = nxt;
     }
@@ -981,8 +1109,6 @@ k_collide(CollideParams P)
 // step index in device memory for graph replays
 __global__ void k_set_t(uint32_t *t_dev, uint32_t v) { *t_dev = v; }
 __global__ void k_bump_t(uint32_t *t_dev) { *t_dev += 1u; }
-
-constexpr size_t collide_smem_bytes(int cap) { return (size_t)cap * 46 + 64; }
 
 // Overflow class: cells larger than the biggest shared-memory class.  Same routine, scratch
 // in global memory (momenta are updated in place in the particle store; the cached energy

@@ -289,10 +289,10 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
     }
 
 #define CUBA_OCC(K, T, I, C, MB)                                                                                          \
-    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, true, false, false>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]); \
-    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, false, true, false>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]); \
-    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, false, false, true>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]); \
-    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, false, false, false>, T, collide_smem_bytes(C), sms, &ctx->grid_cls[K]);
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, true, false, false>, T, collide_smem_bytes(C, T, I), sms, &ctx->grid_cls[K]); \
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, false, true, false>, T, collide_smem_bytes(C, T, I), sms, &ctx->grid_cls[K]); \
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, false, false, true>, T, collide_smem_bytes(C, T, I), sms, &ctx->grid_cls[K]); \
+    if (rc == CUBA_OK) rc = occupancy_grid(k_collide<T, I, C, MB, false, false, false>, T, collide_smem_bytes(C, T, I), sms, &ctx->grid_cls[K]);
     rc = CUBA_OK;
     CUBA_FOR_EACH_CLASS(CUBA_OCC)
 #undef CUBA_OCC
@@ -435,9 +435,9 @@ static int launch_collide(cuba_ctx *ctx, double base, const TraceDev *td, double
         cudaStream_t st = serial ? main : ctx->cls_stream[K];                                    \
         if (!serial) CU(cudaStreamWaitEvent(st, ctx->ev_fork, 0));                               \
         cls(K);                                                                                  \
-        if (!TRACE && ctx->capturing) k_collide<T, I, C, MB, false, false, true><<<ctx->grid_cls[K], T, collide_smem_bytes(C), st>>>(P); \
-        else if (!TRACE && etas > 0.0) k_collide<T, I, C, MB, false, true, false><<<ctx->grid_cls[K], T, collide_smem_bytes(C), st>>>(P); \
-        else k_collide<T, I, C, MB, TRACE, false, false><<<ctx->grid_cls[K], T, collide_smem_bytes(C), st>>>(P);    \
+        if (!TRACE && ctx->capturing) k_collide<T, I, C, MB, false, false, true><<<ctx->grid_cls[K], T, collide_smem_bytes(C, T, I), st>>>(P); \
+        else if (!TRACE && etas > 0.0) k_collide<T, I, C, MB, false, true, false><<<ctx->grid_cls[K], T, collide_smem_bytes(C, T, I), st>>>(P); \
+        else k_collide<T, I, C, MB, TRACE, false, false><<<ctx->grid_cls[K], T, collide_smem_bytes(C, T, I), st>>>(P);    \
         LAUNCHED();                                                                              \
         if (serial) prof_mark(ctx, G_COLLIDE0 + K);                                              \
         else { CU(cudaEventRecord(ctx->ev_join[K], st)); CU(cudaStreamWaitEvent(main, ctx->ev_join[K], 0)); } \
