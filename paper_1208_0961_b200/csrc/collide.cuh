@@ -784,94 +784,21 @@ __device__ __forceinline__ void rank_dirty(const CollideParams &P, const CtaStat
     }
 }
 
-template <int THREADS, int ITEMS, int G, int CAP, int LCAP, bool TRACE, bool LOCAL, bool GRAPH>
-__device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32_t c, uint32_t lo, uint32_t n,
-                                                  uint32_t *s_warp, CtaStats *stats,
-                                                  uint32_t *s_seg, long long *s_esum, ThreadStats &acc,
-                                                  uint32_t lo_next, uint32_t n_next)
+// All R rounds of one staged cell, two per sweep (see above).  On entry: momenta and pids staged, both
+// bitmaps, the duplicate counters, the list counters and chain heads cleared, a block barrier passed.
+// keepE: the caller needs the energies of the final momenta in sE afterwards.  Returns this warp's hits.
+template <int THREADS, int ITEMS, int G, int CAP, int LCAP, bool TRACE>
+__device__ __forceinline__ uint32_t run_sweeps(const CollideParams &P, uint32_t c, uint32_t n, int R, uint32_t tcur,
+                                               bool hist, uint32_t *s_warp, CtaStats *stats)
 {
-    static_assert(ITEMS % G == 0, "items are processed in groups of G");
+    using S = CellSmem<CAP, LCAP>;
     constexpr int NG = ITEMS / G;
     constexpr int PITEMS = (ITEMS + 1) / 2;          // pairs per thread
     constexpr int SCAN = ITEMS | 1;                  // words per thread in the scan (odd stride: no bank conflicts)
-    using S = CellSmem<CAP, LCAP>;
     const int tid = threadIdx.x;
-    // step index: a constant-bank operand normally; a register loaded from device memory when the
-    // kernel is a node of a replayed CUDA graph (small problems only, where registers are plentiful)
-    const uint32_t tcur = GRAPH ? *P.t_dev : P.t;
-    const bool hist = P.next_dt > 0.0;
-    constexpr bool local = LOCAL;     // compile-time: the constant-sigma kernels carry none of its registers
-    // rounds and scale (A5, A6): identical integer/fp64 results on every thread.  With the local
-    // cross section the factor needs the cell's energy sum and is computed after staging.
-    double base = P.base;
-    const double cn = (n & 1u) ? (double)n : (double)(n - 1u);
-    int R = 0;
-    if (!local) {
-        const double pmax = (2.0 * cn) * base;
-        if (!(pmax <= 64.0)) { if (tid == 0) atomicOr(P.flags, kFlagRounds); R = 64; }
-        else R = (pmax <= 1.0) ? 1 : (int)ceil(pmax);
-        if (n < 2u) R = 0;          // a single particle has no partner; it is here for the fused histogram only
-    }
-    for (int e = tid; e < 2 * kChains; e += THREADS) (&stats->head[0][0])[e] = kNil;
-    if (tid == 0) {
-        stats->lo = lo;
-        stats->nlist[0] = 0; stats->nlist[1] = 0;
-        if (!local) {
-            const double scale = (cn * base) / (double)R;
-            stats->scale = scale; stats->hscale = 0.5 * scale;
-        }
-    }
-    if (hist && tid < 32) hist_cell_setup(P.g, c, &stats->h, tid);
     const uint32_t last = n - 1u;
     const uint32_t M = 32u * n;                      // bits of a bitmap: word = bit >> 5 < n
     uint32_t *bmA = S::bm(), *bmB = S::bm() + n;
-    double *sE = S::E();   // E[n] covers exactly the two bitmaps (2 n words)
-
-    // ---- stage the cell: momenta and pids; clear the bitmaps and the duplicate counters ---------
-    long long esum = 0;
-#pragma unroll
-    for (int g = 0; g < NG; ++g) {
-        if ((uint32_t)(g * G * THREADS) >= n) break;
-        double a[G], b[G], cc[G];
-        uint32_t id[G];
-#pragma unroll
-        for (int i = 0; i < G; ++i) {
-            const uint32_t jc = lo + min((uint32_t)(tid + (g * G + i) * THREADS), last);
-            a[i] = P.px[jc]; b[i] = P.py[jc]; cc[i] = P.pz[jc]; id[i] = P.pid[jc];
-        }
-#pragma unroll
-        for (int i = 0; i < G; ++i) {
-            const uint32_t j = tid + (g * G + i) * THREADS;
-            if (j < n) {
-                S::pxy()[j] = make_double2(a[i], b[i]); S::pz()[j] = cc[i]; S::pid()[j] = id[i];
-                *reinterpret_cast<uint2 *>(S::bm() + 2 * j) = make_uint2(0u, 0u); S::cnt()[j] = 0;
-                if (local) esum += energy_fixed(energy(a[i], b[i], cc[i]));
-            }
-        }
-    }
-    if (hist)
-        for (uint32_t e = tid; e < ((lo + n - 1u) / kTile - lo / kTile + 1u) * kDirs; e += THREADS) s_seg[e] = 0;
-    if (local) block_sum_ll_post<THREADS>(esum, s_esum);
-    __syncthreads();
-    if (local) {
-        base = local_base(block_sum_ll_read<THREADS>(s_esum), n, P.dt, P.etas);
-        const double pmax = (2.0 * cn) * base;
-        if (!(pmax <= 64.0)) { if (tid == 0) atomicOr(P.flags, kFlagRounds); R = 64; }
-        else R = (pmax <= 1.0) ? 1 : (int)ceil(pmax);
-        if (n < 2u) R = 0;
-        if (tid == 0) {             // read in the pair phases, several barriers from here
-            const double scale = (cn * base) / (double)R;
-            stats->scale = scale; stats->hscale = 0.5 * scale;
-        }
-    }
-    // the CTA's next cell goes to L2 while this one is processed, so its load phase does not wait on DRAM
-    for (uint32_t l = tid * 16u; n_next && l < n_next + 16u; l += THREADS * 16u) {   // one 128 B line of doubles per thread
-        const uint32_t e = lo_next + min(l, n_next - 1u);
-        prefetch_l2(P.px + e); prefetch_l2(P.py + e); prefetch_l2(P.pz + e);
-        if ((l & 16u) == 0) prefetch_l2(P.pid + e);
-        if (hist) { prefetch_l2(P.x + e); prefetch_l2(P.y + e); prefetch_l2(P.z + e); }
-    }
-
     uint32_t warp_hits = 0;
     for (int rho0 = 0; rho0 < R; rho0 += 2) {
         const bool two = rho0 + 1 < R;
@@ -963,6 +890,98 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
             warp_hits += pair_phase<S, THREADS, PITEMS, TRACE>(P, c, n, tcur, rho0 + sl, sl, sl == 0, sl == 0 ? (two || hist) : hist, stats);
         }
     }
+    return warp_hits;
+}
+
+template <int THREADS, int ITEMS, int G, int CAP, int LCAP, bool TRACE, bool LOCAL, bool GRAPH>
+__device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32_t c, uint32_t lo, uint32_t n,
+                                                  uint32_t *s_warp, CtaStats *stats,
+                                                  uint32_t *s_seg, long long *s_esum, ThreadStats &acc,
+                                                  uint32_t lo_next, uint32_t n_next)
+{
+    static_assert(ITEMS % G == 0, "items are processed in groups of G");
+    constexpr int NG = ITEMS / G;
+    constexpr int PITEMS = (ITEMS + 1) / 2;          // pairs per thread
+    constexpr int SCAN = ITEMS | 1;                  // words per thread in the scan (odd stride: no bank conflicts)
+    using S = CellSmem<CAP, LCAP>;
+    const int tid = threadIdx.x;
+    // step index: a constant-bank operand normally; a register loaded from device memory when the
+    // kernel is a node of a replayed CUDA graph (small problems only, where registers are plentiful)
+    const uint32_t tcur = GRAPH ? *P.t_dev : P.t;
+    const bool hist = P.next_dt > 0.0;
+    constexpr bool local = LOCAL;     // compile-time: the constant-sigma kernels carry none of its registers
+    // rounds and scale (A5, A6): identical integer/fp64 results on every thread.  With the local
+    // cross section the factor needs the cell's energy sum and is computed after staging.
+    double base = P.base;
+    const double cn = (n & 1u) ? (double)n : (double)(n - 1u);
+    int R = 0;
+    if (!local) {
+        const double pmax = (2.0 * cn) * base;
+        if (!(pmax <= 64.0)) { if (tid == 0) atomicOr(P.flags, kFlagRounds); R = 64; }
+        else R = (pmax <= 1.0) ? 1 : (int)ceil(pmax);
+        if (n < 2u) R = 0;          // a single particle has no partner; it is here for the fused histogram only
+    }
+    for (int e = tid; e < 2 * kChains; e += THREADS) (&stats->head[0][0])[e] = kNil;
+    if (tid == 0) {
+        stats->lo = lo;
+        stats->nlist[0] = 0; stats->nlist[1] = 0;
+        if (!local) {
+            const double scale = (cn * base) / (double)R;
+            stats->scale = scale; stats->hscale = 0.5 * scale;
+        }
+    }
+    if (hist && tid < 32) hist_cell_setup(P.g, c, &stats->h, tid);
+    const uint32_t last = n - 1u;
+    const uint32_t M = 32u * n;                      // bits of a bitmap: word = bit >> 5 < n
+    uint32_t *bmA = S::bm(), *bmB = S::bm() + n;
+    double *sE = S::E();   // E[n] covers exactly the two bitmaps (2 n words)
+
+    // ---- stage the cell: momenta and pids; clear the bitmaps and the duplicate counters ---------
+    long long esum = 0;
+#pragma unroll
+    for (int g = 0; g < NG; ++g) {
+        if ((uint32_t)(g * G * THREADS) >= n) break;
+        double a[G], b[G], cc[G];
+        uint32_t id[G];
+#pragma unroll
+        for (int i = 0; i < G; ++i) {
+            const uint32_t jc = lo + min((uint32_t)(tid + (g * G + i) * THREADS), last);
+            a[i] = P.px[jc]; b[i] = P.py[jc]; cc[i] = P.pz[jc]; id[i] = P.pid[jc];
+        }
+#pragma unroll
+        for (int i = 0; i < G; ++i) {
+            const uint32_t j = tid + (g * G + i) * THREADS;
+            if (j < n) {
+                S::pxy()[j] = make_double2(a[i], b[i]); S::pz()[j] = cc[i]; S::pid()[j] = id[i];
+                *reinterpret_cast<uint2 *>(S::bm() + 2 * j) = make_uint2(0u, 0u); S::cnt()[j] = 0;
+                if (local) esum += energy_fixed(energy(a[i], b[i], cc[i]));
+            }
+        }
+    }
+    if (hist)
+        for (uint32_t e = tid; e < ((lo + n - 1u) / kTile - lo / kTile + 1u) * kDirs; e += THREADS) s_seg[e] = 0;
+    if (local) block_sum_ll_post<THREADS>(esum, s_esum);
+    __syncthreads();
+    if (local) {
+        base = local_base(block_sum_ll_read<THREADS>(s_esum), n, P.dt, P.etas);
+        const double pmax = (2.0 * cn) * base;
+        if (!(pmax <= 64.0)) { if (tid == 0) atomicOr(P.flags, kFlagRounds); R = 64; }
+        else R = (pmax <= 1.0) ? 1 : (int)ceil(pmax);
+        if (n < 2u) R = 0;
+        if (tid == 0) {             // read in the pair phases, several barriers from here
+            const double scale = (cn * base) / (double)R;
+            stats->scale = scale; stats->hscale = 0.5 * scale;
+        }
+    }
+    // the CTA's next cell goes to L2 while this one is processed, so its load phase does not wait on DRAM
+    for (uint32_t l = tid * 16u; n_next && l < n_next + 16u; l += THREADS * 16u) {   // one 128 B line of doubles per thread
+        const uint32_t e = lo_next + min(l, n_next - 1u);
+        prefetch_l2(P.px + e); prefetch_l2(P.py + e); prefetch_l2(P.pz + e);
+        if ((l & 16u) == 0) prefetch_l2(P.pid + e);
+        if (hist) { prefetch_l2(P.x + e); prefetch_l2(P.y + e); prefetch_l2(P.z + e); }
+    }
+
+    const uint32_t warp_hits = run_sweeps<THREADS, ITEMS, G, CAP, LCAP, TRACE>(P, c, n, R, tcur, hist, s_warp, stats);
     if (R == 0 && hist && tid == 0) {     // a lone particle: no pair phase has computed its energy
         const double2 xy = S::pxy()[0];
         sE[0] = energy(xy.x, xy.y, S::pz()[0]);
