@@ -150,6 +150,18 @@ int cuba_step_adaptive(cuba_ctx *ctx, int nsteps, double dt_max, double sigma, d
  * can be captured (not the legacy default stream or cudaStreamPerThread) and per-kernel profiling
  * is off.  value 0: plain launches.  Results are identical either way. */
 #define CUBA_OPT_GRAPH 2
+/* CUBA_OPT_SLOTS (default 1): schedule of cuba_step.  1: a call of at least 4 steps on a problem that is
+ * not launch-bound runs on the slotted store (one kernel per step and size class);
+ * 2: every call does; 0: never (the compact schedule: histogram, scan, scatter, collide).  The
+ * slotted store is device memory allocated by the library on first use (two copies of
+ * ncells * slots-per-cell * 52 bytes) and freed by cuba_destroy; if the allocation fails the compact
+ * schedule runs.  Results are bit-identical for every setting. */
+#define CUBA_OPT_SLOTS 3
+/* CUBA_OPT_SLOT_MARGIN (default 100): per cent by which the segment capacities of the slotted store
+ * are scaled, 1..1000.  A run that outgrows a capacity is detected at the next synchronising call and
+ * redone on the compact schedule from the state it started from; small values exist to test that.
+ * Synchronises if a slotted run is still unverified; releases the slotted store. */
+#define CUBA_OPT_SLOT_MARGIN 4
 int cuba_set_option(cuba_ctx *ctx, int option, int value);
 
 /* PAPER.md:66 (total energy) and PAPER.md:68-70 Fig. 2 (energy density along x).
@@ -209,7 +221,7 @@ int cuba_run_host(const double box[3], const int ncell[3], int64_t n,
  * Mode 1 times the collision kernels as one group (the size classes run concurrently on
  * internal streams, as in normal operation); mode 2 serialises them on the caller's stream and
  * times every class by itself (diagnostic: slower than normal operation); 0 switches off. */
-#define CUBA_PROFILE_GROUPS 17
+#define CUBA_PROFILE_GROUPS 21
 int cuba_profile_enable(cuba_ctx *ctx, int on);
 int cuba_profile_read(cuba_ctx *ctx, double *ms_sum, uint64_t *launches);
 const char *cuba_profile_name(int group);

@@ -18,6 +18,11 @@ EXPORTS = ("cuba_workspace_bytes", "cuba_init", "cuba_step", "cuba_observables",
            "cuba_step_adaptive", "cuba_step_local_sigma")
 
 
+# cuba_set_option
+OPT_FUSE_HIST, OPT_GRAPH, OPT_SLOTS, OPT_SLOT_MARGIN = 1, 2, 3, 4
+PROFILE_GROUPS = 21   # CUBA_PROFILE_GROUPS
+
+
 class CubaError(RuntimeError):
     def __init__(self, code, detail=""):
         self.code = code
@@ -260,7 +265,7 @@ class Cuba:
         return T, lrf
 
     def set_option(self, option: int, value: int):
-        """cuba_set_option (OPT_FUSE_HIST = 1)."""
+        """cuba_set_option (OPT_FUSE_HIST, OPT_GRAPH, OPT_SLOTS, OPT_SLOT_MARGIN)."""
         _check(lib().cuba_set_option(self._h, int(option), int(value)))
 
     def profile_enable(self, mode=1):
@@ -269,7 +274,7 @@ class Cuba:
 
     def profile_read(self):
         """{kernel group: (summed device ms, launches)} since profile_enable."""
-        G = 17
+        G = PROFILE_GROUPS
         ms = (c_double * G)()
         cnt = (c_uint64 * G)()
         _check(lib().cuba_profile_read(self._h, ms, cnt))

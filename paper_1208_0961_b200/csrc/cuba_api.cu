@@ -6,6 +6,7 @@
 #include <atomic>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -17,6 +18,7 @@
 #include "common.cuh"
 #include "init_sort.cuh"
 #include "observe.cuh"
+#include "slots.cuh"
 
 using namespace cuba;
 
@@ -139,6 +141,28 @@ struct cuba_ctx {
     uint64_t graph_kernels = 0;             // kernel launches one replay stands for (cuba_launch_count)
     bool fuse_hist = true;   // CUBA_OPT_FUSE_HIST
     double pre_dt = 0.0;     // > 0: cnt / carry already hold the histogram of the next step for this dt
+    // ---- slotted schedule (slots.cuh): one kernel per step on a store with a fixed region per cell ----
+    int slot_mode = 1;            // CUBA_OPT_SLOTS: 0 never, 1 for calls of >= kSlotMinSteps steps, 2 for every call
+    double slot_margin = 1.0;     // CUBA_OPT_SLOT_MARGIN (percent): scales the segment capacities (tests force overflows)
+    double slot_boost = 1.0;      // grows after an overflow so that the next geometry is roomier
+    unsigned char *slot_mem = nullptr;   // library-owned device memory: two slotted copies + the counter backup
+    size_t slot_bytes = 0;
+    SlotGeom slot_geom{};
+    SlotStore slot_st[2]{};
+    unsigned char *slot_backup = nullptr;  // counters (64 B), max_occ (8 B), flags (4 B) at the start of the pending run
+    uint32_t slot_nmax = 0;       // what the geometry was sized for
+    double slot_dt = 0.0;
+    int grid_slot[kSmemClasses] = {};
+    bool slot_grids = false;
+    bool slot_unavailable = false;   // the allocation failed once: stay on the compact path
+    uint64_t slot_runs = 0, slot_replays = 0;
+    // an enqueued slotted run whose overflow flag has not been read back yet: the compact copy it started
+    // from is untouched (the run packs into the other copy), so it can be redone on the compact path
+    bool pend = false;
+    int pend_cur = 0, pend_n = 0;
+    uint32_t pend_t = 0;
+    uint64_t pend_steps = 0;
+    double pend_dt = 0.0, pend_sigma = 0.0;
     int prof_mode = 0;   // 0 off, 1 events per kernel (collision classes as one concurrent group), 2 classes serialised
     bool prof_on = false;
     std::vector<cudaEvent_t> prof_pool;          // reused events
@@ -204,8 +228,9 @@ static int sync_and_check(cuba_ctx *ctx)
     return device_flags_to_error(f);
 }
 
-enum { G_MEMSET = 0, G_STREAM_HIST, G_GATHER, G_SCAN, G_CELL_START, G_CARRY, G_DEST_BASE, G_SCATTER, G_COLLIDE_ALL, G_COLLIDE0 };
-static_assert(G_COLLIDE0 + kNumClasses == CUBA_PROFILE_GROUPS, "profile groups");
+enum { G_MEMSET = 0, G_STREAM_HIST, G_GATHER, G_SCAN, G_CELL_START, G_CARRY, G_DEST_BASE, G_SCATTER, G_COLLIDE_ALL, G_COLLIDE0,
+       G_SLOT_UNPACK = G_COLLIDE0 + kNumClasses, G_SLOT_CLASSIFY, G_SLOT_STEP, G_SLOT_PACK, G_END };
+static_assert(G_END == CUBA_PROFILE_GROUPS, "profile groups");
 
 static void prof_mark(cuba_ctx *ctx, int group)
 {
@@ -300,6 +325,8 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
     if (rc == CUBA_OK) rc = occupancy_grid(k_scatter<true>, kTileThreads, 2 * sizeof(TileStage<7>), sms, &ctx->grid_scat);
     if (rc == CUBA_OK) rc = occupancy_grid(k_scatter<false>, kTileThreads, 2 * sizeof(TileStage<7>), sms, &ctx->grid_scat);
     if (rc != CUBA_OK) return fail(rc);
+    if (const char *e = getenv("CUBA_DEBUG_GRID_C4")) ctx->grid_cls[4] = atoi(e) * sms;      // experiments only
+    if (const char *e = getenv("CUBA_DEBUG_GRID_SCAT")) ctx->grid_scat = atoi(e) * sms;
     ctx->grid_o = sms;
     if (!cuda_ok(cudaFuncSetAttribute(k_observe_partial<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       kObsWarps * kObsMaxSlabs * 8), "cudaFuncSetAttribute")) return fail(CUBA_ERR_CUDA);
@@ -372,6 +399,7 @@ void cuba_destroy(cuba_ctx *ctx)
     if (!ctx) return;
     cudaStreamSynchronize(ctx->stream);
     if (ctx->graph_exec) cudaGraphExecDestroy(ctx->graph_exec);
+    if (ctx->slot_mem) cudaFree(ctx->slot_mem);
     if (ctx->h_obs) cudaFreeHost(ctx->h_obs);
     if (ctx->h_u32) cudaFreeHost(ctx->h_u32);
     for (int k = 0; k < kNumClasses; ++k) {
@@ -589,6 +617,251 @@ static int graph_capture(cuba_ctx *ctx, double dt, double sigma, double base)
     return CUBA_OK;
 }
 
+
+// ---- slotted schedule (slots.cuh) ---------------------------------------------------------------
+// A call of cuba_step with enough steps converts the compact store into the slotted one (k_slot_unpack),
+// runs the steps as one kernel per step and size class (k_slot_step), and converts back (k_slot_pack)
+// into the OTHER compact copy.  The copy the run started from is left untouched until the run has been
+// verified (no segment overflowed: kFlagSlots clear) at the next synchronising call; if the flag is
+// set the run is redone from that copy on the compact path -- the results never depend on the
+// capacities.  All of it is stream-ordered; only the verification synchronises.
+constexpr int kSlotMinSteps = 4;        // below this the two conversion passes cost more than they save
+constexpr size_t kSlotBackupBytes = 128;
+
+// Capacities of the 27 inbox segments for cells of up to nmax particles and time step dt.  A massless
+// particle moves dt in a step, so the share of a cell that leaves through a face is 1/4 dt/d for an
+// isotropic distribution (dt/d if everything flies the same way), through an edge or a corner the
+// product of two or three such factors.  Sized for twice the isotropic share plus six standard
+// deviations plus a constant; the stay segment for nmax plus an eighth.  An overflow is not an
+// error (see above), only slow.
+static SlotGeom slot_geometry(const cuba_ctx *ctx, uint32_t nmax, double dt, double margin)
+{
+    SlotGeom sg{};
+    double r[3];
+    for (int k = 0; k < 3; ++k) r[k] = dt * ctx->g.inv_d[k];
+    uint32_t off = 0;
+    for (int s = 0; s < kDirs; ++s) {
+        const int o[3] = {s / 9 - 1, (s / 3) % 3 - 1, s % 3 - 1};
+        int m = 0;
+        double frac = 1.0;
+        for (int k = 0; k < 3; ++k) if (o[k] != 0) { ++m; frac *= r[k]; }
+        double want;
+        if (m == 0) want = 1.125 * (double)nmax + 64.0;
+        else {
+            const double mean = (m == 1 ? 0.5 : (m == 2 ? 0.25 : 0.125)) * frac * (double)nmax;
+            want = mean + 6.0 * std::sqrt(mean) + (m == 1 ? 16.0 : 8.0);
+        }
+        uint32_t cap = (uint32_t)std::ceil(want * margin);
+        cap = std::max(cap, 4u);
+        cap = (cap + 3u) / 4u * 4u;                      // 32-byte sectors of the fp64 arrays
+        if (s == (int)kDirStay) off = (off + 15u) / 16u * 16u;   // the big segment starts on a 128-byte line
+        sg.seg_off[s] = off;
+        off += cap;
+    }
+    sg.seg_off[kDirs] = off;
+    sg.slots = (off + 15u) / 16u * 16u;
+    return sg;
+}
+
+static void slot_release(cuba_ctx *ctx)
+{
+    if (ctx->slot_mem) cudaFree(ctx->slot_mem);
+    ctx->slot_mem = nullptr; ctx->slot_bytes = 0; ctx->slot_nmax = 0; ctx->slot_dt = 0.0;
+}
+
+// Make sure a slotted store fit for (nmax, dt) exists.  Returns false (and leaves the compact path in
+// charge) when it cannot be had.
+static bool slot_prepare(cuba_ctx *ctx, uint32_t nmax, double dt)
+{
+    if (ctx->slot_unavailable) return false;
+    const double margin = ctx->slot_margin * ctx->slot_boost;
+    if (ctx->slot_mem && nmax <= ctx->slot_nmax && dt <= ctx->slot_dt) return true;
+    slot_release(ctx);
+    const uint32_t size_n = nmax + nmax / 16u;             // a little head room so that small fluctuations do not reallocate
+    const SlotGeom sg = slot_geometry(ctx, size_n, dt, margin);
+    const uint64_t total_slots = (uint64_t)ctx->g.ncells * sg.slots;
+    if (total_slots >= (1ull << 32)) { ctx->slot_unavailable = true; return false; }
+    const size_t arr8 = align_up((size_t)total_slots * 8), arr4 = align_up((size_t)total_slots * 4);
+    const size_t cntb = align_up((size_t)ctx->g.ncells * kDirs * 4);
+    const size_t per_copy = 6 * arr8 + arr4 + cntb;
+    const size_t bytes = 2 * per_copy + kSlotBackupBytes;
+    void *mem = nullptr;
+    if (cudaMalloc(&mem, bytes) != cudaSuccess) {
+        cudaGetLastError();                                // not an error of the step
+        ctx->slot_unavailable = true;
+        return false;
+    }
+    ctx->slot_mem = static_cast<unsigned char *>(mem);
+    ctx->slot_bytes = bytes;
+    for (int c = 0; c < 2; ++c) {
+        unsigned char *b = ctx->slot_mem + (size_t)c * per_copy;
+        SlotStore &st = ctx->slot_st[c];
+        double **arr[6] = {&st.x, &st.y, &st.z, &st.px, &st.py, &st.pz};
+        for (int k = 0; k < 6; ++k) *arr[k] = reinterpret_cast<double *>(b + (size_t)k * arr8);
+        st.pid = reinterpret_cast<uint32_t *>(b + 6 * arr8);
+        st.cnt = reinterpret_cast<uint32_t *>(b + 6 * arr8 + arr4);
+        // counts of segments whose source cell lies outside the box are never written: they stay zero
+        if (cudaMemsetAsync(st.cnt, 0, cntb, ctx->stream) != cudaSuccess) { cudaGetLastError(); slot_release(ctx); ctx->slot_unavailable = true; return false; }
+    }
+    ctx->slot_backup = ctx->slot_mem + 2 * per_copy;
+    ctx->slot_geom = sg;
+    ctx->slot_nmax = size_n;
+    ctx->slot_dt = dt;
+    return true;
+}
+
+static int slot_grids(cuba_ctx *ctx)
+{
+    if (ctx->slot_grids) return CUBA_OK;
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    int rc = CUBA_OK;
+#define CUBA_OCC(K, T, I, C, MB) \
+    if (rc == CUBA_OK) rc = occupancy_grid(k_slot_step<T, I, C, MB, kSlotFirst>, T, collide_smem_bytes(C, T, I), sms, &ctx->grid_slot[K]); \
+    if (rc == CUBA_OK) rc = occupancy_grid(k_slot_step<T, I, C, MB, kSlotLast>, T, collide_smem_bytes(C, T, I), sms, &ctx->grid_slot[K]); \
+    if (rc == CUBA_OK) rc = occupancy_grid(k_slot_step<T, I, C, MB, kSlotMiddle>, T, collide_smem_bytes(C, T, I), sms, &ctx->grid_slot[K]);
+    CUBA_FOR_EACH_CLASS(CUBA_OCC)
+#undef CUBA_OCC
+    if (rc == CUBA_OK) ctx->slot_grids = true;
+    return rc;
+}
+
+// nsteps steps on the slotted store, from and back to the compact one: nsteps + 1 passes (slots.cuh).
+// Preconditions: no pending run, slot_prepare() succeeded.
+static int slot_run(cuba_ctx *ctx, int nsteps, double dt, double sigma, double base)
+{
+    const Layout &lay = ctx->lay;
+    cudaStream_t main = ctx->stream;
+    const uint32_t ncells = ctx->g.ncells;
+    int rc = slot_grids(ctx);
+    if (rc != CUBA_OK) return rc;
+    uint32_t *zero = ctx->at<uint32_t>(lay.zero);
+    uint32_t *flags = ctx->at<uint32_t>(lay.flags);
+    uint4 *lists = ctx->at<uint4>(lay.class_list);
+    uint32_t *cell_start = ctx->at<uint32_t>(lay.cell_start);
+    // what a replay needs: counters and flags as they are now, and where the state is
+    CU(cudaMemcpyAsync(ctx->slot_backup, ctx->at<void>(lay.counters), 64, cudaMemcpyDeviceToDevice, main));
+    CU(cudaMemcpyAsync(ctx->slot_backup + 64, ctx->at<void>(lay.max_occ), 8, cudaMemcpyDeviceToDevice, main));
+    CU(cudaMemcpyAsync(ctx->slot_backup + 72, flags, 4, cudaMemcpyDeviceToDevice, main));
+    ctx->pend = true; ctx->pend_cur = ctx->cur; ctx->pend_n = nsteps; ctx->pend_t = ctx->t; ctx->pend_steps = ctx->steps;
+    ctx->pend_dt = dt; ctx->pend_sigma = sigma;
+    ctx->slot_runs += 1;
+    ctx->pre_dt = 0.0;
+
+    ClassTable ct{};
+#define CUBA_CAP(K, T, I, C, MB) ct.max_n[K] = C;
+    CUBA_FOR_EACH_CLASS(CUBA_CAP)
+#undef CUBA_CAP
+    ct.max_n[kSmemClasses] = 0xFFFFFFFFu;
+
+    CollideParams P{};
+    P.seed = ctx->seed; P.base = base; P.g = ctx->g;
+    for (uint32_t r = 0; r < 10; ++r) {
+        P.rk[2 * r] = (uint32_t)ctx->seed + r * 0x9E3779B9u;
+        P.rk[2 * r + 1] = (uint32_t)(ctx->seed >> 32) + r * 0xBB67AE85u;
+    }
+    P.counters = ctx->at<unsigned long long>(lay.counters);
+    P.flags = flags;
+    SlotParams Q{};
+    Q.sg = ctx->slot_geom; Q.dt = dt;
+    const bool serial = ctx->prof_mode == 2;
+    const Soa &from = ctx->set[ctx->cur], &to = ctx->set[1 - ctx->cur];
+    const SlotStore compact_in{from.x, from.y, from.z, from.px, from.py, from.pz, from.pid, nullptr};
+    const SlotStore compact_out{to.x, to.y, to.z, to.px, to.py, to.pz, to.pid, nullptr};
+
+    // the size classes of one pass, forked onto their own streams
+    auto launch_pass = [&](int mode) -> int {
+        if (!serial) CU(cudaEventRecord(ctx->ev_fork, main));
+#define CUBA_LAUNCH(K, T, I, C, MB)                                                              \
+        {                                                                                        \
+            cudaStream_t st = serial ? main : ctx->cls_stream[K];                                \
+            if (!serial) CU(cudaStreamWaitEvent(st, ctx->ev_fork, 0));                           \
+            P.list = lists + (size_t)K * ncells; P.list_count = zero + K; P.work = zero + 8 + K; \
+            const size_t sm = collide_smem_bytes(C, T, I);                                       \
+            if (mode == kSlotFirst) k_slot_step<T, I, C, MB, kSlotFirst><<<ctx->grid_slot[K], T, sm, st>>>(P, Q); \
+            else if (mode == kSlotLast) k_slot_step<T, I, C, MB, kSlotLast><<<ctx->grid_slot[K], T, sm, st>>>(P, Q); \
+            else k_slot_step<T, I, C, MB, kSlotMiddle><<<ctx->grid_slot[K], T, sm, st>>>(P, Q);  \
+            LAUNCHED();                                                                          \
+            if (serial) prof_mark(ctx, G_COLLIDE0 + K);                                          \
+            else { CU(cudaEventRecord(ctx->ev_join[K], st)); CU(cudaStreamWaitEvent(main, ctx->ev_join[K], 0)); } \
+        }
+        CUBA_FOR_EACH_CLASS(CUBA_LAUNCH)
+#undef CUBA_LAUNCH
+        return CUBA_OK;
+    };
+
+    prof_mark(ctx, -1);
+    k_slot_init_counts<<<(ncells * kDirs + 255u) / 256u, 256, 0, main>>>(ncells, cell_start, ctx->slot_geom, ctx->slot_st[0].cnt);
+    LAUNCHED();
+    int par = 0;
+    for (int pass = 0; pass <= nsteps; ++pass) {
+        const int mode = pass == 0 ? kSlotFirst : (pass == nsteps ? kSlotLast : kSlotMiddle);
+        if (pass > 0) prof_mark(ctx, -1);
+        CU(cudaMemsetAsync(zero, 0, kZeroWords * 4, main));
+        k_slot_classify<<<(unsigned)lay.nblocks_cells, 256, 0, main>>>(ctx->g, ctx->slot_st[par].cnt, ctx->slot_st[1 - par].cnt, ct, zero, lists,
+                                                                         ctx->at<unsigned long long>(lay.max_occ), zero + kStepMaxWord, flags,
+                                                                         mode == kSlotFirst ? cell_start : nullptr);
+        LAUNCHED();
+        if (mode == kSlotLast) {
+            // collisions move nobody: the compact layout of the result is known before the last pass
+            k_slot_count<<<(unsigned)lay.nblocks_cells, 256, 0, main>>>(ncells, ctx->slot_st[par].cnt, ctx->at<uint32_t>(lay.count_new),
+                                                                          ctx->at<uint32_t>(lay.block_sum));
+            LAUNCHED();
+            k_scan_blocks<<<1, 1024, 0, main>>>(ctx->at<uint32_t>(lay.block_sum), (int)lay.nblocks_cells, zero, kZeroWords);
+            LAUNCHED();
+            k_cell_start<<<(unsigned)lay.nblocks_cells, 256, 0, main>>>(ncells, ctx->at<uint32_t>(lay.count_new), ctx->at<uint32_t>(lay.block_sum),
+                                                                          cell_start, ct, zero, lists,
+                                                                          ctx->at<unsigned long long>(lay.max_occ), zero + kStepMaxWord);
+            LAUNCHED();
+        }
+        prof_mark(ctx, G_SLOT_CLASSIFY);
+        P.t = ctx->t + (uint32_t)(pass > 0 ? pass - 1 : 0);
+        Q.in = mode == kSlotFirst ? compact_in : ctx->slot_st[par];
+        Q.out = mode == kSlotLast ? compact_out : ctx->slot_st[1 - par];
+        rc = launch_pass(mode);
+        if (rc != CUBA_OK) return rc;
+        if (!serial) prof_mark(ctx, mode == kSlotFirst ? G_SLOT_UNPACK : (mode == kSlotLast ? G_SLOT_PACK : G_SLOT_STEP));
+        par = 1 - par;
+    }
+    ctx->cur = 1 - ctx->cur;
+    ctx->t += (uint32_t)nsteps; ctx->steps += (uint64_t)nsteps; ctx->nmax_valid = false;
+    return CUBA_OK;
+}
+
+static int step_fixed(cuba_ctx *ctx, int nsteps, double dt, double sigma, double etas);
+static int read_step_max(cuba_ctx *ctx);
+
+// Verify a pending slotted run (see above).  Called at the start of every entry point that reads or
+// advances the state.  Synchronises only when a run is pending.
+static int settle(cuba_ctx *ctx)
+{
+    if (!ctx->pend) return CUBA_OK;
+    const Layout &lay = ctx->lay;
+    uint32_t *h = ctx->h_u32;
+    CU(cudaMemcpyAsync(h, ctx->at<uint32_t>(lay.flags), 4, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaMemcpyAsync(h + 1, ctx->at<uint32_t>(lay.zero) + kStepMaxWord, 4, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    ctx->pend = false;
+    if (!(h[0] & kFlagSlots)) {
+        ctx->nmax_cur = h[1]; ctx->nmax_valid = true;    // k_cell_start of the conversion recorded it
+        return CUBA_OK;
+    }
+    // a segment (or a cell) outgrew the layout: restore the starting point and redo the run on the compact path
+    ctx->slot_replays += 1;
+    ctx->slot_boost *= 1.5;
+    CU(cudaMemcpyAsync(ctx->at<void>(lay.counters), ctx->slot_backup, 64, cudaMemcpyDeviceToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->at<void>(lay.max_occ), ctx->slot_backup + 64, 8, cudaMemcpyDeviceToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(ctx->at<void>(lay.flags), ctx->slot_backup + 72, 4, cudaMemcpyDeviceToDevice, ctx->stream));
+    ctx->cur = ctx->pend_cur; ctx->t = ctx->pend_t; ctx->steps = ctx->pend_steps;
+    ctx->pre_dt = 0.0; ctx->nmax_valid = false;
+    const int mode = ctx->slot_mode;
+    ctx->slot_mode = 0;
+    const int rc = step_fixed(ctx, ctx->pend_n, ctx->pend_dt, ctx->pend_sigma, 0.0);
+    ctx->slot_mode = mode;
+    return rc;
+}
+
 // fixed time step; etas > 0 selects the local cross section (sigma is then unused)
 static int step_fixed(cuba_ctx *ctx, int nsteps, double dt, double sigma, double etas)
 {
@@ -596,6 +869,8 @@ static int step_fixed(cuba_ctx *ctx, int nsteps, double dt, double sigma, double
     if (nsteps < 0) return CUBA_ERR_SIZE;
     double base;
     int rc = check_step_args(ctx, dt, sigma, &base);
+    if (rc != CUBA_OK) return rc;
+    rc = settle(ctx);
     if (rc != CUBA_OK) return rc;
     int s = 0;
     auto plain = [&]() -> int {
@@ -607,6 +882,17 @@ static int step_fixed(cuba_ctx *ctx, int nsteps, double dt, double sigma, double
     // the legacy default stream (0, cudaStreamLegacy) and cudaStreamPerThread cannot be captured
     const bool graphable = ctx->use_graph && ctx->fuse_hist && !ctx->prof_on && etas == 0.0 && ctx->n <= kGraphMaxParticles &&
                            reinterpret_cast<uintptr_t>(ctx->stream) > 2;
+    // Slotted schedule: one kernel per step (slots.cuh).  Small problems are launch-bound and keep the graph.
+    if (etas == 0.0 && ctx->slot_mode != 0 && !ctx->capturing && nsteps >= (ctx->slot_mode == 2 ? 1 : kSlotMinSteps) &&
+        (ctx->slot_mode == 2 || !(graphable && nsteps >= 4))) {
+        if (!ctx->nmax_valid) { rc = read_step_max(ctx); if (rc != CUBA_OK) return rc; }
+        uint32_t cap_max = 0;
+#define CUBA_CAPMAX(K, T, I, C, MB) cap_max = cap_max > (uint32_t)C ? cap_max : (uint32_t)C;
+        CUBA_FOR_EACH_CLASS(CUBA_CAPMAX)
+#undef CUBA_CAPMAX
+        if (ctx->nmax_cur >= 1u && ctx->nmax_cur + ctx->nmax_cur / 8u <= cap_max && slot_prepare(ctx, ctx->nmax_cur, dt))
+            return slot_run(ctx, nsteps, dt, sigma, base);
+    }
     if (graphable && nsteps >= 4) {
         // reach the steady state the graph was captured in: histogram prepared for this dt, store in copy 0
         while (s < nsteps && !(ctx->pre_dt == dt && ctx->cur == 0)) { rc = plain(); if (rc != CUBA_OK) return rc; }
@@ -677,7 +963,8 @@ int cuba_step_adaptive(cuba_ctx *ctx, int nsteps, double dt_max, double sigma, d
     if (nsteps < 0) return CUBA_ERR_SIZE;
     if (!(dt_max > 0.0) || !std::isfinite(dt_max) || !(sigma >= 0.0) || !std::isfinite(sigma)) return CUBA_ERR_VALUE;
     double sum = 0.0;
-    int rc = CUBA_OK;
+    int rc = settle(ctx);
+    if (rc != CUBA_OK) { if (elapsed) *elapsed = 0.0; return rc; }
     if (nsteps > 0 && !ctx->nmax_valid) {      // the last binning's value is still on the device
         rc = read_step_max(ctx);
         if (rc != CUBA_OK) return rc;
@@ -716,6 +1003,8 @@ int cuba_step_traced(cuba_ctx *ctx, double dt, double sigma, cuba_trace *out)
                                    !out->u || !out->decided)) return CUBA_ERR_NULL;
     double base;
     int rc = check_step_args(ctx, dt, sigma, &base);
+    if (rc != CUBA_OK) return rc;
+    rc = settle(ctx);
     if (rc != CUBA_OK) return rc;
     const int64_t n = ctx->n;
     const uint32_t ncells = ctx->g.ncells;
@@ -796,6 +1085,19 @@ int cuba_step_traced(cuba_ctx *ctx, double dt, double sigma, cuba_trace *out)
 int cuba_set_option(cuba_ctx *ctx, int option, int value)
 {
     if (!ctx) return CUBA_ERR_NULL;
+    if (option == CUBA_OPT_SLOTS) {
+        if (value < 0 || value > 2) return CUBA_ERR_VALUE;
+        ctx->slot_mode = value;
+        return CUBA_OK;
+    }
+    if (option == CUBA_OPT_SLOT_MARGIN) {
+        if (value < 1 || value > 1000) return CUBA_ERR_VALUE;
+        ctx->slot_margin = (double)value / 100.0;
+        ctx->slot_boost = 1.0;
+        const int rs = settle(ctx);
+        slot_release(ctx);
+        return rs;
+    }
     if ((option != CUBA_OPT_FUSE_HIST && option != CUBA_OPT_GRAPH) || (value != 0 && value != 1)) return CUBA_ERR_VALUE;
     if (option == CUBA_OPT_GRAPH) { ctx->use_graph = value != 0; return CUBA_OK; }
     ctx->fuse_hist = value != 0;
@@ -807,6 +1109,7 @@ int cuba_observables(cuba_ctx *ctx, double total[4], int nslab, double *edens)
 {
     if (!ctx || !total || !edens) return CUBA_ERR_NULL;
     if (nslab < 1 || nslab > kObsMaxSlabs) return CUBA_ERR_SIZE;
+    { const int rs = settle(ctx); if (rs != CUBA_OK) return rs; }
     const Layout &lay = ctx->lay;
     const Soa &cur = ctx->set[ctx->cur];
     cudaStream_t st = ctx->stream;
@@ -830,6 +1133,7 @@ int cuba_observables_lrf(cuba_ctx *ctx, int nslab, double *T, double *lrf)
 {
     if (!ctx || !T || !lrf) return CUBA_ERR_NULL;
     if (nslab < 1 || nslab > kLrfMaxSlabs) return CUBA_ERR_SIZE;
+    { const int rs = settle(ctx); if (rs != CUBA_OK) return rs; }
     const Layout &lay = ctx->lay;
     const Soa &cur = ctx->set[ctx->cur];
     cudaStream_t st = ctx->stream;
@@ -854,6 +1158,7 @@ int cuba_observables_lrf(cuba_ctx *ctx, int nslab, double *T, double *lrf)
 int cuba_state(cuba_ctx *ctx, cuba_soa *out)
 {
     if (!ctx || !out) return CUBA_ERR_NULL;
+    { const int rs = settle(ctx); if (rs != CUBA_OK) return rs; }
     const Soa &c = ctx->set[ctx->cur];
     out->x = c.x; out->y = c.y; out->z = c.z; out->px = c.px; out->py = c.py; out->pz = c.pz;
     out->pid = c.pid;
@@ -865,7 +1170,9 @@ int cuba_get_particles(cuba_ctx *ctx, uint32_t *pid, double *x, double *y, doubl
                        double *px, double *py, double *pz)
 {
     if (!ctx) return CUBA_ERR_NULL;
-    int rc = sync_and_check(ctx);
+    int rc = settle(ctx);
+    if (rc != CUBA_OK) return rc;
+    rc = sync_and_check(ctx);
     if (rc != CUBA_OK) return rc;
     const Soa &c = ctx->set[ctx->cur];
     const size_t b = (size_t)ctx->n * 8;
@@ -890,6 +1197,10 @@ const char *cuba_profile_name(int group)
     CUBA_FOR_EACH_CLASS(CUBA_NAME)
 #undef CUBA_NAME
     names[G_COLLIDE0 + kSmemClasses] = "k_collide_overflow";
+    names[G_SLOT_UNPACK] = "k_slot_step<first> (stream from the compact store)";
+    names[G_SLOT_CLASSIFY] = "k_slot_classify";
+    names[G_SLOT_STEP] = "k_slot_step (all classes, concurrent)";
+    names[G_SLOT_PACK] = "k_slot_step<last> (collide into the compact store)";
     return (group >= 0 && group < CUBA_PROFILE_GROUPS) ? names[group] : "?";
 }
 
@@ -925,7 +1236,9 @@ int cuba_profile_read(cuba_ctx *ctx, double *ms_sum, uint64_t *launches)
 int cuba_get_cells(cuba_ctx *ctx, uint32_t *cell_start)
 {
     if (!ctx || !cell_start) return CUBA_ERR_NULL;
-    int rc = sync_and_check(ctx);
+    int rc = settle(ctx);
+    if (rc != CUBA_OK) return rc;
+    rc = sync_and_check(ctx);
     if (rc != CUBA_OK) return rc;
     CU(cudaMemcpy(cell_start, ctx->at<uint32_t>(ctx->lay.cell_start), ((size_t)ctx->g.ncells + 1) * 4, cudaMemcpyDeviceToHost));
     return CUBA_OK;
@@ -937,6 +1250,7 @@ int cuba_counters(cuba_ctx *ctx, cuba_counters_t *out)
     unsigned long long c[8] = {0};
     unsigned long long mo = 0;
     uint32_t f = 0;
+    { const int rs = settle(ctx); if (rs != CUBA_OK) return rs; }
     CU(cudaStreamSynchronize(ctx->stream));
     CU(cudaMemcpy(c, ctx->at<void>(ctx->lay.counters), 64, cudaMemcpyDeviceToHost));
     CU(cudaMemcpy(&mo, ctx->at<void>(ctx->lay.max_occ), 8, cudaMemcpyDeviceToHost));
