@@ -202,6 +202,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-fuse", action="store_true", help="run the separate k_stream_hist pass every step (A/B diagnostic)")
+    ap.add_argument("--slots", type=int, default=-1, help="CUBA_OPT_SLOTS: 0 compact schedule, 1/2 slotted schedule; -1 library default (A/B diagnostic)")
     ap.add_argument("--profile-mode", type=int, default=1, help="1: normal operation; 2: serialise the collision classes (diagnostic)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuba" else args.warmup
@@ -240,6 +241,8 @@ def main():
     n = w.n
     fused = not args.no_fuse
     sim.set_option(1, 1 if fused else 0)
+    if args.slots >= 0:
+        sim.set_option(3, args.slots)
     bytes_collide = BYTES_COLLIDE_FUSED if fused else BYTES_COLLIDE
 
     sampler = ClockSampler(local)

@@ -226,6 +226,15 @@ int cuba_profile_enable(cuba_ctx *ctx, int on);
 int cuba_profile_read(cuba_ctx *ctx, double *ms_sum, uint64_t *launches);
 const char *cuba_profile_name(int group);
 
+/* fp64 leg of the roofline (fp64-pipe utilisation against a measured peak; no passage of
+ * the paper: a timing probe).  Launches a kernel of dependent DFMA chains (8 per thread, 8 x SM count
+ * CTAs of 256 threads) `repeats` times (1..64) after one warm-up on `cuda_stream` (a cudaStream_t, may
+ * be null = default stream), times each with CUDA events and writes the best rate to the HOST double
+ * *dfma_per_s: thread-level fp64 FMA instructions per second of the whole device (x 2 = FLOP/s,
+ * / 32 = warp instructions/s).  Allocates and frees its own small device buffer; synchronises.
+ * Errors: CUBA_ERR_NULL, CUBA_ERR_SIZE, CUBA_ERR_CUDA (*dfma_per_s = 0). */
+int cuba_probe_fp64(void *cuda_stream, int repeats, double *dfma_per_s);
+
 void cuba_destroy(cuba_ctx *ctx);
 const char *cuba_strerror(int code);
 /* Text of the last CUDA runtime error seen by this library in the calling process. */

@@ -6,9 +6,9 @@ There is no CPU fallback: importing works anywhere (so the ABI can be inspected)
 compute call needs the built library and a CUDA device and fails loudly otherwise.
 """
 from .binding import (Cuba, CubaError, Counters, Trace, lib, lib_path, run_host,  # noqa: F401
-                      workspace_bytes, launch_count, strerror, EXPORTS,
+                      workspace_bytes, launch_count, probe_fp64, strerror, EXPORTS,
                       OPT_FUSE_HIST, OPT_GRAPH, OPT_SLOTS, OPT_SLOT_MARGIN)
 
 __all__ = ["Cuba", "CubaError", "Counters", "Trace", "lib", "lib_path", "run_host",
-           "workspace_bytes", "launch_count", "strerror", "EXPORTS",
+           "workspace_bytes", "launch_count", "probe_fp64", "strerror", "EXPORTS",
            "OPT_FUSE_HIST", "OPT_GRAPH", "OPT_SLOTS", "OPT_SLOT_MARGIN"]

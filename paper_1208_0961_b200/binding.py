@@ -15,7 +15,7 @@ EXPORTS = ("cuba_workspace_bytes", "cuba_init", "cuba_step", "cuba_observables",
            "cuba_get_particles", "cuba_get_cells", "cuba_step_traced", "cuba_counters", "cuba_run_host", "cuba_destroy",
            "cuba_strerror", "cuba_last_cuda_error", "cuba_launch_count", "cuba_profile_enable",
            "cuba_profile_read", "cuba_profile_name", "cuba_set_option", "cuba_observables_lrf",
-           "cuba_step_adaptive", "cuba_step_local_sigma")
+           "cuba_step_adaptive", "cuba_step_local_sigma", "cuba_probe_fp64")
 
 
 # cuba_set_option
@@ -114,6 +114,7 @@ def lib():
         L.cuba_step_adaptive.argtypes = [c_void_p, c_int, c_double, c_double, dp, dp]
         L.cuba_step_local_sigma.argtypes = [c_void_p, c_int, c_double, c_double]
         L.cuba_profile_read.argtypes = [c_void_p, dp, POINTER(c_uint64)]
+        L.cuba_probe_fp64.argtypes = [c_void_p, c_int, dp]
         L.cuba_profile_name.argtypes = [c_int]
         L.cuba_profile_name.restype = c_char_p
         _lib = L
@@ -147,6 +148,13 @@ def workspace_bytes(n, ncell) -> int:
 
 def launch_count() -> int:
     return int(lib().cuba_launch_count())
+
+
+def probe_fp64(stream=None, repeats=5) -> float:
+    """cuba_probe_fp64: measured thread-level fp64 FMA instructions per second of the device."""
+    v = c_double(0.0)
+    _check(lib().cuba_probe_fp64(c_void_p(stream) if stream else None, int(repeats), ctypes.byref(v)))
+    return float(v.value)
 
 
 def _np_ptr(a):

@@ -19,6 +19,7 @@
 #include "init_sort.cuh"
 #include "observe.cuh"
 #include "slots.cuh"
+#include "probe.cuh"
 
 using namespace cuba;
 
@@ -1231,6 +1232,38 @@ int cuba_profile_read(cuba_ctx *ctx, double *ms_sum, uint64_t *launches)
     for (auto &pe : ctx->prof_log) ctx->prof_pool.push_back(pe.first);
     ctx->prof_log.clear();
     return CUBA_OK;
+}
+
+// fp64 FMA micro-benchmark (probe.cuh): thread-level DFMA instructions per second of the whole device
+int cuba_probe_fp64(void *cuda_stream, int repeats, double *dfma_per_s)
+{
+    if (!dfma_per_s) return CUBA_ERR_NULL;
+    if (repeats < 1 || repeats > 64) return CUBA_ERR_SIZE;
+    *dfma_per_s = 0.0;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    int dev = 0, sms = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int grid = sms * 8, iters = 1 << 14;
+    double *out = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    CU(cudaMalloc(&out, (size_t)grid * kProbeThreads * sizeof(double)));
+    auto done = [&](int code) { if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); cudaFree(out); return code; };
+    if (!cuda_ok(cudaEventCreate(&e0), "cudaEventCreate") || !cuda_ok(cudaEventCreate(&e1), "cudaEventCreate")) return done(CUBA_ERR_CUDA);
+    double best = 0.0;
+    for (int r = 0; r <= repeats; ++r) {       // the first launch warms up
+        cudaEventRecord(e0, st);
+        k_probe_fp64<<<grid, kProbeThreads, 0, st>>>(iters, 0.999999, 1e-6, out);
+        LAUNCHED();
+        cudaEventRecord(e1, st);
+        if (!cuda_ok(cudaEventSynchronize(e1), "cudaEventSynchronize")) return done(CUBA_ERR_CUDA);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double rate = (double)grid * kProbeThreads * kProbeChains * (double)iters / ((double)ms * 1e-3);
+        if (r > 0 && rate > best) best = rate;
+    }
+    *dfma_per_s = best;
+    return done(CUBA_OK);
 }
 
 int cuba_get_cells(cuba_ctx *ctx, uint32_t *cell_start)
