@@ -43,19 +43,62 @@ BYTES_STEP = BYTES_STREAM_HIST + BYTES_SCATTER + BYTES_COLLIDE   # 204, SURVEY.m
 BYTES_STEP_FUSED = BYTES_SCATTER + BYTES_COLLIDE_FUSED           # 180: what the fused schedule actually has to move
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
-# `ncu --set full` capture (profiles/r01_v4_summary.md): (config, fused schedule, kernel group) -> bytes.
-# The group is the hot collision class (1.487 + 0.508 GB) plus the cold one (0.138 + 0.029 GB).
-NCU_TRAFFIC = {(2, True, "k_collide (all classes, concurrent)"): 2.162e9}
-# smsp__inst_executed.sum (warp instructions) per step of the same kernel group from the same capture:
-# the collision kernels are bound by instruction issue and latency, not by HBM, so the line also says
-# how far they are from the issue peak of 148 SMs x 4 schedulers x 1 warp instruction per clock.
-NCU_WARP_INST = {(2, True, "k_collide (all classes, concurrent)"): 645.1e6}
+# ncu evidence: the raw per-launch metric export of one step under profiles/ (written by the command named in
+# the .md beside it), keyed by a hash of the kernel sources so that a stale capture reads as null, never as a
+# number.  Metrics: dram__bytes_read.sum, dram__bytes_write.sum, smsp__inst_executed.sum,
+# smsp__inst_executed_pipe_fp64.sum (warp-level), gpu__time_duration.sum, launch__registers_per_thread,
+# sm__warps_active.avg.pct_of_peak_sustained_active.
+NCU_EXPORT = os.path.join(ROOT, "profiles", "r02_ncu_step_c%d.csv")
 ISSUE_SLOTS_PER_CLOCK = 148 * 4
 
 
-def issue_roofline(warp_inst, ms, clocks):
-    """Secondary roofline of an issue-bound kernel: recorded warp instructions per launch / measured
+def kernel_source_hash():
+    """sha256 over the CUDA sources of the library (csrc/*.cu, *.cuh, sorted by name)."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_1208_0961_b200", "csrc", "*.cu*"))):
+        h.update(os.path.basename(f).encode())
+        with open(f, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
+
+
+def ncu_export(config):
+    """{kernel base name: {metric: summed value over the launches of ONE step}} from the tracked export, or
+    (None, why).  The first line of the file is '# source_sha256: <hash> ...'."""
+    path = NCU_EXPORT % config
+    if not os.path.exists(path):
+        return None, "no tracked ncu export for this config"
+    import csv
+    with open(path) as f:
+        lines = f.read().splitlines()
+    head = [l for l in lines if l.startswith("#")]
+    sha = next((l.split("source_sha256:")[1].split()[0] for l in head if "source_sha256:" in l), None)
+    if sha != kernel_source_hash():
+        return None, "stale: kernel sources changed since %s was captured" % os.path.relpath(path, ROOT)
+    rows = list(csv.DictReader([l for l in lines if l.startswith('"')]))
+    out = {}
+    for r in rows:
+        name = r["Kernel Name"].replace("void ", "").replace("cuba::", "")
+        base = name.split("<")[0].split("(")[0]
+        try:
+            v = float(r["Metric Value"].replace(",", ""))
+        except ValueError:
+            continue
+        unit = r["Metric Unit"]
+        scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0, "ms": 1e6, "us": 1e3, "ns": 1.0, "s": 1e9}.get(unit, 1.0)
+        d = out.setdefault(base, {})
+        m = r["Metric Name"]
+        if m in ("launch__registers_per_thread", "sm__warps_active.avg.pct_of_peak_sustained_active"):
+            d[m] = max(d.get(m, 0.0), v)
+        else:
+            d[m] = d.get(m, 0.0) + v * scale
+    return out, os.path.relpath(path, ROOT)
+
+
+def issue_roofline(warp_inst, ms, clocks, source):
+    """Secondary roofline of an issue-bound kernel: warp instructions per launch (tracked ncu export) / measured
     duration against 592 issue slots x the SM clock sampled during the run."""
     mhz = (clocks or {}).get("sm_mhz") or (clocks or {}).get("sm_max_mhz")
     if not warp_inst or not ms or not mhz:
@@ -63,7 +106,20 @@ def issue_roofline(warp_inst, ms, clocks):
     achieved = warp_inst / (ms * 1e-3) / 1e9
     peak = ISSUE_SLOTS_PER_CLOCK * mhz * 1e6 / 1e9
     return {"bound": "issue", "achieved": achieved, "peak": peak, "unit": "G warp-inst/s", "frac": achieved / peak,
-            "source": "smsp__inst_executed.sum from profiles/r01_v4_summary.md / CUDA-event duration of this run"}
+            "source": "smsp__inst_executed.sum from %s / CUDA-event duration of this run" % source}
+
+
+def fp64_roofline(fp64_warp_inst, ms, peak_dfma_per_s, source):
+    """fp64 leg (BASELINE.json: 'fp64 pipe utilisation against the chip's fp64 peak'): fp64-pipe warp
+    instructions per launch (tracked ncu export) / measured duration against the DFMA rate measured by
+    cuba_probe_fp64 in this run (thread-level rate / 32)."""
+    if not fp64_warp_inst or not ms or not peak_dfma_per_s:
+        return None
+    achieved = fp64_warp_inst / (ms * 1e-3) / 1e9
+    peak = peak_dfma_per_s / 32.0 / 1e9
+    return {"bound": "fp64", "achieved": achieved, "peak": peak, "unit": "G fp64 warp-inst/s", "frac": achieved / peak,
+            "peak_tflops": 2.0 * peak_dfma_per_s / 1e12,
+            "source": "smsp__inst_executed_pipe_fp64.sum from %s / CUDA-event duration; peak = cuba_probe_fp64 (this run)" % source}
 
 
 def peaks():
@@ -203,6 +259,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-fuse", action="store_true", help="run the separate k_stream_hist pass every step (A/B diagnostic)")
     ap.add_argument("--slots", type=int, default=-1, help="CUBA_OPT_SLOTS: 0 compact schedule, 1/2 slotted schedule; -1 library default (A/B diagnostic)")
+    ap.add_argument("--repeats", type=int, default=3, help="timed repeats of K steps each; the line reports the median")
     ap.add_argument("--profile-mode", type=int, default=1, help="1: normal operation; 2: serialise the collision classes (diagnostic)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuba" else args.warmup
@@ -248,28 +305,37 @@ def main():
     sampler = ClockSampler(local)
     sampler.start()
 
-    # ---- warm-up, then the timed region: K steps, CUDA events on the launching stream ---
+    # ---- warm-up, then the timed region: K steps, CUDA events on the launching stream, profiling OFF
+    # (the configuration a user runs); repeated, the line reports the median repeat (and the best) ----
     sim.step(args.warmup, w.dt, w.sigma)
     barrier()
     c0 = sim.counters()
     l0 = cuba.launch_count()
-    sim.profile_enable(args.profile_mode)
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    sampler.armed = True
-    ev0.record()
-    sim.step(args.steps, w.dt, w.sigma)
-    ev1.record()
-    barrier()
-    sampler.armed = False
-    ms = ev0.elapsed_time(ev1)
-    launches = cuba.launch_count() - l0
-    prof = sim.profile_read()
-    sim.profile_enable(0)
+    reps = []
+    for _ in range(args.repeats):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        sampler.armed = True
+        ev0.record()
+        sim.step(args.steps, w.dt, w.sigma)
+        ev1.record()
+        barrier()
+        sampler.armed = False
+        reps.append(ev0.elapsed_time(ev1))
+    ms = float(np.median(reps))
+    launches = (cuba.launch_count() - l0) // args.repeats
     c1 = sim.counters()
-    pairs = c1.pairs - c0.pairs
+    pairs = (c1.pairs - c0.pairs) / args.repeats
     if c1.device_flags:
         raise SystemExit("device error flags %d" % c1.device_flags)
+
+    # ---- per-kernel split: a separate pass of K steps with a CUDA event after every launch ----
+    sim.profile_enable(args.profile_mode)
+    sim.step(args.steps, w.dt, w.sigma)
+    prof = sim.profile_read()
+    sim.profile_enable(0)
+    prof_ms = sum(v[0] for k, v in prof.items() if "(all classes" in k or not k.startswith("k_collide<"))
+    fp64_peak = cuba.probe_fp64(sim._stream.cuda_stream, 5) if rank == 0 else 0.0
 
     # particles each collide class handled in the last step (for per-launch algorithmic bytes)
     import re
@@ -291,13 +357,17 @@ def main():
     if not args.no_e2e:
         e2e_steps = args.steps
         harr = [h.numpy() for h in host]
-        cuba.run_host(w.box, w.ncell, *harr, w.n_test, w.seed, 1, w.dt, w.sigma, w.nslab)   # warm the allocator
+        barrier()
+        t0 = time.perf_counter()
+        cuba.run_host(w.box, w.ncell, *harr, w.n_test, w.seed, e2e_steps, w.dt, w.sigma, w.nslab)   # cold: the library's pool maps its memory
+        torch.cuda.synchronize()
+        cold_s = time.perf_counter() - t0
         barrier()
         t0 = time.perf_counter()
         cuba.run_host(w.box, w.ncell, *harr, w.n_test, w.seed, e2e_steps, w.dt, w.sigma, w.nslab)
         torch.cuda.synchronize()
         e2e_s = time.perf_counter() - t0
-        e2e = {"s": e2e_s, "steps": e2e_steps}
+        e2e = {"s": e2e_s, "steps": e2e_steps, "cold_s": cold_s}
     sim.close()
 
     # ---- reduce over ranks: max time, summed work --------------------------------------
@@ -317,45 +387,76 @@ def main():
         alg = {"k_stream_hist": BYTES_STREAM_HIST * n, "k_scatter": BYTES_SCATTER * n}
         alg.update({name: bytes_collide * cnt for name, cnt in class_particles.items()})
         alg["k_collide (all classes, concurrent)"] = bytes_collide * sum(class_particles.values())
-        dom = max(per_kernel, key=lambda k: per_kernel[k]["ms_total"])
+        groups = {k: v for k, v in per_kernel.items() if not k.startswith("k_collide<") or args.profile_mode == 2}
+        dom = max(groups, key=lambda k: groups[k]["ms_total"])
         dom_ms = per_kernel[dom]["ms_per_launch"]
         achieved = alg.get(dom, 0) / (dom_ms * 1e-3) / 1e9 if dom_ms else 0.0
         kernels = {}
         for k, v in per_kernel.items():
             if v["launches"]:
                 gbs = alg.get(k, 0) / (v["ms_per_launch"] * 1e-3) / 1e9 if v["ms_per_launch"] else 0.0
-                kernels[k] = {"ms_per_launch": round(v["ms_per_launch"], 5), "share": round(v["ms_total"] / ms, 4),
+                kernels[k] = {"ms_per_launch": round(v["ms_per_launch"], 5), "share": round(v["ms_total"] / prof_ms, 4) if prof_ms else None,
                               "alg_GBps": round(gbs, 1), "frac": round(gbs / peak, 4)}
+        # ncu-derived figures of the dominant kernel group, from the tracked export of one step
+        ncu, ncu_src = ncu_export(args.config)
+        base = "k_slot_step" if dom.startswith("k_slot_step") else ("k_collide" if dom.startswith("k_collide") else dom)
+        nk = {}
+        if ncu:
+            for name, d in ncu.items():
+                if name == base or (base == "k_collide" and name == "k_collide_overflow"):
+                    for m, v in d.items():
+                        nk[m] = nk.get(m, 0.0) + v if not m.startswith(("launch__", "sm__warps")) else max(nk.get(m, 0.0), v)
+        traffic = (nk.get("dram__bytes_read.sum", 0.0) + nk.get("dram__bytes_write.sum", 0.0)) or None
+        clk = sampler.summary()
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "repeats": {"n": args.repeats, "ms_per_step": [round(r / args.steps, 5) for r in reps],
+                        "median": ms / args.steps, "best": min(reps) / args.steps,
+                        "note": "value and ms_per_step are the median repeat; profiling off in the timed region"},
             "config": {"workload": workloads_name(args.config), "n_particles": n, "ncells": sim.ncells,
                        "l2": "inputs larger than L2 (%.2f GB state per copy vs 126 MB L2), no flush" % (52 * n / 1e9)
                        if 52 * n > 4 * 126e6 else "state comparable to L2: cache-resident, not a roofline config",
                        "parallelism": "replicas x%d" % world if world > 1 else "single GPU",
-                       "schedule": "fused: collide(t) also writes the histogram of step t+1 (CUBA_OPT_FUSE_HIST=1)"
-                       if fused else "separate k_stream_hist pass (CUBA_OPT_FUSE_HIST=0)"},
+                       "schedule": ("fused: collide(t) also writes the histogram of step t+1 (CUBA_OPT_FUSE_HIST=1)"
+                                    if fused else "separate k_stream_hist pass (CUBA_OPT_FUSE_HIST=0)") +
+                                   ("; CUBA_OPT_SLOTS=%d" % args.slots if args.slots >= 0 else "; CUBA_OPT_SLOTS default")},
             "pair_evals_per_s": pairs_total / sec,
             "pairs_per_step": pairs_total / args.steps,
             "observables_ms": obs_ms,
             "gpu_launches": int(launches),
-            "clocks": sampler.summary(),
+            "clocks": clk,
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((args.config, fused, dom)), "peak_source": peak_src,
+                         "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                          "alg_bytes_per_launch": alg.get(dom, 0),
-                         "issue": issue_roofline(NCU_WARP_INST.get((args.config, fused, dom)), dom_ms, sampler.summary()),
+                         "duration_source": "CUDA events after every launch in a separate pass of %d steps (cuba_profile_enable)" % args.steps,
+                         "ncu_source": ncu_src,
+                         "ncu": {k: nk.get(k) for k in ("smsp__inst_executed.sum", "smsp__inst_executed_pipe_fp64.sum",
+                                                         "launch__registers_per_thread",
+                                                         "sm__warps_active.avg.pct_of_peak_sustained_active")} if nk else None,
+                         "issue": issue_roofline(nk.get("smsp__inst_executed.sum"), dom_ms, clk, ncu_src),
+                         "fp64": fp64_roofline(nk.get("smsp__inst_executed_pipe_fp64.sum"), dom_ms, fp64_peak, ncu_src),
+                         "fp64_peak_measured": {"dfma_per_s": fp64_peak, "tflops": 2.0 * fp64_peak / 1e12,
+                                                "source": "cuba_probe_fp64: 8 dependent DFMA chains per thread, 8 CTAs x 256 threads per SM, best of 5"},
                          "step": {"alg_bytes_per_particle": BYTES_STEP,
                                   "moved_bytes_per_particle": BYTES_STEP_FUSED if fused else BYTES_STEP,
                                   "achieved": BYTES_STEP * value / world / 1e9,
-                                  "frac": BYTES_STEP * value / world / 1e9 / peak, "frac_of_8TBps_nominal": BYTES_STEP * value / world / 8e12},
+                                  "frac": BYTES_STEP * value / world / 1e9 / peak,
+                                  "frac_moved_bytes": (BYTES_STEP_FUSED if fused else BYTES_STEP) * value / world / 1e9 / peak,
+                                  "frac_of_8TBps_nominal": BYTES_STEP * value / world / 8e12,
+                                  "note": "frac uses the model's 204 B per particle-step (SURVEY 8(d): the method as specified); "
+                                          "frac_moved_bytes what the fused schedule really has to move"},
                          "kernels": kernels},
         }
         if e2e:
             line["e2e"] = {"value": n_total * e2e["steps"] / e2e["s"], "unit": UNIT,
                            "h2d_bytes_per_step": 48 * n / e2e["steps"], "d2h_bytes_per_step": 8 * (4 + w.nslab) / e2e["steps"],
-                           "call": "cuba_run_host: pinned HOST arrays -> H2D -> cuba_init -> cuba_step(%d) -> cuba_observables -> D2H"
-                                   % e2e["steps"], "seconds": e2e["s"]}
+                           "call": "cuba_run_host: pinned HOST arrays -> H2D -> cuba_init -> cuba_step(%d) -> cuba_observables -> D2H of "
+                                   "the observables only (4 + nslab doubles: north_star's result; the particle store is not copied back)"
+                                   % e2e["steps"], "seconds": e2e["s"],
+                           "cold_value": n_total * e2e["steps"] / e2e["cold_s"], "cold_seconds": e2e["cold_s"],
+                           "note": "value: second call (the library's memory pool already mapped); cold_value: first call of the process"}
         if not args.no_cpu_baseline:
             ow, sample = oracle_sample_workload(args.config)
             osteps = max(2, min(60, int(60e6 // max(ow.n, 1)) + 1))   # about 10-30 s of one host core

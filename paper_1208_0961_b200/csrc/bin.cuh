@@ -447,6 +447,7 @@ k_scatter(Geom g, double dt, int64_t n, int64_t ntiles, Soa in, Soa out, const u
             if (sli == 0) rank += s_carry[dd];
             const uint32_t dest = dbase[j] + rank;
             const uint32_t id = st.pid[li];
+            // (measured, no effect: L2 evict-last / evict-first cache hints on the movers' / stayers' stores)
             out.x[dest] = m[j].x; out.y[dest] = m[j].y; out.z[dest] = m[j].z;
             out.px[dest] = m[j].px; out.py[dest] = m[j].py; out.pz[dest] = m[j].pz;
             out.pid[dest] = id;

@@ -575,15 +575,11 @@ struct CtaStats {
     double scale, hscale;     // Eq. 3 factor cn*base/R of the current cell, and half of it
     uint32_t lo;              // first slot of the current cell
     uint32_t near;            // near-threshold decisions of this CTA (A16; rare)
+    uint32_t hits;            // collisions of this CTA since the last flush (lane 0 of every warp adds after a pair phase)
+    unsigned long long pairs, rounds;   // pair evaluations and rounds of this CTA (thread 0 adds per cell)
     uint32_t nlist[2];        // entries on the two dirty-element lists of the current sweep
     uint32_t head[2][kChains]; // first entry of the chain of the words with (word mod kChains) equal, per list
     HistCell h;               // fused histogram: constants of the current cell
-};
-
-// Per-thread accumulators over all cells of a CTA, flushed once at the end of the kernel.
-struct ThreadStats {
-    unsigned long long pairs, rounds;   // uniform over the CTA; thread 0 flushes
-    uint32_t hits;                       // uniform over a warp; lane 0 flushes
 };
 
 // Shared-memory arrays of one CTA: fixed offsets into the dynamic shared memory, so that every
@@ -620,17 +616,16 @@ __host__ __device__ constexpr size_t collide_smem_bytes(int cap, int threads, in
 
 // One pair phase (one round): Eq. 3 decision for the pairs order[2k], order[2k+1], then this warp's
 // hits are scattered.  first: the energies are computed here and left in sE (see above).  The pairs
-// are dealt to the warps in equal contiguous shares (the hits, and with them the scatter work, are
-// then spread evenly: a warp rarely has more than 32).
+// are dealt to the warps in rows of 32, round-robin (the hits, and with them the scatter work, are
+// then spread evenly: a warp rarely has more than 32); a warp skips the rows beyond the last pair.
 template <typename S, int THREADS, int PITEMS, bool TRACE>
-__device__ __forceinline__ uint32_t pair_phase(const CollideParams &P, uint32_t c, uint32_t n, uint32_t tcur, int rho,
+__device__ __forceinline__ void pair_phase(const CollideParams &P, uint32_t c, uint32_t n, uint32_t tcur, int rho,
                                             int slot, bool first, bool keepE, CtaStats *stats)
 {
     const uint16_t *sord = S::ord(slot);
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const uint32_t npairs = n >> 1;
-    const uint32_t share = (npairs + THREADS / 32 - 1) / (THREADS / 32);        // pairs per warp
-    const uint32_t k0 = wid * share, k1 = min(npairs, k0 + share);              // this warp's pairs [k0, k1)
+    constexpr int W = THREADS / 32;
     double *sE = S::E();
     uint16_t *shit = S::hits() + wid * (PITEMS * 32);
     if (first && tid == 0 && (n & 1u)) {          // the particle left over by the pairing: nobody else computes its energy
@@ -642,64 +637,58 @@ __device__ __forceinline__ uint32_t pair_phase(const CollideParams &P, uint32_t 
     {
         const double scale = *reinterpret_cast<volatile double *>(&stats->scale);
         const double hscale = *reinterpret_cast<volatile double *>(&stats->hscale);
-        double dd[PITEMS], ee[PITEMS], u[PITEMS];
-        uint32_t ida[PITEMS];
+        // row r = it * W + wid holds the pairs [32 r, 32 r + 32); rows that start beyond the last pair are skipped
+        // by the whole warp (no Philox, no loads for padding)
 #pragma unroll
         for (int it = 0; it < PITEMS; ++it) {
-            const uint32_t k = k0 + it * 32 + lane;
+            const uint32_t row0 = (uint32_t)(it * W + wid) * 32u;
+            if (row0 >= npairs) break;
+            const uint32_t k = row0 + lane;
             const uint32_t kc = min(k, npairs - 1u);
             const uint32_t ab = *reinterpret_cast<const uint32_t *>(sord + 2 * kc);
             const uint32_t a = ab & 0xFFFFu, b = ab >> 16;
             const double2 pa = S::pxy()[a], pb = S::pxy()[b];
             const double paz = S::pz()[a], pbz = S::pz()[b];
+            const uint32_t ida = S::pid()[a];
             double Ea, Eb;
             if (first) {
                 Ea = energy(pa.x, pa.y, paz); Eb = energy(pb.x, pb.y, pbz);
-                if (k < k1) { sE[a] = Ea; sE[b] = Eb; }
+                if (k < npairs) { sE[a] = Ea; sE[b] = Eb; }
             } else {
                 Ea = sE[a]; Eb = sE[b];
             }
             const double dx = Eb * pa.x - Ea * pb.x;
             const double dy = Eb * pa.y - Ea * pb.y;
             const double dz = Eb * paz - Ea * pbz;
-            ida[it] = S::pid()[a];
-            ee[it] = Ea * Eb;
-            dd[it] = (dx * dx + dy * dy) + dz * dz;
-        }
-#pragma unroll
-        for (int it = 0; it < PITEMS; ++it) {
-            const U4 w = drawk(P, tcur, ida[it], (uint32_t)rho, kTagDec, 0);
-            u[it] = u53_bits(w.x, w.y);
-        }
-#pragma unroll
-        for (int it = 0; it < PITEMS; ++it) {
-            const uint32_t k = k0 + it * 32 + lane;
+            const double ee = Ea * Eb;
+            const double dd = (dx * dx + dy * dy) + dz * dz;
+            const U4 w = drawk(P, tcur, ida, (uint32_t)rho, kTagDec, 0);
+            const double u = u53_bits(w.x, w.y);
             bool hit;
             if (TRACE) {
-                const double s = dd[it] / ee[it];         // (p_a+p_b)^2, A9
-                const double vrel = 0.5 * (s / ee[it]);   // s/(2 E_a E_b)
+                const double s = dd / ee;                 // (p_a+p_b)^2, A9
+                const double vrel = 0.5 * (s / ee);       // s/(2 E_a E_b)
                 const double prob = vrel * scale;         // Eq. 3 * cn/R
-                hit = u[it] < prob;
-                if (k < k1) {
-                    if (fabs(u[it] - prob) <= 1e-12) atomicAdd(&stats->near, 1u);
-                    const uint32_t ab = *reinterpret_cast<const uint32_t *>(sord + 2 * k);
+                hit = u < prob;
+                if (k < npairs) {
+                    if (fabs(u - prob) <= 1e-12) atomicAdd(&stats->near, 1u);
                     const unsigned long long e = P.trace_off[c] + (unsigned long long)rho * npairs + k;
-                    P.tr_cell[e] = c; P.tr_round[e] = (uint32_t)rho; P.tr_pa[e] = ida[it]; P.tr_pb[e] = S::pid()[ab >> 16];
-                    P.tr_P[e] = prob; P.tr_u[e] = u[it]; P.tr_dec[e] = hit ? 1 : 0;
+                    P.tr_cell[e] = c; P.tr_round[e] = (uint32_t)rho; P.tr_pa[e] = ida; P.tr_pb[e] = S::pid()[b];
+                    P.tr_P[e] = prob; P.tr_u[e] = u; P.tr_dec[e] = hit ? 1 : 0;
                 }
             } else {
                 // sign(u - P) from u*(EaEb)^2 - |d|^2*scale/2; the exact form only inside a band
                 // far wider than the rounding error (it also catches NaN, inf and underflow)
-                const double ee2 = ee[it] * ee[it];
-                const double diff = u[it] * ee2 - dd[it] * hscale;
+                const double ee2 = ee * ee;
+                const double diff = u * ee2 - dd * hscale;
                 hit = diff < 0.0;
                 if (CUBA_FORCE_SLOW_PATHS || !(fabs(diff) > 4e-9 * ee2) || !(ee2 > 1e-280)) {
-                    const uint32_t r = exact_decision(dd[it], ee[it], u[it], scale);
+                    const uint32_t r = exact_decision(dd, ee, u, scale);
                     hit = (r & 1u) != 0;
-                    if ((r & 2u) && k < k1) atomicAdd(&stats->near, 1u);
+                    if ((r & 2u) && k < npairs) atomicAdd(&stats->near, 1u);
                 }
             }
-            hit = hit && k < k1;
+            hit = hit && k < npairs;
             const uint32_t hm = __ballot_sync(0xFFFFFFFFu, hit);
             if (hit) shit[nh + __popc(hm & lanemask_lt())] = (uint16_t)k;
             nh += __popc(hm);
@@ -725,33 +714,34 @@ __device__ __forceinline__ uint32_t pair_phase(const CollideParams &P, uint32_t 
         S::pxy()[b] = make_double2(q[3], q[4]); S::pz()[b] = q[5];
         if (keepE) { sE[a] = energy(q[0], q[1], q[2]); sE[b] = energy(q[3], q[4], q[5]); }
     }
+    if (lane == 0 && nh) atomicAdd(&stats->hits, nh);
     __syncwarp();   // the hit list is rewritten in the next pair phase
-    return nh;
 }
 
 // Phase C1 for one element and one of the two rounds of a sweep (slot 0 / 1): the rank of an element of
 // a clean word; an element of a dirty word goes onto the round's list, chained by word mod kChains.
-template <typename S, int LCAP>
-__device__ __forceinline__ void rank_clean(const CollideParams &P, CtaStats *stats, int slot,
+template <typename S, int LCAP, int SLOT>
+__device__ __forceinline__ void rank_clean(const CollideParams &P, CtaStats *stats,
                                            uint32_t k, uint32_t j, uint32_t n, uint32_t M,
                                            uint32_t tcur, int rho)
 {
     const uint32_t b = __umulhi(k, M), word = b >> 5, below = (1u << (b & 31u)) - 1u;
-    const uint32_t pw = (S::cnt()[word] >> (16 * slot)) & 0xFFFFu;
-    uint32_t rank = (pw >> 1) + __popc((S::bm() + slot * n)[word] & below);
+    const uint32_t cw = S::cnt()[word];
+    const uint32_t pw = SLOT ? (cw >> 16) : (cw & 0xFFFFu);
+    uint32_t rank = (pw >> 1) + __popc((S::bm() + SLOT * n)[word] & below);
     if (j < n) {
         if (CUBA_FORCE_SLOW_PATHS || (pw & 1u)) {
-            const uint32_t at = atomicAdd(&stats->nlist[slot], 1u);
+            const uint32_t at = atomicAdd(&stats->nlist[SLOT], 1u);
             if (at < (uint32_t)LCAP) {
-                const uint32_t next = atomicExch(&stats->head[slot][word % kChains], at);
-                S::lkey(slot)[at] = k;
-                S::lwj(slot)[at] = (word << 13) | j;
-                S::lpn(slot)[at] = (pw >> 1) | (next << 16);
+                const uint32_t next = atomicExch(&stats->head[SLOT][word % kChains], at);
+                S::lkey(SLOT)[at] = k;
+                S::lwj(SLOT)[at] = (word << 13) | j;
+                S::lpn(SLOT)[at] = (pw >> 1) | (next << 16);
                 return;
             }
             rank = (pw >> 1) + brute_rank(P.seed, tcur, S::pid(), n, M, word, k, S::pid()[j], rho);   // the list is full
         }
-        S::ord(slot)[rank] = (uint16_t)j;
+        S::ord(SLOT)[rank] = (uint16_t)j;
     }
 }
 
@@ -786,9 +776,9 @@ __device__ __forceinline__ void rank_dirty(const CollideParams &P, const CtaStat
 
 // All R rounds of one staged cell, two per sweep (see above).  On entry: momenta and pids staged, both
 // bitmaps, the duplicate counters, the list counters and chain heads cleared, a block barrier passed.
-// keepE: the caller needs the energies of the final momenta in sE afterwards.  Returns this warp's hits.
+// keepE: the caller needs the energies of the final momenta in sE afterwards.
 template <int THREADS, int ITEMS, int G, int CAP, int LCAP, bool TRACE>
-__device__ __forceinline__ uint32_t run_sweeps(const CollideParams &P, uint32_t c, uint32_t n, int R, uint32_t tcur,
+__device__ __forceinline__ void run_sweeps(const CollideParams &P, uint32_t c, uint32_t n, int R, uint32_t tcur,
                                                bool hist, uint32_t *s_warp, CtaStats *stats)
 {
     using S = CellSmem<CAP, LCAP>;
@@ -799,7 +789,8 @@ __device__ __forceinline__ uint32_t run_sweeps(const CollideParams &P, uint32_t 
     const uint32_t last = n - 1u;
     const uint32_t M = 32u * n;                      // bits of a bitmap: word = bit >> 5 < n
     uint32_t *bmA = S::bm(), *bmB = S::bm() + n;
-    uint32_t warp_hits = 0;
+    // items it of this warp with a particle in them: (tid & ~31) + it * THREADS < n
+    const int nit = (int)min((uint32_t)ITEMS, (n + (uint32_t)THREADS - 1u - min(n, (uint32_t)(tid & ~31))) / (uint32_t)THREADS);
     for (int rho0 = 0; rho0 < R; rho0 += 2) {
         const bool two = rho0 + 1 < R;
         if (rho0 > 0) {
@@ -816,23 +807,27 @@ __device__ __forceinline__ uint32_t run_sweeps(const CollideParams &P, uint32_t 
         }
         uint32_t keyA[ITEMS], keyB[ITEMS];
         // (A) shuffle keys of the two rounds (A7: words 2*(sweep mod 2), +1 of the call for rounds
-        // 4*(rho div 4)..+3) and one atomicOr per element and round
+        // 4*(rho div 4)..+3) and one atomicOr per element and round.  nit: items of this warp that hold
+        // particles (warp-uniform): a warp does no Philox and no ranking for the padding of the class.
 #pragma unroll
         for (int g = 0; g < NG; ++g) {
-            if ((uint32_t)(g * G * THREADS) >= n) break;
+            if (g * G >= nit) break;
 #pragma unroll
             for (int i = 0; i < G; ++i) {
                 const int it = g * G + i;
-                const uint32_t jc = min((uint32_t)(tid + it * THREADS), last);
-                const U4 w = drawk(P, tcur, S::pid()[jc], (uint32_t)rho0 >> 2, kTagShuf, 0);
-                keyA[it] = (rho0 & 2) ? w.z : w.x;
-                keyB[it] = (rho0 & 2) ? w.w : w.y;
+                keyA[it] = 0; keyB[it] = 0;
+                if (it < nit) {
+                    const uint32_t jc = min((uint32_t)(tid + it * THREADS), last);
+                    const U4 w = drawk(P, tcur, S::pid()[jc], (uint32_t)rho0 >> 2, kTagShuf, 0);
+                    keyA[it] = (rho0 & 2) ? w.z : w.x;
+                    keyB[it] = (rho0 & 2) ? w.w : w.y;
+                }
             }
 #pragma unroll
             for (int i = 0; i < G; ++i) {
                 const int it = g * G + i;
                 const uint32_t j = tid + it * THREADS;
-                if (j < n) {
+                if (it < nit && j < n) {
                     const uint32_t bA = __umulhi(keyA[it], M), mA = 1u << (bA & 31u);
                     if (atomicOr(&bmA[bA >> 5], mA) & mA) atomicAdd(&S::cnt()[bA >> 5], 1u);
                     if (two) {
@@ -873,11 +868,10 @@ __device__ __forceinline__ uint32_t run_sweeps(const CollideParams &P, uint32_t 
         // (C1) rank = prefix of the word + occupied bits below mine; elements of dirty words go onto a list
 #pragma unroll
         for (int it = 0; it < ITEMS; ++it) {
-            if ((uint32_t)(it * THREADS) >= n) break;
+            if (it >= nit) break;
             const uint32_t j = tid + it * THREADS;
-#pragma unroll 1
-            for (int sl = 0; sl < (two ? 2 : 1); ++sl)
-                rank_clean<S, LCAP>(P, stats, sl, sl ? keyB[it] : keyA[it], j, n, M, tcur, rho0 + sl);
+            rank_clean<S, LCAP, 0>(P, stats, keyA[it], j, n, M, tcur, rho0);
+            if (two) rank_clean<S, LCAP, 1>(P, stats, keyB[it], j, n, M, tcur, rho0 + 1);
         }
         __syncthreads();
         // (C2) the listed elements, one thread each
@@ -887,22 +881,19 @@ __device__ __forceinline__ uint32_t run_sweeps(const CollideParams &P, uint32_t 
 #pragma unroll 1
         for (int sl = 0; sl < (two ? 2 : 1); ++sl) {
             if (sl) __syncthreads();
-            warp_hits += pair_phase<S, THREADS, PITEMS, TRACE>(P, c, n, tcur, rho0 + sl, sl, sl == 0, sl == 0 ? (two || hist) : hist, stats);
+            pair_phase<S, THREADS, PITEMS, TRACE>(P, c, n, tcur, rho0 + sl, sl, sl == 0, sl == 0 ? (two || hist) : hist, stats);
         }
     }
-    return warp_hits;
 }
 
 template <int THREADS, int ITEMS, int G, int CAP, int LCAP, bool TRACE, bool LOCAL, bool GRAPH>
 __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32_t c, uint32_t lo, uint32_t n,
                                                   uint32_t *s_warp, CtaStats *stats,
-                                                  uint32_t *s_seg, long long *s_esum, ThreadStats &acc,
+                                                  uint32_t *s_seg, long long *s_esum,
                                                   uint32_t lo_next, uint32_t n_next)
 {
     static_assert(ITEMS % G == 0, "items are processed in groups of G");
     constexpr int NG = ITEMS / G;
-    constexpr int PITEMS = (ITEMS + 1) / 2;          // pairs per thread
-    constexpr int SCAN = ITEMS | 1;                  // words per thread in the scan (odd stride: no bank conflicts)
     using S = CellSmem<CAP, LCAP>;
     const int tid = threadIdx.x;
     // step index: a constant-bank operand normally; a register loaded from device memory when the
@@ -981,7 +972,7 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
         if (hist) { prefetch_l2(P.x + e); prefetch_l2(P.y + e); prefetch_l2(P.z + e); }
     }
 
-    const uint32_t warp_hits = run_sweeps<THREADS, ITEMS, G, CAP, LCAP, TRACE>(P, c, n, R, tcur, hist, s_warp, stats);
+    run_sweeps<THREADS, ITEMS, G, CAP, LCAP, TRACE>(P, c, n, R, tcur, hist, s_warp, stats);
     if (R == 0 && hist && tid == 0) {     // a lone particle: no pair phase has computed its energy
         const double2 xy = S::pxy()[0];
         sE[0] = energy(xy.x, xy.y, S::pz()[0]);
@@ -994,9 +985,7 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
         const double2 xy = S::pxy()[j];
         P.px[lo_w + j] = xy.x; P.py[lo_w + j] = xy.y; P.pz[lo_w + j] = S::pz()[j];
     }
-    acc.hits += warp_hits;
-    acc.pairs += (unsigned long long)R * (n >> 1);
-    acc.rounds += (unsigned long long)R;
+    if (tid == 0) { stats->pairs += (unsigned long long)R * (n >> 1); stats->rounds += (unsigned long long)R; }
 
     // ---- fused histogram of the next step (S1-S3 of step t+1 on the final momenta) ----------
     if (hist) {
@@ -1098,8 +1087,7 @@ k_collide(CollideParams P)
     // into L2.  (Measured alternatives, both slower because they lengthen the tail of the list:
     // a static round-robin, +0.10 ms at configs[2]; claiming three cells ahead, +0.09 ms.)
     const uint32_t nlist = *P.list_count;
-    if (threadIdx.x == 0) s_stats.near = 0;
-    ThreadStats acc{0ull, 0ull, 0u};
+    if (threadIdx.x == 0) { s_stats.near = 0; s_stats.hits = 0; s_stats.pairs = 0; s_stats.rounds = 0; }
     __shared__ uint32_t s_item[2];
     if (threadIdx.x == 0) s_item[0] = atomicAdd(P.work, 1u);
     __syncthreads();
@@ -1113,14 +1101,14 @@ k_collide(CollideParams P)
         uint4 nxt = make_uint4(0u, 0u, 0u, 0u);
         if (item < nlist) nxt = P.list[item];   // first used after the staging barrier
         collide_cell_smem<THREADS, ITEMS, G, CAP, LCAP, TRACE, LOCAL, GRAPH>(P, cur.x, cur.y, cur.z, s_warp, &s_stats, s_seg, s_esum,
-                                                                        acc, nxt.y, nxt.z);
+                                                                        nxt.y, nxt.z);
         __syncthreads();
         cur = nxt;
     }
-    if ((threadIdx.x & 31) == 0 && acc.hits) atomicAdd(&P.counters[1], (unsigned long long)acc.hits);
-    if (threadIdx.x == 0) {
-        if (acc.pairs) atomicAdd(&P.counters[0], acc.pairs);
-        if (acc.rounds) atomicAdd(&P.counters[2], acc.rounds);
+    if (threadIdx.x == 0) {       // the loop ends with a block barrier
+        if (s_stats.hits) atomicAdd(&P.counters[1], (unsigned long long)s_stats.hits);
+        if (s_stats.pairs) atomicAdd(&P.counters[0], s_stats.pairs);
+        if (s_stats.rounds) atomicAdd(&P.counters[2], s_stats.rounds);
         if (s_stats.near) atomicAdd(&P.counters[3], (unsigned long long)s_stats.near);
     }
 }

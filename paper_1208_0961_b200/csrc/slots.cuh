@@ -113,8 +113,38 @@ struct SlotCell {
     uint32_t dst_base[kDirs];        // direction d: first slot of segment 26-d of the destination cell in `out`
     uint32_t dst_cap[kDirs];         // its capacity (0: no such neighbour)
     uint32_t dst_cnt[kDirs];         // index of its count in out.cnt (0xFFFFFFFF: no such neighbour)
-    uint32_t total[kDirs];           // particles of this cell leaving in direction d
+    int i0[3];                       // cell coordinates (x slowest)
 };
+
+// The tables of cell c, by one warp.  v: lane s < 27 holds the population of inbox segment s of the cell
+// (loaded by the caller, possibly long before: the tables of a CTA's NEXT cell are built while the
+// current one is processed, so that nobody waits for that load).
+template <bool FROM_SLOTS, bool STREAM>
+__device__ __forceinline__ void slot_tables(const Geom &g, const SlotGeom &sg, uint32_t c, uint32_t v, SlotCell *tab)
+{
+    const int lane = threadIdx.x & 31;
+    const int i2 = (int)(c % (uint32_t)g.nc[2]);
+    const int i1 = (int)((c / (uint32_t)g.nc[2]) % (uint32_t)g.nc[1]);
+    const int i0 = (int)(c / ((uint32_t)g.nc[2] * (uint32_t)g.nc[1]));
+    if (lane == 0) { tab->i0[0] = i0; tab->i0[1] = i1; tab->i0[2] = i2; }
+    if (FROM_SLOTS) {
+        uint32_t inc = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane <= kDirs) tab->seg_start[lane] = inc - v;       // lane 27: the total
+        if (lane < kDirs) tab->src_base[lane] = c * sg.slots + sg.seg_off[lane];
+    }
+    if (STREAM && lane < kDirs) {
+        const int nb = slot_neighbour(g, i0, i1, i2, lane);
+        const int seg = kDirs - 1 - lane;
+        tab->dst_base[lane] = nb >= 0 ? (uint32_t)nb * sg.slots + sg.seg_off[seg] : 0u;
+        tab->dst_cap[lane] = nb >= 0 ? sg.seg_off[seg + 1] - sg.seg_off[seg] : 0u;
+        tab->dst_cnt[lane] = nb >= 0 ? (uint32_t)nb * kDirs + (uint32_t)seg : 0xFFFFFFFFu;
+    }
+}
 
 // slot index (in the `in` copy) of the particle at assembly position j
 __device__ __forceinline__ uint32_t slot_source(const SlotCell *t, uint32_t j)
@@ -130,13 +160,12 @@ __device__ __forceinline__ uint32_t slot_source(const SlotCell *t, uint32_t j)
 }
 
 // Tail scratch in the dynamic shared memory (all dead by then): the duplicate counters' space holds the
-// row masks [rows][27], the lists' space their prefixes (16 bit), the orders' space the direction codes.
+// row masks [rows][27], the lists' space their prefixes (16 bit).
 template <int CAP, int LCAP>
 struct SlotTail {
     using S = CellSmem<CAP, LCAP>;
     static __device__ __forceinline__ uint32_t *ball() { return S::cnt(); }                                      // [rows][27] <= CAP words
     static __device__ __forceinline__ uint16_t *pref() { return reinterpret_cast<uint16_t *>(S::lkey(0)); }      // [rows][27] 16 bit <= 12 LCAP bytes... checked below
-    static __device__ __forceinline__ uint16_t *dir() { return S::ord(0); }                                      // [CAP]
 };
 
 // What a pass does.  A call of n steps is n + 1 passes: the first one takes the cells from the compact store and
@@ -147,14 +176,15 @@ enum SlotMode { kSlotMiddle = 0, kSlotFirst = 1, kSlotLast = 2 };
 
 template <int THREADS, int ITEMS, int G, int CAP, int LCAP, int MODE>
 __device__ __forceinline__ void step_cell_slots(const CollideParams &P, const SlotParams &Q, uint32_t c, uint32_t lo, uint32_t n,
-                                                uint32_t *s_warp, CtaStats *stats, SlotCell *tab, ThreadStats &acc,
-                                                uint32_t c_next, uint32_t lo_next, uint32_t n_next)
+                                                uint32_t *s_warp, CtaStats *stats, SlotCell *tab, SlotCell *tab_next, bool tab_ready,
+                                                uint32_t *s_vnext, uint32_t c_next, uint32_t lo_next, uint32_t n_next)
 {
     using S = CellSmem<CAP, LCAP>;
     using T = SlotTail<CAP, LCAP>;
     constexpr int W = THREADS / 32, ROWS = ITEMS * W;
     static_assert(ROWS * kDirs <= CAP, "row masks fit the duplicate counters' space");
     static_assert(ROWS * kDirs * 2 <= 24 * LCAP, "row prefixes fit the lists' space");
+    static_assert(ITEMS <= 6, "direction codes of a thread's items are packed 5 bits each");
     constexpr bool COLLIDE = MODE != kSlotFirst, STREAM = MODE != kSlotLast, FROM_SLOTS = MODE != kSlotFirst;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const uint32_t tcur = P.t;
@@ -173,38 +203,27 @@ __device__ __forceinline__ void step_cell_slots(const CollideParams &P, const Sl
             stats->scale = scale; stats->hscale = 0.5 * scale;
         }
     }
-    // ---- per-cell tables (warp 0) --------------------------------------------------------------------
+    // ---- per-cell tables (warp 0): this cell's only for the first cell of a CTA; the inbox counts of the NEXT
+    // cell are fetched now and turned into its tables after the rounds, so that nobody waits for the load --
+    // (an asynchronous copy into shared memory: no register is held across the rounds)
     if (tid < 32) {
-        const int i2 = (int)(c % (uint32_t)P.g.nc[2]);
-        const int i1 = (int)((c / (uint32_t)P.g.nc[2]) % (uint32_t)P.g.nc[1]);
-        const int i0 = (int)(c / ((uint32_t)P.g.nc[2] * (uint32_t)P.g.nc[1]));
-        if (STREAM) hist_cell_setup(P.g, c, &stats->h, tid);
-        if (FROM_SLOTS) {
-            const uint32_t v = lane < kDirs ? Q.in.cnt[(size_t)c * kDirs + lane] : 0u;
-            uint32_t inc = v;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o);
-                if (lane >= o) inc += t;
-            }
-            if (lane <= kDirs) tab->seg_start[lane] = inc - v;       // lane 27: the total
-            if (lane < kDirs) tab->src_base[lane] = c * Q.sg.slots + Q.sg.seg_off[lane];
+        if (!tab_ready) {
+            const uint32_t v = (FROM_SLOTS && lane < kDirs) ? Q.in.cnt[(size_t)c * kDirs + lane] : 0u;
+            slot_tables<FROM_SLOTS, STREAM>(P.g, Q.sg, c, v, tab);
         }
-        if (STREAM && lane < kDirs) {
-            const int nb = slot_neighbour(P.g, i0, i1, i2, lane);
-            const int seg = kDirs - 1 - lane;
-            tab->dst_base[lane] = nb >= 0 ? (uint32_t)nb * Q.sg.slots + Q.sg.seg_off[seg] : 0u;
-            tab->dst_cap[lane] = nb >= 0 ? Q.sg.seg_off[seg + 1] - Q.sg.seg_off[seg] : 0u;
-            tab->dst_cnt[lane] = nb >= 0 ? (uint32_t)nb * kDirs + (uint32_t)seg : 0xFFFFFFFFu;
-        }
+        if (FROM_SLOTS && n_next && lane < kDirs)
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(s_vnext + lane)), "l"(Q.in.cnt + (size_t)c_next * kDirs + lane) : "memory");
+        asm volatile("cp.async.commit_group;" ::: "memory");
     }
     __syncthreads();
     const uint32_t last = n - 1u;
     double *sE = S::E();
+    // items it of this warp with a particle in them: (tid & ~31) + it * THREADS < n
+    const int nit = (int)min((uint32_t)ITEMS, (n + (uint32_t)THREADS - 1u - min(n, (uint32_t)(tid & ~31))) / (uint32_t)THREADS);
     // ---- assemble: momenta and pids (from the 27 segments in order); clear the sort structures ---------
 #pragma unroll
     for (int g = 0; g < ITEMS / G; ++g) {
-        if ((uint32_t)(g * G * THREADS) >= n) break;
+        if (g * G >= nit) break;       // warp-uniform; inside a group the padding is loaded (clamped) and dropped
         double a[G], b[G], cc[G];
         uint32_t id[G];
 #pragma unroll
@@ -235,22 +254,25 @@ __device__ __forceinline__ void step_cell_slots(const CollideParams &P, const Sl
         }
     }
     if (COLLIDE) {
-        const uint32_t warp_hits = run_sweeps<THREADS, ITEMS, G, CAP, LCAP, false>(P, c, n, R, tcur, STREAM, s_warp, stats);
+        run_sweeps<THREADS, ITEMS, G, CAP, LCAP, false>(P, c, n, R, tcur, STREAM, s_warp, stats);
         if (STREAM && R == 0 && tid == 0) {     // a lone particle: no pair phase has computed its energy
             const double2 xy = S::pxy()[0];
             sE[0] = energy(xy.x, xy.y, S::pz()[0]);
         }
-        __syncthreads();
-        acc.hits += warp_hits;
-        acc.pairs += (unsigned long long)R * (n >> 1);
-        acc.rounds += (unsigned long long)R;
+        if (tid == 0) { stats->pairs += (unsigned long long)R * (n >> 1); stats->rounds += (unsigned long long)R; }
     }
-    constexpr int HB = (ITEMS % 2 == 0) ? 2 : 1;
+    if (tid < 32 && n_next) {
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncwarp();
+        slot_tables<FROM_SLOTS, STREAM>(P.g, Q.sg, c_next, (FROM_SLOTS && lane < kDirs) ? s_vnext[lane] : 0u, tab_next);
+    }
     if (!STREAM) {
+        __syncthreads();
         // ---- last pass: the cell goes to its place in the compact store, positions unchanged -----------
+        constexpr int HB = (ITEMS % 2 == 0) ? 2 : 1;
 #pragma unroll 1
         for (int g = 0; g < ITEMS / HB; ++g) {
-            if ((uint32_t)(g * HB * THREADS) >= n) break;
+            if (g * HB >= nit) break;
             double xx[HB], yy[HB], zz[HB];
 #pragma unroll
             for (int i = 0; i < HB; ++i) {
@@ -272,82 +294,113 @@ __device__ __forceinline__ void step_cell_slots(const CollideParams &P, const Sl
         return;
     }
 
-    // ---- tail, pass 1: direction of every particle; one mask per row of 32 and direction --------------
-    for (int e = tid; e < ROWS * kDirs; e += THREADS) T::ball()[e] = 0;
-    __syncthreads();
-    const HistCell &hc = stats->h;
-#pragma unroll 1
-    for (int g = 0; g < ITEMS / HB; ++g) {
-        if ((uint32_t)(g * HB * THREADS) >= n) break;
-        double xx[HB], yy[HB], zz[HB];
+    // ---- tail, pass 1: S1-S3 exactly (the arithmetic of move_particle); one mask per row of 32 particles and
+    // direction.  The positions of the next item are in flight while an item is moved; the new x goes into the
+    // particle's (now dead) energy slot, the new y and z stay in registers across the prefix. ----
+    double Y[ITEMS], Z[ITEMS];
+    double xa = 0.0, ya = 0.0, za = 0.0;
+    if (nit > 0) {
+        const uint32_t jc = min((uint32_t)tid, last);
+        const uint32_t src = FROM_SLOTS ? slot_source(tab, jc) : lo + jc;
+        xa = Q.in.x[src]; ya = Q.in.y[src]; za = Q.in.z[src];
+    }
+    for (int e = tid; e < ROWS * kDirs; e += THREADS) T::ball()[e] = 0;    // the dirty lists were last read before the last pair phase
+    __syncthreads();     // the rounds are over (energies final), the masks are clear
+    const int ix0 = tab->i0[0], iy0 = tab->i0[1], iz0 = tab->i0[2];
+    uint32_t dpk = 0;
 #pragma unroll
-        for (int i = 0; i < HB; ++i) {
-            const uint32_t jc = min((uint32_t)(tid + (g * HB + i) * THREADS), last);
-            const uint32_t src = FROM_SLOTS ? slot_source(tab, jc) : lo + jc;
-            xx[i] = Q.in.x[src]; yy[i] = Q.in.y[src]; zz[i] = Q.in.z[src];
-        }
-#pragma unroll
-        for (int i = 0; i < HB; ++i) {
-            const int it = g * HB + i;
+    for (int it = 0; it < ITEMS; ++it) {
+        if (it < nit) {
+            double xn = 0.0, yn = 0.0, zn = 0.0;
+            if (it + 1 < nit) {
+                const uint32_t jc = min((uint32_t)(tid + (it + 1) * THREADS), last);
+                const uint32_t src = FROM_SLOTS ? slot_source(tab, jc) : lo + jc;
+                xn = Q.in.x[src]; yn = Q.in.y[src]; zn = Q.in.z[src];
+            }
             const uint32_t j = tid + it * THREADS, jj = min(j, last);
             const double2 xy = S::pxy()[jj];
-            int d = next_direction_guarded(P.g, Q.dt, hc, xx[i], yy[i], zz[i], xy.x, xy.y, S::pz()[jj], sE[jj]);
+            const double pz0 = S::pz()[jj];
+            double px = xy.x, py = xy.y, pz = pz0;
+            const double w = Q.dt / sE[jj];                   // PAPER.md:34 Eq. 2 with c = 1; E = |p| as in S1
+            double x = xa + px * w;
+            double y = ya + py * w;
+            double z = za + pz * w;
+            reflect_axis(x, px, P.g.L[0]);
+            reflect_axis(y, py, P.g.L[1]);
+            reflect_axis(z, pz, P.g.L[2]);
+            const int dx = axis_index(x, P.g.inv_d[0], P.g.nc[0]) - ix0 + 1;
+            const int dy = axis_index(y, P.g.inv_d[1], P.g.nc[1]) - iy0 + 1;
+            const int dz = axis_index(z, P.g.inv_d[2], P.g.nc[2]) - iz0 + 1;
+            int d = ((unsigned)dx <= 2u && (unsigned)dy <= 2u && (unsigned)dz <= 2u) ? (dx * 9 + dy * 3 + dz) : -1;
             if (j >= n) d = 31;                                   // not a particle
             else if (d < 0) { atomicOr(P.flags, kFlagMoved); d = 30; }   // dropped from the placement, as in k_scatter
             const uint32_t peers = __match_any_sync(0xFFFFFFFFu, d);
             if (d < kDirs && (peers & lanemask_lt()) == 0) T::ball()[(it * W + wid) * kDirs + d] = peers;
-            if (j < n) T::dir()[j] = (uint16_t)d;
-        }
-    }
-    __syncthreads();
-    // ---- prefix of the row masks per direction (27 threads walk the rows) ------------------------------
-    if (tid < kDirs) {
-        uint32_t run = 0;
-#pragma unroll 4
-        for (int r = 0; r < ROWS; ++r) {
-            T::pref()[r * kDirs + tid] = (uint16_t)run;
-            run += __popc(T::ball()[r * kDirs + tid]);
-        }
-        tab->total[tid] = run;
-        if (tab->dst_cnt[tid] != 0xFFFFFFFFu) Q.out.cnt[tab->dst_cnt[tid]] = min(run, tab->dst_cap[tid]);
-        if (run > tab->dst_cap[tid]) atomicOr(P.flags, kFlagSlots);          // capacity: the host redoes the run on the compact path
-    }
-    __syncthreads();
-    // ---- tail, pass 2: S1-S2 exactly, stable rank, write into the destination's inbox -------------------
-#pragma unroll 1
-    for (int g = 0; g < ITEMS / HB; ++g) {
-        if ((uint32_t)(g * HB * THREADS) >= n) break;
-        double xx[HB], yy[HB], zz[HB];
-#pragma unroll
-        for (int i = 0; i < HB; ++i) {
-            const uint32_t jc = min((uint32_t)(tid + (g * HB + i) * THREADS), last);
-            const uint32_t src = FROM_SLOTS ? slot_source(tab, jc) : lo + jc;
-            xx[i] = Q.in.x[src]; yy[i] = Q.in.y[src]; zz[i] = Q.in.z[src];
-        }
-#pragma unroll
-        for (int i = 0; i < HB; ++i) {
-            const int it = g * HB + i;
-            const uint32_t j = tid + it * THREADS;
             if (j < n) {
-                const double2 xy = S::pxy()[j];
-                double x = xx[i], y = yy[i], z = zz[i], px = xy.x, py = xy.y, pz = S::pz()[j];
-                const double w = Q.dt / sE[j];                    // PAPER.md:34 Eq. 2 with c = 1; E = |p| as in S1
-                x = x + px * w;
-                y = y + py * w;
-                z = z + pz * w;
-                reflect_axis(x, px, P.g.L[0]);
-                reflect_axis(y, py, P.g.L[1]);
-                reflect_axis(z, pz, P.g.L[2]);
-                const uint32_t d = T::dir()[j];
-                if (d < (uint32_t)kDirs) {
-                    const uint32_t row = (uint32_t)(it * W + wid) * kDirs + d;
-                    const uint32_t rank = T::pref()[row] + __popc(T::ball()[row] & lanemask_lt());
-                    if (rank < tab->dst_cap[d]) {
-                        const uint32_t dst = tab->dst_base[d] + rank;
-                        Q.out.x[dst] = x; Q.out.y[dst] = y; Q.out.z[dst] = z;
-                        Q.out.px[dst] = px; Q.out.py[dst] = py; Q.out.pz[dst] = pz;
-                        Q.out.pid[dst] = S::pid()[j];
-                    }
+                sE[j] = x;                                        // only this thread reads the slot again
+                if (px != xy.x || py != xy.y || pz != pz0) {      // reflected off a wall: rare
+                    S::pxy()[j] = make_double2(px, py); S::pz()[j] = pz;
+                }
+            }
+            Y[it] = y; Z[it] = z;
+            dpk |= (uint32_t)d << (5 * it);
+            xa = xn; ya = yn; za = zn;
+        }
+    }
+    __syncthreads();
+    // ---- exclusive prefix of the row masks per direction: 27 directions x 8 chunks of rows, 8 adjacent lanes each ----
+    {
+        constexpr int RCH = (ROWS + 7) / 8;
+#pragma unroll 1
+        for (int e0 = 0; e0 < kDirs * 8; e0 += THREADS) {
+            const int e = e0 + tid;
+            const bool valid = e < kDirs * 8;
+            const int d = min(e >> 3, kDirs - 1), q = e & 7;
+            uint32_t v[RCH], sum = 0;
+#pragma unroll
+            for (int r = 0; r < RCH; ++r) {
+                const int row = q * RCH + r;
+                v[r] = row < ROWS ? (uint32_t)__popc(T::ball()[row * kDirs + d]) : 0u;
+                sum += v[r];
+            }
+            uint32_t inc = sum;
+#pragma unroll
+            for (int o = 1; o < 8; o <<= 1) {
+                const uint32_t t = __shfl_up_sync(0xFFFFFFFFu, inc, o, 8);
+                if (q >= o) inc += t;
+            }
+            uint32_t run = inc - sum;
+            if (valid) {
+#pragma unroll
+                for (int r = 0; r < RCH; ++r) {
+                    const int row = q * RCH + r;
+                    if (row < ROWS) T::pref()[row * kDirs + d] = (uint16_t)run;
+                    run += v[r];
+                }
+                if (q == 7) {                 // inc: all particles of the cell that leave in direction d
+                    const uint32_t cap = tab->dst_cap[d], at = tab->dst_cnt[d];
+                    if (at != 0xFFFFFFFFu) Q.out.cnt[at] = min(inc, cap);
+                    if (inc > cap) atomicOr(P.flags, kFlagSlots);          // capacity: the host redoes the run on the compact path
+                }
+            }
+        }
+    }
+    __syncthreads();
+    // ---- tail, pass 2: stable rank, write into the destination's inbox ------------------------------------
+#pragma unroll
+    for (int it = 0; it < ITEMS; ++it) {
+        if (it < nit) {
+            const uint32_t j = tid + it * THREADS;
+            const uint32_t d = (dpk >> (5 * it)) & 31u;
+            if (j < n && d < (uint32_t)kDirs) {
+                const uint32_t row = (uint32_t)(it * W + wid) * kDirs + d;
+                const uint32_t rank = T::pref()[row] + __popc(T::ball()[row] & lanemask_lt());
+                if (rank < tab->dst_cap[d]) {
+                    const uint32_t dst = tab->dst_base[d] + rank;
+                    const double2 xy = S::pxy()[j];
+                    Q.out.x[dst] = sE[j]; Q.out.y[dst] = Y[it]; Q.out.z[dst] = Z[it];
+                    Q.out.px[dst] = xy.x; Q.out.py[dst] = xy.y; Q.out.pz[dst] = S::pz()[j];
+                    Q.out.pid[dst] = S::pid()[j];
                 }
             }
         }
@@ -363,10 +416,10 @@ k_slot_step(CollideParams P, SlotParams Q)
     constexpr int LCAP = collide_list_cap(CAP);
     __shared__ uint32_t s_warp[32];
     __shared__ CtaStats s_stats;
-    __shared__ SlotCell s_tab;
+    __shared__ SlotCell s_tab[2];
     const uint32_t nlist = *P.list_count;
-    if (threadIdx.x == 0) s_stats.near = 0;
-    ThreadStats acc{0ull, 0ull, 0u};
+    __shared__ uint32_t s_vnext[32];
+    if (threadIdx.x == 0) { s_stats.near = 0; s_stats.hits = 0; s_stats.pairs = 0; s_stats.rounds = 0; }
     __shared__ uint32_t s_item[2];
     if (threadIdx.x == 0) s_item[0] = atomicAdd(P.work, 1u);
     __syncthreads();
@@ -379,14 +432,15 @@ k_slot_step(CollideParams P, SlotParams Q)
         item = s_item[(it + 1) & 1];
         uint4 nxt = make_uint4(0u, 0u, 0u, 0u);
         if (item < nlist) nxt = P.list[item];
-        step_cell_slots<THREADS, ITEMS, G, CAP, LCAP, MODE>(P, Q, cur.x, cur.y, cur.z, s_warp, &s_stats, &s_tab, acc, nxt.x, nxt.y, nxt.z);
+        step_cell_slots<THREADS, ITEMS, G, CAP, LCAP, MODE>(P, Q, cur.x, cur.y, cur.z, s_warp, &s_stats, &s_tab[it & 1], &s_tab[(it + 1) & 1], it > 0,
+                                                            s_vnext, nxt.x, nxt.y, nxt.z);
         __syncthreads();
         cur = nxt;
     }
-    if ((threadIdx.x & 31) == 0 && acc.hits) atomicAdd(&P.counters[1], (unsigned long long)acc.hits);
-    if (threadIdx.x == 0) {
-        if (acc.pairs) atomicAdd(&P.counters[0], acc.pairs);
-        if (acc.rounds) atomicAdd(&P.counters[2], acc.rounds);
+    if (threadIdx.x == 0) {       // the loop ends with a block barrier
+        if (s_stats.hits) atomicAdd(&P.counters[1], (unsigned long long)s_stats.hits);
+        if (s_stats.pairs) atomicAdd(&P.counters[0], s_stats.pairs);
+        if (s_stats.rounds) atomicAdd(&P.counters[2], s_stats.rounds);
         if (s_stats.near) atomicAdd(&P.counters[3], (unsigned long long)s_stats.near);
     }
 }
