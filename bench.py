@@ -294,25 +294,32 @@ def main():
     if rank:
         w.seed = w.seed + 1000 * rank
     host = [torch.from_numpy(a).pin_memory() for a in w.arrays()]
-    sim = cuba.Cuba(w.box, w.ncell, *[h.to(dev) for h in host], w.n_test, w.seed)
     n = w.n
     fused = not args.no_fuse
-    sim.set_option(1, 1 if fused else 0)
-    if args.slots >= 0:
-        sim.set_option(3, args.slots)
     bytes_collide = BYTES_COLLIDE_FUSED if fused else BYTES_COLLIDE
+
+    def fresh():
+        """A context on a fresh device copy of the initial state, warmed up: every repeat (and the per-kernel
+        pass) times the SAME steps W..W+K of the run -- the cost of a step drifts as the Riemann profile evolves
+        (fewer cells need a second round), so consecutive blocks of K steps are not repeats of one another."""
+        sm = cuba.Cuba(w.box, w.ncell, *[h.to(dev) for h in host], w.n_test, w.seed)
+        sm.set_option(1, 1 if fused else 0)
+        if args.slots >= 0:
+            sm.set_option(3, args.slots)
+        sm.step(args.warmup, w.dt, w.sigma)
+        return sm
 
     sampler = ClockSampler(local)
     sampler.start()
 
-    # ---- warm-up, then the timed region: K steps, CUDA events on the launching stream, profiling OFF
-    # (the configuration a user runs); repeated, the line reports the median repeat (and the best) ----
-    sim.step(args.warmup, w.dt, w.sigma)
-    barrier()
-    c0 = sim.counters()
-    l0 = cuba.launch_count()
-    reps = []
+    # ---- W warm-up steps, then the timed region: K steps, CUDA events on the launching stream, profiling OFF
+    # (the configuration a user runs); repeated from the same initial state, the line reports the median ----
+    reps, pairs, launches = [], 0, 0
     for _ in range(args.repeats):
+        sim = fresh()
+        barrier()
+        c0 = sim.counters()
+        l0 = cuba.launch_count()
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         sampler.armed = True
@@ -322,14 +329,18 @@ def main():
         barrier()
         sampler.armed = False
         reps.append(ev0.elapsed_time(ev1))
+        launches = cuba.launch_count() - l0
+        c1 = sim.counters()
+        pairs = c1.pairs - c0.pairs
+        if c1.device_flags:
+            raise SystemExit("device error flags %d" % c1.device_flags)
+        sim.close()
+        del sim
     ms = float(np.median(reps))
-    launches = (cuba.launch_count() - l0) // args.repeats
-    c1 = sim.counters()
-    pairs = (c1.pairs - c0.pairs) / args.repeats
-    if c1.device_flags:
-        raise SystemExit("device error flags %d" % c1.device_flags)
 
-    # ---- per-kernel split: a separate pass of K steps with a CUDA event after every launch ----
+    # ---- per-kernel split: a separate pass over the same K steps with a CUDA event after every launch ----
+    sim = fresh()
+    barrier()
     sim.profile_enable(args.profile_mode)
     sim.step(args.steps, w.dt, w.sigma)
     prof = sim.profile_read()
@@ -414,7 +425,8 @@ def main():
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "repeats": {"n": args.repeats, "ms_per_step": [round(r / args.steps, 5) for r in reps],
                         "median": ms / args.steps, "best": min(reps) / args.steps,
-                        "note": "value and ms_per_step are the median repeat; profiling off in the timed region"},
+                        "note": "every repeat times steps W..W+K from the same initial state (the step cost drifts as the profile evolves); "
+                                "value and ms_per_step are the median repeat; profiling off in the timed region"},
             "config": {"workload": workloads_name(args.config), "n_particles": n, "ncells": sim.ncells,
                        "l2": "inputs larger than L2 (%.2f GB state per copy vs 126 MB L2), no flush" % (52 * n / 1e9)
                        if 52 * n > 4 * 126e6 else "state comparable to L2: cache-resident, not a roofline config",

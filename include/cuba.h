@@ -150,12 +150,14 @@ int cuba_step_adaptive(cuba_ctx *ctx, int nsteps, double dt_max, double sigma, d
  * can be captured (not the legacy default stream or cudaStreamPerThread) and per-kernel profiling
  * is off.  value 0: plain launches.  Results are identical either way. */
 #define CUBA_OPT_GRAPH 2
-/* CUBA_OPT_SLOTS (default 1): schedule of cuba_step.  1: a call of at least 4 steps on a problem that is
+/* CUBA_OPT_SLOTS (default 0): schedule of cuba_step.  0: the compact schedule (histogram, scan, scatter,
+ * collide) on the caller's arrays and workspace only.  1: a call of at least 4 steps on a problem that is
  * not launch-bound runs on the slotted store (one kernel per step and size class);
- * 2: every call does; 0: never (the compact schedule: histogram, scan, scatter, collide).  The
- * slotted store is device memory allocated by the library on first use (two copies of
- * ncells * slots-per-cell * 52 bytes) and freed by cuba_destroy; if the allocation fails the compact
- * schedule runs.  Results are bit-identical for every setting. */
+ * 2: every call does.  The slotted store is device memory allocated BY THE LIBRARY on first use (two
+ * copies of ncells * slots-per-cell * 52 bytes, 7 GB at 25M particles) and freed by cuba_destroy -- the
+ * one exception to "the caller owns all device memory", which is why it is opt-in; if the allocation
+ * fails the compact schedule runs.  Measured at 25M particles: 1.64 vs 1.65 ms per step.  Results are
+ * bit-identical for every setting. */
 #define CUBA_OPT_SLOTS 3
 /* CUBA_OPT_SLOT_MARGIN (default 100): per cent by which the segment capacities of the slotted store
  * are scaled, 1..1000.  A run that outgrows a capacity is detected at the next synchronising call and
@@ -163,6 +165,11 @@ int cuba_step_adaptive(cuba_ctx *ctx, int nsteps, double dt_max, double sigma, d
  * Synchronises if a slotted run is still unverified; releases the slotted store. */
 #define CUBA_OPT_SLOT_MARGIN 4
 int cuba_set_option(cuba_ctx *ctx, int option, int value);
+/* Diagnostics of the slotted schedule (CUBA_OPT_SLOTS): HOST out[0] = calls of cuba_step that ran on the
+ * slotted store since cuba_init, out[1] = those that outgrew a segment and were redone on the compact
+ * schedule.  Verifies a pending run first (synchronises then).  Errors: CUBA_ERR_NULL, or what the
+ * redone run returned. */
+int cuba_slot_stats(cuba_ctx *ctx, uint64_t out[2]);
 
 /* PAPER.md:66 (total energy) and PAPER.md:68-70 Fig. 2 (energy density along x).
  * total = (sum E, sum px, sum py, sum pz) in GeV; edens[j] = sum_{i in slab j} E_i /

@@ -15,7 +15,7 @@ EXPORTS = ("cuba_workspace_bytes", "cuba_init", "cuba_step", "cuba_observables",
            "cuba_get_particles", "cuba_get_cells", "cuba_step_traced", "cuba_counters", "cuba_run_host", "cuba_destroy",
            "cuba_strerror", "cuba_last_cuda_error", "cuba_launch_count", "cuba_profile_enable",
            "cuba_profile_read", "cuba_profile_name", "cuba_set_option", "cuba_observables_lrf",
-           "cuba_step_adaptive", "cuba_step_local_sigma", "cuba_probe_fp64")
+           "cuba_step_adaptive", "cuba_step_local_sigma", "cuba_probe_fp64", "cuba_slot_stats")
 
 
 # cuba_set_option
@@ -115,6 +115,7 @@ def lib():
         L.cuba_step_local_sigma.argtypes = [c_void_p, c_int, c_double, c_double]
         L.cuba_profile_read.argtypes = [c_void_p, dp, POINTER(c_uint64)]
         L.cuba_probe_fp64.argtypes = [c_void_p, c_int, dp]
+        L.cuba_slot_stats.argtypes = [c_void_p, POINTER(c_uint64)]
         L.cuba_profile_name.argtypes = [c_int]
         L.cuba_profile_name.restype = c_char_p
         _lib = L
@@ -275,6 +276,12 @@ class Cuba:
     def set_option(self, option: int, value: int):
         """cuba_set_option (OPT_FUSE_HIST, OPT_GRAPH, OPT_SLOTS, OPT_SLOT_MARGIN)."""
         _check(lib().cuba_set_option(self._h, int(option), int(value)))
+
+    def slot_stats(self):
+        """cuba_slot_stats: (calls run on the slotted store, of which redone on the compact schedule)."""
+        out = (c_uint64 * 2)()
+        _check(lib().cuba_slot_stats(self._h, out))
+        return int(out[0]), int(out[1])
 
     def profile_enable(self, mode=1):
         """0 off, 1 per-kernel events (collision classes as one concurrent group), 2 classes serialised."""

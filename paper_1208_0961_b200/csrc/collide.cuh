@@ -618,6 +618,8 @@ __host__ __device__ constexpr size_t collide_smem_bytes(int cap, int threads, in
 // hits are scattered.  first: the energies are computed here and left in sE (see above).  The pairs
 // are dealt to the warps in rows of 32, round-robin (the hits, and with them the scatter work, are
 // then spread evenly: a warp rarely has more than 32); a warp skips the rows beyond the last pair.
+// (Measured and rejected: the decisions of a warp's three rows interleaved through register arrays,
+// hot class 0.788 -> 0.804 ms.)
 template <typename S, int THREADS, int PITEMS, bool TRACE>
 __device__ __forceinline__ void pair_phase(const CollideParams &P, uint32_t c, uint32_t n, uint32_t tcur, int rho,
                                             int slot, bool first, bool keepE, CtaStats *stats)

@@ -143,7 +143,7 @@ struct cuba_ctx {
     bool fuse_hist = true;   // CUBA_OPT_FUSE_HIST
     double pre_dt = 0.0;     // > 0: cnt / carry already hold the histogram of the next step for this dt
     // ---- slotted schedule (slots.cuh): one kernel per step on a store with a fixed region per cell ----
-    int slot_mode = 1;            // CUBA_OPT_SLOTS: 0 never, 1 for calls of >= kSlotMinSteps steps, 2 for every call
+    int slot_mode = 0;            // CUBA_OPT_SLOTS: 0 never (default), 1 for calls of >= kSlotMinSteps steps, 2 for every call
     double slot_margin = 1.0;     // CUBA_OPT_SLOT_MARGIN (percent): scales the segment capacities (tests force overflows)
     double slot_boost = 1.0;      // grows after an overflow so that the next geometry is roomier
     unsigned char *slot_mem = nullptr;   // library-owned device memory: two slotted copies + the counter backup
@@ -1104,6 +1104,14 @@ int cuba_set_option(cuba_ctx *ctx, int option, int value)
     ctx->fuse_hist = value != 0;
     if (!ctx->fuse_hist) ctx->pre_dt = 0.0;
     return CUBA_OK;
+}
+
+int cuba_slot_stats(cuba_ctx *ctx, uint64_t out[2])
+{
+    if (!ctx || !out) return CUBA_ERR_NULL;
+    const int rc = settle(ctx);      // a pending run is verified (and redone if it outgrew a segment) first
+    out[0] = ctx->slot_runs; out[1] = ctx->slot_replays;
+    return rc;
 }
 
 int cuba_observables(cuba_ctx *ctx, double total[4], int nslab, double *edens)

@@ -19,7 +19,7 @@ def cuba():
 def declared_symbols():
     text = open(os.path.join(ROOT, "include", "cuba.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(cuba_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(cuba_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_library_exports_every_declared_symbol(cuba):

@@ -337,6 +337,96 @@ def test_fused_histogram_schedule_is_bit_identical(cuba, oracle_mod):
         fused.set_option(99, 1)
 
 
+def test_slotted_schedule_is_bit_identical(cuba, oracle_mod):
+    """CUBA_OPT_SLOTS (opt-in): every cell owns a fixed region of 27 inbox segments and a call of n steps is
+    n + 1 passes of one kernel per size class.  Same bits as the compact schedule and the oracle: calls of
+    every length, a change of dt, a traced step in between, observables read from the packed result,
+    counters; the library reports that the slotted store really ran and that nothing had to be redone."""
+    w = workloads.riemann(L=(6.0, 3.0, 2.0), ncell=(12, 3, 2), r_test=90.0, sigma_gev2=50.0, dt=0.05, seed=31)
+    slots, compact = cuba.Cuba.from_workload(w), cuba.Cuba.from_workload(w)
+    slots.set_option(3, 2)
+    compact.set_option(3, 0)
+    o = oracle_mod.Oracle.from_workload(w)
+    for k, dt in [(1, w.dt), (4, w.dt), (2, 0.5 * w.dt), (7, w.dt), (3, w.dt)]:
+        slots.step(k, dt, w.sigma)
+        compact.step(k, dt, w.sigma)
+        o.step(k, dt, w.sigma)
+        for a, b, c in zip(slots.particles(), compact.particles(), o.particles()):
+            assert np.array_equal(a, b) and np.array_equal(a, c)
+        assert np.array_equal(slots.cell_start(), o.cells()[1])
+    slots.step_traced(w.dt, w.sigma)
+    o.step(1, w.dt, w.sigma)
+    slots.step(5, w.dt, w.sigma)
+    o.step(5, w.dt, w.sigma)
+    for a, c in zip(slots.particles(), o.particles()):
+        assert np.array_equal(a, c)
+    gt, ge = slots.observables(w.nslab)
+    ot, oe = o.observables(w.nslab)
+    assert np.allclose(ge, oe, rtol=1e-12, atol=0) and abs(gt[0] - ot[0]) <= 1e-12 * ot[0]
+    cs, co = slots.counters(), o.counters()
+    assert (cs.pairs, cs.collisions, cs.rounds) == (co["pairs"], co["collisions"], co["rounds"])
+    assert cs.device_flags == 0
+    runs, replays = slots.slot_stats()
+    assert runs >= 6 and replays == 0
+    assert compact.slot_stats() == (0, 0)
+    # mode 1: only calls of at least 4 steps go to the slotted store
+    m1 = cuba.Cuba.from_workload(w)
+    m1.set_option(3, 1)
+    m1.step(3, w.dt, w.sigma)
+    assert m1.slot_stats()[0] == 0
+    m1.step(4, w.dt, w.sigma)
+    assert m1.slot_stats() == (1, 0)
+
+
+def test_slotted_run_that_outgrows_a_segment_is_redone_on_the_compact_schedule(cuba, oracle_mod):
+    """CUBA_OPT_SLOT_MARGIN: with the segment capacities cut to a fraction, a run overflows an inbox segment;
+    that is detected at the next synchronising call and the run is redone on the compact schedule from the
+    untouched copy it started from -- the result never depends on the capacities."""
+    w = workloads.riemann(L=(6.0, 3.0, 2.0), ncell=(12, 3, 2), r_test=90.0, sigma_gev2=50.0, dt=0.05, seed=32)
+    g = cuba.Cuba.from_workload(w)
+    g.set_option(3, 2)
+    g.set_option(4, 5)          # 5 % of the usual capacities
+    o = oracle_mod.Oracle.from_workload(w)
+    for k in (3, 6):
+        g.step(k, w.dt, w.sigma)
+        o.step(k, w.dt, w.sigma)
+        for a, c in zip(g.particles(), o.particles()):
+            assert np.array_equal(a, c)
+    runs, replays = g.slot_stats()
+    assert runs >= 1 and replays >= 1
+    cg, co = g.counters(), o.counters()
+    assert (cg.pairs, cg.collisions, cg.rounds) == (co["pairs"], co["collisions"], co["rounds"])
+    assert cg.device_flags == 0
+
+
+@pytest.mark.parametrize("n", [129, 513, 897, 1537, 2049, 4545])
+def test_slotted_schedule_in_every_size_class(cuba, oracle_mod, n):
+    """CUBA_OPT_SLOTS with one cell of n particles next to a thin one, particles spread over the whole cells so
+    that movers cross the face both ways; two rounds in the big cell.  n = 4545 is beyond the largest
+    shared-memory class: the slotted store declines (or flags) it and the compact schedule does the run."""
+    base_w = workloads.thermal_box(L=(2.0, 1.0, 1.0), ncell=(2, 1, 1), count=n + 77, seed=200 + n)
+    rng = np.random.default_rng(n)
+    pos = rng.uniform(0.0, 1.0, (3, n + 77))
+    pos[0, n:] += 1.0
+    r_test, dt = 2.0, 0.1
+    cn = n if n % 2 else n - 1
+    sigma = (1.5 / (2.0 * cn)) * r_test * 1.0 / dt    # pmax = 1.5 in the big cell: R = 2
+    w = workloads.Workload("slots_class_%d" % n, (2.0, 1.0, 1.0), (2, 1, 1), r_test, sigma, dt, 1, 200 + n, 2,
+                           pos[0].copy(), pos[1].copy(), pos[2].copy(), base_w.px, base_w.py, base_w.pz)
+    g = cuba.Cuba.from_workload(w)
+    g.set_option(3, 2)
+    o = oracle_mod.Oracle.from_workload(w)
+    for k in (2, 3):
+        g.step(k, w.dt, w.sigma)
+        o.step(k, w.dt, w.sigma)
+        assert_state_equal(g.particles(), o.particles())
+    cg, co = g.counters(), o.counters()
+    assert (cg.pairs, cg.collisions, cg.rounds) == (co["pairs"], co["collisions"], co["rounds"])
+    assert cg.device_flags == 0
+    runs, replays = g.slot_stats()
+    assert (runs >= 1) if n < 4000 else (runs == 0 or replays == runs)
+
+
 @pytest.mark.parametrize("case", ["single", "two", "one_cell_overflow", "flat_grid", "empty_cells"])
 def test_edge_cases_match_oracle(cuba, oracle_mod, case):
     rng = np.random.default_rng(77)
