@@ -46,7 +46,7 @@ BYTES_STEP_FUSED = BYTES_SCATTER + BYTES_COLLIDE_FUSED           # 180: what the
 # ncu evidence: the raw per-launch metric export of one step under profiles/ (written by the command named in
 # the .md beside it), keyed by a hash of the kernel sources so that a stale capture reads as null, never as a
 # number.  Metrics: dram__bytes_read.sum, dram__bytes_write.sum, smsp__inst_executed.sum,
-# smsp__inst_executed_pipe_fp64.sum (warp-level), gpu__time_duration.sum, launch__registers_per_thread,
+# sm__inst_executed_pipe_fp64.sum (warp-level), gpu__time_duration.sum, launch__registers_per_thread,
 # sm__warps_active.avg.pct_of_peak_sustained_active.
 NCU_EXPORT = os.path.join(ROOT, "profiles", "r02_ncu_step_c%d.csv")
 ISSUE_SLOTS_PER_CLOCK = 148 * 4
@@ -78,8 +78,15 @@ def ncu_export(config):
     if sha != kernel_source_hash():
         return None, "stale: kernel sources changed since %s was captured" % os.path.relpath(path, ROOT)
     rows = list(csv.DictReader([l for l in lines if l.startswith('"')]))
+    # the export lists every launch of a short run; ONE step = the last launch of every distinct kernel
+    # instantiation (the size classes of k_collide are distinct instantiations)
+    last_id = {}
+    for r in rows:
+        last_id[r["Kernel Name"]] = r["ID"]
     out = {}
     for r in rows:
+        if last_id[r["Kernel Name"]] != r["ID"]:
+            continue
         name = r["Kernel Name"].replace("void ", "").replace("cuba::", "")
         base = name.split("<")[0].split("(")[0]
         try:
@@ -95,6 +102,26 @@ def ncu_export(config):
         else:
             d[m] = d.get(m, 0.0) + v * scale
     return out, os.path.relpath(path, ROOT)
+
+
+def import_ncu(raw_csv, config):
+    """`python bench.py --import-ncu <ncu --csv log> --config C`: writes the tracked export profiles/r02_ncu_step_cC.csv:
+    the rows of the LAST launch of every kernel instantiation (one step), headed by the hash of the kernel
+    sources they were measured on."""
+    import csv
+    with open(raw_csv) as f:
+        lines = [l for l in f.read().splitlines() if l.startswith('"')]
+    rows = list(csv.DictReader(lines))
+    last_id = {}
+    for r in rows:
+        last_id[r["Kernel Name"]] = r["ID"]
+    keep = [lines[0]] + [l for l, r in zip(lines[1:], rows) if last_id[r["Kernel Name"]] == r["ID"]]
+    path = NCU_EXPORT % config
+    with open(path, "w") as f:
+        f.write("# source_sha256: %s  (csrc/*.cu, *.cuh this export was measured on; bench.py reports null once they change)\n"
+                % kernel_source_hash())
+        f.write("\n".join(keep) + "\n")
+    print("wrote %s: %d rows of %d kernel instantiations" % (os.path.relpath(path, ROOT), len(keep) - 1, len(last_id)))
 
 
 def issue_roofline(warp_inst, ms, clocks, source):
@@ -119,7 +146,7 @@ def fp64_roofline(fp64_warp_inst, ms, peak_dfma_per_s, source):
     peak = peak_dfma_per_s / 32.0 / 1e9
     return {"bound": "fp64", "achieved": achieved, "peak": peak, "unit": "G fp64 warp-inst/s", "frac": achieved / peak,
             "peak_tflops": 2.0 * peak_dfma_per_s / 1e12,
-            "source": "smsp__inst_executed_pipe_fp64.sum from %s / CUDA-event duration; peak = cuba_probe_fp64 (this run)" % source}
+            "source": "sm__inst_executed_pipe_fp64.sum from %s / CUDA-event duration; peak = cuba_probe_fp64 (this run)" % source}
 
 
 def peaks():
@@ -259,10 +286,14 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-fuse", action="store_true", help="run the separate k_stream_hist pass every step (A/B diagnostic)")
     ap.add_argument("--slots", type=int, default=-1, help="CUBA_OPT_SLOTS: 0 compact schedule, 1/2 slotted schedule; -1 library default (A/B diagnostic)")
+    ap.add_argument("--import-ncu", default=None, help="ncu --csv log of a short bench run: write the tracked export under profiles/ and exit")
     ap.add_argument("--repeats", type=int, default=3, help="timed repeats of K steps each; the line reports the median")
     ap.add_argument("--profile-mode", type=int, default=1, help="1: normal operation; 2: serialise the collision classes (diagnostic)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuba" else args.warmup
+    if args.import_ncu:
+        import_ncu(args.import_ncu, args.config)
+        return
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -444,11 +475,11 @@ def main():
                          "alg_bytes_per_launch": alg.get(dom, 0),
                          "duration_source": "CUDA events after every launch in a separate pass of %d steps (cuba_profile_enable)" % args.steps,
                          "ncu_source": ncu_src,
-                         "ncu": {k: nk.get(k) for k in ("smsp__inst_executed.sum", "smsp__inst_executed_pipe_fp64.sum",
+                         "ncu": {k: nk.get(k) for k in ("smsp__inst_executed.sum", "sm__inst_executed_pipe_fp64.sum",
                                                          "launch__registers_per_thread",
                                                          "sm__warps_active.avg.pct_of_peak_sustained_active")} if nk else None,
                          "issue": issue_roofline(nk.get("smsp__inst_executed.sum"), dom_ms, clk, ncu_src),
-                         "fp64": fp64_roofline(nk.get("smsp__inst_executed_pipe_fp64.sum"), dom_ms, fp64_peak, ncu_src),
+                         "fp64": fp64_roofline(nk.get("sm__inst_executed_pipe_fp64.sum"), dom_ms, fp64_peak, ncu_src),
                          "fp64_peak_measured": {"dfma_per_s": fp64_peak, "tflops": 2.0 * fp64_peak / 1e12,
                                                 "source": "cuba_probe_fp64: 8 dependent DFMA chains per thread, 8 CTAs x 256 threads per SM, best of 5"},
                          "step": {"alg_bytes_per_particle": BYTES_STEP,

@@ -329,10 +329,14 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
     if (const char *e = getenv("CUBA_DEBUG_GRID_C4")) ctx->grid_cls[4] = atoi(e) * sms;      // experiments only
     if (const char *e = getenv("CUBA_DEBUG_GRID_SCAT")) ctx->grid_scat = atoi(e) * sms;
     ctx->grid_o = sms;
-    if (!cuda_ok(cudaFuncSetAttribute(k_observe_partial<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    if (!cuda_ok(cudaFuncSetAttribute(k_observe_partial<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       kObsWarps * kObsMaxSlabs * 8), "cudaFuncSetAttribute")) return fail(CUBA_ERR_CUDA);
-    if (!cuda_ok(cudaFuncSetAttribute(k_observe_partial<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    if (!cuda_ok(cudaFuncSetAttribute(k_observe_partial<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       kObsWarps * kLrfComp * kLrfMaxSlabs * 8), "cudaFuncSetAttribute")) return fail(CUBA_ERR_CUDA);
+    if (!cuda_ok(cudaFuncSetAttribute(k_observe_partial<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      kObsWarps * (kObsMaxSlabs + kObsWindowMax * 32) * 8), "cudaFuncSetAttribute")) return fail(CUBA_ERR_CUDA);
+    if (!cuda_ok(cudaFuncSetAttribute(k_observe_partial<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      kObsWarps * kLrfComp * (kLrfMaxSlabs + kLrfWindowMax * 32) * 8), "cudaFuncSetAttribute")) return fail(CUBA_ERR_CUDA);
 
     cudaStream_t st = ctx->stream;
     auto body = [&]() -> int {
@@ -1125,8 +1129,16 @@ int cuba_observables(cuba_ctx *ctx, double total[4], int nslab, double *edens)
     const double inv_w = (double)nslab / ctx->box[0];
     const double vol = ((ctx->n_test * (ctx->box[0] / (double)nslab)) * ctx->box[1]) * ctx->box[2];
     double *partial = ctx->at<double>(lay.obs_partial), *result = ctx->at<double>(lay.obs_result);
-    k_observe_partial<false><<<kObsGrid, kObsThreads, (size_t)kObsWarps * nslab * 8, st>>>(ctx->n, cur.x, cur.px, cur.py, cur.pz,
-                                                                                  inv_w, nslab, partial);
+    // slabs a layer of cells can touch; more than two: running sums in shared memory (observe.cuh, WIDE)
+    const int per_layer = (nslab + ctx->g.nc[0] - 1) / ctx->g.nc[0] + 1;
+    if (nslab > 2 * ctx->g.nc[0]) {
+        const int window = per_layer < kObsWindowMax ? per_layer : kObsWindowMax;
+        k_observe_partial<false, true><<<kObsGrid, kObsThreads, (size_t)kObsWarps * (nslab + window * 32) * 8, st>>>(
+            ctx->n, cur.x, cur.px, cur.py, cur.pz, inv_w, nslab, window, partial);
+    } else {
+        k_observe_partial<false, false><<<kObsGrid, kObsThreads, (size_t)kObsWarps * nslab * 8, st>>>(ctx->n, cur.x, cur.px, cur.py, cur.pz,
+                                                                                                 inv_w, nslab, 2, partial);
+    }
     LAUNCHED();
     k_observe_final<<<(4 + nslab + 7) / 8, 256, 0, st>>>(kObsGrid, nslab, partial, vol, result);
     LAUNCHED();
@@ -1151,8 +1163,15 @@ int cuba_observables_lrf(cuba_ctx *ctx, int nslab, double *T, double *lrf)
     double *partial = ctx->at<double>(lay.obs_partial), *result = ctx->at<double>(lay.obs_result);
     const int grid = 148 * 3;           // 3 CTAs per SM (2 when nslab needs more than 75 KB of shared memory each)
     static_assert(148 * 3 <= kObsGrid, "partial buffer is sized for kObsGrid blocks");
-    k_observe_partial<true><<<grid, kObsThreads, (size_t)kObsWarps * kLrfComp * nslab * 8, st>>>(ctx->n, cur.x, cur.px, cur.py, cur.pz,
-                                                                                              inv_w, nslab, partial);
+    const int per_layer = (nslab + ctx->g.nc[0] - 1) / ctx->g.nc[0] + 1;
+    if (nslab > 2 * ctx->g.nc[0]) {
+        const int window = per_layer < kLrfWindowMax ? per_layer : kLrfWindowMax;
+        k_observe_partial<true, true><<<grid, kObsThreads, (size_t)kObsWarps * kLrfComp * (nslab + window * 32) * 8, st>>>(
+            ctx->n, cur.x, cur.px, cur.py, cur.pz, inv_w, nslab, window, partial);
+    } else {
+        k_observe_partial<true, false><<<grid, kObsThreads, (size_t)kObsWarps * kLrfComp * nslab * 8, st>>>(ctx->n, cur.x, cur.px, cur.py, cur.pz,
+                                                                                                         inv_w, nslab, 2, partial);
+    }
     LAUNCHED();
     k_observe_lrf_final<<<(nslab + 7) / 8, 256, 0, st>>>(grid, nslab, partial, vol, result);
     LAUNCHED();

@@ -49,18 +49,46 @@ __device__ __forceinline__ void warp_flush(double (&acc0)[NC], double (&acc1)[NC
 //       w = 1/E and the contributions E, px, (px*px)*w, (py*py)*w, (pz*pz)*w; partial layout
 //       per block: [comp][nslab].
 // One HBM pass over x, px, py, pz (32 B per particle).
-template <bool LRF>
-__global__ void __launch_bounds__(kObsThreads, LRF ? 3 : 4)
+// WIDE (more than two slabs per layer of cells, nslab > 2 nx): the running sums live in shared memory
+//       instead of registers -- every lane owns a private column of `window` consecutive slabs
+//       [base, base + window) per component (index (s * NC + q) * 32 + lane: no bank conflicts, no
+//       atomics, the order of a lane's additions is the order of its particles), reduced over the
+//       lanes (shuffle trees) into the warp's bins when a particle falls outside the window.  Data-
+//       dependent only, like the register path: bit-reproducible.  Rows that span more than `window`
+//       slabs are peeled slab by slab as before.
+constexpr int kObsWindowMax = 32, kLrfWindowMax = 9;
+
+template <int NC>
+__device__ __forceinline__ void window_flush(double *wb, int window, int base, double *bins, int nslab, int lane)
+{
+    if (base < 0) return;
+    for (int s = 0; s < window && base + s < nslab; ++s) {
+#pragma unroll
+        for (int q = 0; q < NC; ++q) {
+            double r = wb[(s * NC + q) * 32 + lane];
+            wb[(s * NC + q) * 32 + lane] = 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) r += __shfl_xor_sync(0xFFFFFFFFu, r, o);
+            if (lane == 0) bins[q * nslab + base + s] += r;
+        }
+    }
+}
+
+template <bool LRF, bool WIDE>
+__global__ void __launch_bounds__(kObsThreads, WIDE ? 1 : (LRF ? 3 : 4))
 k_observe_partial(int64_t n, const double *__restrict__ x, const double *__restrict__ px,
                   const double *__restrict__ py, const double *__restrict__ pz, double inv_w,
-                  int nslab, double *__restrict__ partial)
+                  int nslab, int window, double *__restrict__ partial)
 {
     constexpr int NC = LRF ? kLrfComp : 1;
-    extern __shared__ double s_bins[];          // [kObsWarps][NC][nslab]
+    extern __shared__ double s_bins[];          // [kObsWarps][NC][nslab], WIDE: then [kObsWarps][window][NC][32]
     __shared__ double s_tot[kObsWarps][4];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     double *bins = s_bins + (size_t)wid * NC * nslab;
     for (int s = lane; s < NC * nslab; s += 32) bins[s] = 0.0;
+    double *wb = s_bins + (size_t)kObsWarps * NC * nslab + (size_t)wid * window * NC * 32;
+    if (WIDE)
+        for (int s = 0; s < window * NC; ++s) wb[s * 32 + lane] = 0.0;
     __syncwarp();
     double tE = 0.0, tx = 0.0, ty = 0.0, tz = 0.0;
     double acc0[NC], acc1[NC];
@@ -98,14 +126,16 @@ k_observe_partial(int64_t n, const double *__restrict__ x, const double *__restr
             }
             const int slab = valid ? min(max(__double2int_rz(xx[k] * inv_w), 0), nslab - 1) : -1;
             bool keep = true;
-            if (__any_sync(0xFFFFFFFFu, valid && (base < 0 || slab < base || slab > base + 1))) {
-                warp_flush<NC>(acc0, acc1, base, bins, nslab, lane);
+            const int span = WIDE ? window : 2;           // slabs the running sums cover: [base, base + span)
+            if (__any_sync(0xFFFFFFFFu, valid && (base < 0 || slab < base || slab >= base + span))) {
+                if (WIDE) window_flush<NC>(wb, window, base, bins, nslab, lane);
+                else warp_flush<NC>(acc0, acc1, base, bins, nslab, lane);
                 int m = valid ? slab : 0x7FFFFFFF;              // new base: the smallest slab present
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) m = min(m, __shfl_xor_sync(0xFFFFFFFFu, m, o));
                 base = m;
-                if (__any_sync(0xFFFFFFFFu, valid && slab > base + 1)) {
-                    // more than two slabs among these 32 particles (nslab > 2 nx): peel them off one
+                if (__any_sync(0xFFFFFFFFu, valid && slab >= base + span)) {
+                    // more slabs among these 32 particles than the running sums cover: peel them off one
                     // slab at a time straight into the bins; nothing is carried over
                     uint32_t todo = __ballot_sync(0xFFFFFFFFu, valid);
                     while (todo) {
@@ -126,7 +156,11 @@ k_observe_partial(int64_t n, const double *__restrict__ x, const double *__restr
                 }
             }
             if (keep && valid) {
-                if (slab == base) {
+                if (WIDE) {
+                    double *col = wb + (size_t)(slab - base) * NC * 32 + lane;
+#pragma unroll
+                    for (int q = 0; q < NC; ++q) col[q * 32] += v[q];
+                } else if (slab == base) {
 #pragma unroll
                     for (int q = 0; q < NC; ++q) acc0[q] += v[q];
                 } else {
@@ -136,7 +170,8 @@ k_observe_partial(int64_t n, const double *__restrict__ x, const double *__restr
             }
         }
     }
-    warp_flush<NC>(acc0, acc1, base, bins, nslab, lane);
+    if (WIDE) window_flush<NC>(wb, window, base, bins, nslab, lane);
+    else warp_flush<NC>(acc0, acc1, base, bins, nslab, lane);
     if (!LRF) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {

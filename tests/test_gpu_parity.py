@@ -159,6 +159,28 @@ def assert_lrf_equal(got, ref):
     assert np.all(np.abs(gl[2:] - ol[2:]) <= 1e-10 * scale), "P_L, P_T"
 
 
+def test_observables_with_many_slabs_per_cell_layer(cuba, oracle_mod):
+    """nslab > 2 nx: a layer of cells touches more than two slabs and the running sums live in per-lane
+    shared-memory columns over a window of slabs (observe.cuh, WIDE), beyond the window the peel loop:
+    energy density and tensor within 1e-12 / 1e-10 of the oracle, and bit-reproducible from call to call."""
+    w = workloads.riemann(L=(16.0, 4.0, 4.0), ncell=(16, 4, 4), r_test=10.0, seed=16)
+    g = cuba.Cuba.from_workload(w)
+    o = oracle_mod.Oracle.from_workload(w)
+    g.step(5, w.dt, w.sigma)
+    o.step(5, w.dt, w.sigma)
+    for nslab in (33, 40, 128, 500, 1024):          # windows of 4, 4, 9, 32 + peel, 32 + peel
+        gt, ge = g.observables(nslab)
+        ot, oe = o.observables(nslab)
+        assert np.allclose(ge, oe, rtol=REL, atol=0) and np.allclose(gt, ot, rtol=REL, atol=1e-9)
+        gt2, ge2 = g.observables(nslab)
+        assert np.array_equal(ge, ge2) and np.array_equal(gt, gt2)
+    for nslab in (33, 40, 100, 144, 256):           # tensor: windows of 4, 4, 8, 9 + peel, 9 + peel
+        a = g.observables_lrf(nslab)
+        assert_lrf_equal(a, o.observables_lrf(nslab))
+        b = g.observables_lrf(nslab)
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
 def test_lrf_observables_match_oracle(cuba, oracle_mod):
     """T00, T0x, Txx, Tyy, Tzz per slab and the Landau matching, on an evolving
     Riemann problem (a flow develops at the discontinuity), for several slab counts incl. the
