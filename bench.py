@@ -214,8 +214,8 @@ def oracle_sample_workload(config):
     if config == 3:
         w = workloads.riemann(L=(32.0, 8.0, 8.0), ncell=(64, 8, 8), r_test=40.0, sigma_gev2=50.0, dt=0.05, seed=4)
         return w, "configs[3] restricted to a 32x8x8 fm^3 transverse slice"
-    if config == 4:
-        w = workloads.skewed(L=(64.0, 8.0, 8.0), ncell=(64, 8, 8), r_test=100.0, seed=5)
+    if config in (4, 5):
+        w = workloads.skewed(L=(64.0, 8.0, 8.0), ncell=(64, 8, 8), r_test=100.0 if config == 4 else 185.5, seed=5)
         return w, "configs[4] restricted to a 64x8x8 fm^3 transverse slice"
     w = workloads.make(0)
     return w, "configs[0] whole"
@@ -272,7 +272,8 @@ def workloads_name(config):
             1: "configs[1] Riemann 32^3 fm^3, r_test=10 (2.49M particles)",
             2: "configs[2] Riemann 32^3 fm^3, T=0.4/0.2 GeV, r_test=100 (24.9M particles), sigma=10 GeV^-2, dt=0.1 fm/c",
             3: "configs[3] Riemann fine cells 0.5x1x1 fm, r_test=40 (9.96M particles), sigma=50 GeV^-2, dt=0.05",
-            4: "configs[4] skewed occupancy 64x32x32 fm^3, r_test=100 (53.9M particles)"}[config]
+            4: "configs[4] skewed occupancy 64x32x32 fm^3, r_test=100 (53.9M particles)",
+            5: "configs[4] at ~100M particles: skewed occupancy 64x32x32 fm^3, r_test=185.5 (100.0M particles)"}[config]
 
 
 def main():

@@ -233,6 +233,47 @@ int cuba_profile_enable(cuba_ctx *ctx, int on);
 int cuba_profile_read(cuba_ctx *ctx, double *ms_sum, uint64_t *launches);
 const char *cuba_profile_name(int group);
 
+/* ---- x-slab decomposition over several GPUs (collisions happen inside a
+ * cell only: dt below the cell edge) ----------------------------------------------------------------
+ * One context per rank.  A rank OWNS the cell layers [layer_lo, layer_hi) along x of the global grid and keeps a
+ * copy (ghost) of the adjacent boundary layer of each neighbour, all in the coordinates and cell numbering of
+ * the whole problem, so that every operation rounds exactly as on one GPU.  Protocol of one step, the same on
+ * every rank:  cuba_step(ctx, 1, dt, sigma)  ->  cuba_slab_count / cuba_slab_pack for side 0 (lowest owned layer)
+ * and side 1 (highest)  ->  send each buffer to that neighbour, receive theirs (torch.distributed / NCCL: the
+ * library does not communicate)  ->  cuba_slab_unpack.  The owned ranges of all ranks, concatenated in rank
+ * order, are the one-GPU store bit for bit (array order, positions, momenta, pids); counters add up.
+ *
+ * cuba_slab_init: like cuba_init, but the DEVICE arrays x..pz hold `capacity` doubles (room for the ghosts and for
+ * fluctuations), the first n entries given: ALL particles of the problem whose cell lies in the layers
+ * [layer_lo - 1, layer_hi + 1), in ascending order of their global index, and pid (DEVICE, n) those global
+ * indices.  workspace: cuba_workspace_bytes(capacity, ncell).  Every rank passes the same box, ncell, n_test, seed.
+ * In a slab context: cuba_step takes nsteps <= 1; the fused histogram, the CUDA graph and the slotted schedule
+ * are off; cuba_step_traced and cuba_step_adaptive return CUBA_ERR_VALUE; cuba_observables(_lrf) cover the owned
+ * particles only (add the ranks' results); cuba_get_particles / cuba_state give the whole local store, of which
+ * cuba_slab_owned names the owned part.  Errors as cuba_init, plus CUBA_ERR_SIZE (n > capacity) and
+ * CUBA_ERR_VALUE (layers). */
+int cuba_slab_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t capacity, int64_t n,
+                   double *x, double *y, double *z, double *px, double *py, double *pz, const uint32_t *pid,
+                   double n_test, uint64_t seed, void *workspace, size_t workspace_bytes, void *cuda_stream,
+                   int layer_lo, int layer_hi);
+/* HOST out[4] = first slot of the owned part of the current store, its length, particles in the store, capacity.
+ * Synchronises (reads four words back) once after a step. */
+int cuba_slab_owned(cuba_ctx *ctx, int64_t out[4]);
+/* HOST *count = particles in the owned boundary layer on `side` (0: layer_lo, 1: layer_hi - 1). */
+int cuba_slab_count(cuba_ctx *ctx, int side, int64_t *count);
+/* Bytes of a halo buffer for `count` particles: 16-byte header {count, cells per layer}, six double arrays,
+ * the pids, the population of every cell of the layer. */
+size_t cuba_slab_buffer_bytes(int64_t count, const int ncell[3]);
+/* Copies the owned boundary layer on `side` into `buffer` (DEVICE, 16-byte aligned, at least
+ * cuba_slab_buffer_bytes(cuba_slab_count)); stream-ordered.  CUBA_ERR_SIZE if the buffer is too small. */
+int cuba_slab_pack(cuba_ctx *ctx, int side, void *buffer, size_t buffer_bytes);
+/* Rebuilds the store as [lo_buffer's particles][owned cells][hi_buffer's particles] and its cell table; the
+ * buffers are what the lower / upper neighbour packed for its side 1 / side 0 (DEVICE; null exactly where there
+ * is no neighbour), the counts those of cuba_slab_count there.  Stream-ordered after one synchronisation.
+ * CUBA_ERR_SIZE if the capacity is exceeded, CUBA_ERR_VALUE for a buffer where no neighbour is (or none where
+ * one is). */
+int cuba_slab_unpack(cuba_ctx *ctx, const void *lo_buffer, int64_t lo_count, const void *hi_buffer, int64_t hi_count);
+
 /* fp64 leg of the roofline (fp64-pipe utilisation against a measured peak; no passage of
  * the paper: a timing probe).  Launches a kernel of dependent DFMA chains (8 per thread, 8 x SM count
  * CTAs of 256 threads) `repeats` times (1..64) after one warm-up on `cuda_stream` (a cudaStream_t, may

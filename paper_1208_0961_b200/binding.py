@@ -15,7 +15,8 @@ EXPORTS = ("cuba_workspace_bytes", "cuba_init", "cuba_step", "cuba_observables",
            "cuba_get_particles", "cuba_get_cells", "cuba_step_traced", "cuba_counters", "cuba_run_host", "cuba_destroy",
            "cuba_strerror", "cuba_last_cuda_error", "cuba_launch_count", "cuba_profile_enable",
            "cuba_profile_read", "cuba_profile_name", "cuba_set_option", "cuba_observables_lrf",
-           "cuba_step_adaptive", "cuba_step_local_sigma", "cuba_probe_fp64", "cuba_slot_stats")
+           "cuba_step_adaptive", "cuba_step_local_sigma", "cuba_probe_fp64", "cuba_slot_stats",
+           "cuba_slab_init", "cuba_slab_owned", "cuba_slab_count", "cuba_slab_buffer_bytes", "cuba_slab_pack", "cuba_slab_unpack")
 
 
 # cuba_set_option
@@ -116,6 +117,14 @@ def lib():
         L.cuba_profile_read.argtypes = [c_void_p, dp, POINTER(c_uint64)]
         L.cuba_probe_fp64.argtypes = [c_void_p, c_int, dp]
         L.cuba_slot_stats.argtypes = [c_void_p, POINTER(c_uint64)]
+        L.cuba_slab_init.argtypes = [POINTER(c_void_p), dp, POINTER(c_int), c_int64, c_int64] + [c_void_p] * 7 + \
+                                    [c_double, c_uint64, c_void_p, c_size_t, c_void_p, c_int, c_int]
+        L.cuba_slab_owned.argtypes = [c_void_p, POINTER(c_int64)]
+        L.cuba_slab_count.argtypes = [c_void_p, c_int, POINTER(c_int64)]
+        L.cuba_slab_buffer_bytes.argtypes = [c_int64, POINTER(c_int)]
+        L.cuba_slab_buffer_bytes.restype = c_size_t
+        L.cuba_slab_pack.argtypes = [c_void_p, c_int, c_void_p, c_size_t]
+        L.cuba_slab_unpack.argtypes = [c_void_p, c_void_p, c_int64, c_void_p, c_int64]
         L.cuba_profile_name.argtypes = [c_int]
         L.cuba_profile_name.restype = c_char_p
         _lib = L

@@ -261,6 +261,7 @@ constexpr int kNumClasses = 8;   // 7 shared-memory classes + the global-memory 
 
 struct ClassTable {
     uint32_t max_n[kNumClasses];   // inclusive upper bound of each class (last = UINT32_MAX)
+    uint32_t c_lo, c_hi;           // cells [c_lo, c_hi) are collided (x-slab decomposition: the owned layers; else all)
 };
 
 __global__ void __launch_bounds__(256)
@@ -291,7 +292,7 @@ k_cell_start(uint32_t ncells, const uint32_t *__restrict__ count_new,
     // size class (warp-aggregated append; the list order does not affect any result).  Cells with
     // a single particle have no pair but take part in the fused histogram of the next step.
     int k = -1;
-    if (v >= 1) {
+    if (v >= 1 && c >= ct.c_lo && c < ct.c_hi) {
         k = 0;
         while (v > ct.max_n[k]) ++k;
     }

@@ -117,7 +117,15 @@ Layout make_layout(int64_t n, int64_t ncells)
 
 struct cuba_ctx {
     Geom g;
-    int64_t n;
+    int64_t n;           // particles in the store (x-slab decomposition: changes with every halo exchange)
+    int64_t cap;         // particles the arrays and the workspace were sized for
+    // x-slab decomposition (cuba_slab_*): this context owns the cell layers [layer_lo, layer_hi) = the cells
+    // [own_lo, own_hi); its store also holds a copy of the neighbours' boundary layers (ghosts)
+    bool slab = false;
+    int layer_lo = 0, layer_hi = 0;
+    uint32_t own_lo = 0, own_hi = 0;
+    bool own_valid = false;                 // own_cs below is current
+    uint32_t own_cs[4] = {0, 0, 0, 0};      // cell_start at own_lo, end of the first owned layer, start of the last one, own_hi
     double n_test;
     double box[3];
     uint64_t seed;
@@ -255,19 +263,24 @@ static int occupancy_grid(K kernel, int threads, size_t smem, int sms, int *grid
     return CUBA_OK;
 }
 
-int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n,
-              double *x, double *y, double *z, double *px, double *py, double *pz,
-              double n_test, uint64_t seed, void *workspace, size_t workspace_bytes,
-              void *cuda_stream)
+// cuba_init and cuba_slab_init.  cap: particles the arrays and the workspace hold; n <= cap of them are
+// given.  pid_global (DEVICE, n; null: pid = index) names the particles of a slab by their index in the
+// whole problem; [layer_lo, layer_hi) are the owned cell layers along x.
+static int init_impl(cuba_ctx **out, const double box[3], const int ncell[3], int64_t cap, int64_t n,
+                     double *x, double *y, double *z, double *px, double *py, double *pz,
+                     double n_test, uint64_t seed, void *workspace, size_t workspace_bytes,
+                     void *cuda_stream, const uint32_t *pid_global, int layer_lo, int layer_hi, bool slab)
 {
     if (!out || !box || !ncell || !x || !y || !z || !px || !py || !pz || !workspace) return CUBA_ERR_NULL;
     *out = nullptr;
     int64_t ncells;
-    int rc = check_grid(n, ncell, &ncells);
+    int rc = check_grid(cap, ncell, &ncells);
     if (rc != CUBA_OK) return rc;
+    if (n < 1 || n > cap) return CUBA_ERR_SIZE;
+    if (layer_lo < 0 || layer_hi > ncell[0] || layer_lo >= layer_hi) return CUBA_ERR_VALUE;
     for (int k = 0; k < 3; ++k) if (!(box[k] > 0.0) || !std::isfinite(box[k])) return CUBA_ERR_VALUE;
     if (!(n_test > 0.0) || !std::isfinite(n_test)) return CUBA_ERR_VALUE;
-    Layout lay = make_layout(n, ncells);
+    Layout lay = make_layout(cap, ncells);
     if (workspace_bytes < lay.total || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return CUBA_ERR_WORKSPACE;
     for (const double *a : {x, y, z, px, py, pz})
         if (reinterpret_cast<uintptr_t>(a) & 15u) return CUBA_ERR_WORKSPACE;   // bulk copies need 16-byte alignment
@@ -278,7 +291,13 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
 
     cuba_ctx *ctx = new (std::nothrow) cuba_ctx();
     if (!ctx) return CUBA_ERR_CUDA;
-    ctx->n = n; ctx->n_test = n_test; ctx->seed = seed; ctx->t = 0; ctx->steps = 0;
+    ctx->n = n; ctx->cap = cap; ctx->n_test = n_test; ctx->seed = seed; ctx->t = 0; ctx->steps = 0;
+    ctx->slab = slab; ctx->layer_lo = layer_lo; ctx->layer_hi = layer_hi;
+    ctx->own_lo = (uint32_t)layer_lo * (uint32_t)(ncell[1] * ncell[2]);
+    ctx->own_hi = (uint32_t)layer_hi * (uint32_t)(ncell[1] * ncell[2]);
+    if (slab) {          // every step is followed by a halo exchange that rebuilds the store: plain compact steps
+        ctx->fuse_hist = false; ctx->use_graph = false; ctx->slot_mode = 0;
+    }
     ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     ctx->lay = lay;
     ctx->ws = static_cast<unsigned char *>(workspace);
@@ -354,7 +373,7 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
         while (bits < 32 && (((uint64_t)ncells - 1) >> bits) != 0) ++bits;
         const int passes = bits == 0 ? 1 : (bits + 7) / 8;
         uint32_t *H = ctx->at<uint32_t>(lay.rsH);
-        const uint32_t nb = (uint32_t)lay.rs_blocks;
+        const uint32_t nb = (uint32_t)((n + kRsTile - 1) / kRsTile);
         int src = 0;
         for (int p = 0; p < passes; ++p) {
             k_rs_hist<<<nb, kRsThreads, 0, st>>>(keys[src], n, 8 * p, nb, H);
@@ -376,6 +395,10 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
         }
         k_gather_perm<<<gb, 256, 0, st>>>(n, vals[src], ctx->set[0], ctx->set[1]);
         LAUNCHED();
+        if (pid_global) {
+            k_map_pid<<<gb, 256, 0, st>>>(n, ctx->set[1].pid, pid_global);
+            LAUNCHED();
+        }
         k_starts_from_sorted<<<gb, 256, 0, st>>>(n, (uint32_t)ncells, keys[src], ctx->at<uint32_t>(lay.cell_start));
         LAUNCHED();
         // hand the sorted store back to the caller's arrays: the current set is 0 after init
@@ -397,6 +420,26 @@ int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n
     if (rc != CUBA_OK) return fail(rc);
     *out = ctx;
     return CUBA_OK;
+}
+
+int cuba_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t n,
+              double *x, double *y, double *z, double *px, double *py, double *pz,
+              double n_test, uint64_t seed, void *workspace, size_t workspace_bytes,
+              void *cuda_stream)
+{
+    if (!ncell) return CUBA_ERR_NULL;
+    return init_impl(out, box, ncell, n, n, x, y, z, px, py, pz, n_test, seed, workspace, workspace_bytes, cuda_stream,
+                     nullptr, 0, ncell[0] > 0 ? ncell[0] : 1, false);
+}
+
+int cuba_slab_init(cuba_ctx **out, const double box[3], const int ncell[3], int64_t capacity, int64_t n,
+                   double *x, double *y, double *z, double *px, double *py, double *pz, const uint32_t *pid,
+                   double n_test, uint64_t seed, void *workspace, size_t workspace_bytes, void *cuda_stream,
+                   int layer_lo, int layer_hi)
+{
+    if (!pid) return CUBA_ERR_NULL;
+    return init_impl(out, box, ncell, capacity, n, x, y, z, px, py, pz, n_test, seed, workspace, workspace_bytes, cuda_stream,
+                     pid, layer_lo, layer_hi, true);
 }
 
 void cuba_destroy(cuba_ctx *ctx)
@@ -510,6 +553,7 @@ static int enqueue_bin(cuba_ctx *ctx, double dt, uint32_t *cell_of_pid)
     const Layout &lay = ctx->lay;
     cudaStream_t st = ctx->stream;
     const int64_t n = ctx->n;
+    const int64_t ntiles = (n + kTile - 1) / kTile;      // (the layout is sized for the capacity)
     const uint32_t ncells = ctx->g.ncells;
     Soa &in = ctx->set[ctx->cur], &outp = ctx->set[1 - ctx->cur];
     uint32_t *cnt = ctx->at<uint32_t>(lay.cnt);
@@ -520,7 +564,7 @@ static int enqueue_bin(cuba_ctx *ctx, double dt, uint32_t *cell_of_pid)
     if (!have_hist) {
         CU(cudaMemsetAsync(cnt, 0, (size_t)kDirs * ncells * 4, st));
         prof_mark(ctx, G_MEMSET);
-        k_stream_hist<<<ctx->grid_hist, kTileThreads, 2 * sizeof(TileStage<6>), st>>>(ctx->g, dt, n, lay.ntiles, in, cnt, ctx->at<uint32_t>(lay.tile_rec),
+        k_stream_hist<<<ctx->grid_hist, kTileThreads, 2 * sizeof(TileStage<6>), st>>>(ctx->g, dt, n, ntiles, in, cnt, ctx->at<uint32_t>(lay.tile_rec),
                                                                       ctx->at<uint32_t>(lay.flags));
         LAUNCHED();
         prof_mark(ctx, G_STREAM_HIST);
@@ -537,6 +581,7 @@ static int enqueue_bin(cuba_ctx *ctx, double dt, uint32_t *cell_of_pid)
     CUBA_FOR_EACH_CLASS(CUBA_CAP)
 #undef CUBA_CAP
     ct.max_n[kSmemClasses] = 0xFFFFFFFFu;
+    ct.c_lo = ctx->own_lo; ct.c_hi = ctx->own_hi;
     k_cell_start<<<(unsigned)lay.nblocks_cells, 256, 0, st>>>(ncells, ctx->at<uint32_t>(lay.count_new),
                                                               ctx->at<uint32_t>(lay.block_sum), ctx->at<uint32_t>(lay.cell_start),
                                                               ct, zero, ctx->at<uint4>(lay.class_list),
@@ -544,7 +589,7 @@ static int enqueue_bin(cuba_ctx *ctx, double dt, uint32_t *cell_of_pid)
     LAUNCHED();
     prof_mark(ctx, G_CELL_START);
     if (!have_hist) {
-        k_carry<<<(unsigned)((lay.ntiles + 7) / 8), 256, 0, st>>>((int)lay.ntiles, ctx->at<uint32_t>(lay.tile_rec),
+        k_carry<<<(unsigned)((ntiles + 7) / 8), 256, 0, st>>>((int)ntiles, ctx->at<uint32_t>(lay.tile_rec),
                                                                   ctx->at<uint32_t>(lay.carry));
         LAUNCHED();
         prof_mark(ctx, G_CARRY);
@@ -553,10 +598,10 @@ static int enqueue_bin(cuba_ctx *ctx, double dt, uint32_t *cell_of_pid)
     LAUNCHED();
     prof_mark(ctx, G_DEST_BASE);
     if (cell_of_pid)
-        k_scatter<true><<<ctx->grid_scat, kTileThreads, 2 * sizeof(TileStage<7>), st>>>(ctx->g, dt, n, lay.ntiles, in, outp, cnt,
+        k_scatter<true><<<ctx->grid_scat, kTileThreads, 2 * sizeof(TileStage<7>), st>>>(ctx->g, dt, n, ntiles, in, outp, cnt,
                                                                        ctx->at<uint32_t>(lay.carry), cell_of_pid);
     else
-        k_scatter<false><<<ctx->grid_scat, kTileThreads, 2 * sizeof(TileStage<7>), st>>>(ctx->g, dt, n, lay.ntiles, in, outp, cnt,
+        k_scatter<false><<<ctx->grid_scat, kTileThreads, 2 * sizeof(TileStage<7>), st>>>(ctx->g, dt, n, ntiles, in, outp, cnt,
                                                                         ctx->at<uint32_t>(lay.carry), nullptr);
     LAUNCHED();
     prof_mark(ctx, G_SCATTER);
@@ -759,6 +804,7 @@ static int slot_run(cuba_ctx *ctx, int nsteps, double dt, double sigma, double b
     CUBA_FOR_EACH_CLASS(CUBA_CAP)
 #undef CUBA_CAP
     ct.max_n[kSmemClasses] = 0xFFFFFFFFu;
+    ct.c_lo = 0; ct.c_hi = ncells;
 
     CollideParams P{};
     P.seed = ctx->seed; P.base = base; P.g = ctx->g;
@@ -872,11 +918,13 @@ static int step_fixed(cuba_ctx *ctx, int nsteps, double dt, double sigma, double
 {
     if (!ctx) return CUBA_ERR_NULL;
     if (nsteps < 0) return CUBA_ERR_SIZE;
+    if (ctx->slab && nsteps > 1) return CUBA_ERR_VALUE;     // a halo exchange belongs between two steps of a slab
     double base;
     int rc = check_step_args(ctx, dt, sigma, &base);
     if (rc != CUBA_OK) return rc;
     rc = settle(ctx);
     if (rc != CUBA_OK) return rc;
+    ctx->own_valid = false;
     int s = 0;
     auto plain = [&]() -> int {
         const int r = step_once(ctx, dt, base, etas);
@@ -966,6 +1014,7 @@ int cuba_step_adaptive(cuba_ctx *ctx, int nsteps, double dt_max, double sigma, d
 {
     if (!ctx) return CUBA_ERR_NULL;
     if (nsteps < 0) return CUBA_ERR_SIZE;
+    if (ctx->slab) return CUBA_ERR_VALUE;      // the rule needs the fullest cell of ALL slabs: not built
     if (!(dt_max > 0.0) || !std::isfinite(dt_max) || !(sigma >= 0.0) || !std::isfinite(sigma)) return CUBA_ERR_VALUE;
     double sum = 0.0;
     int rc = settle(ctx);
@@ -1004,6 +1053,7 @@ int cuba_step_adaptive(cuba_ctx *ctx, int nsteps, double dt_max, double sigma, d
 int cuba_step_traced(cuba_ctx *ctx, double dt, double sigma, cuba_trace *out)
 {
     if (!ctx || !out || !out->cell_of_pid) return CUBA_ERR_NULL;
+    if (ctx->slab) return CUBA_ERR_VALUE;      // pids are global in a slab: the per-pid trace arrays do not apply
     if (out->pair_capacity > 0 && (!out->pair_cell || !out->pair_round || !out->pid_a || !out->pid_b || !out->P ||
                                    !out->u || !out->decided)) return CUBA_ERR_NULL;
     double base;
@@ -1110,6 +1160,174 @@ int cuba_set_option(cuba_ctx *ctx, int option, int value)
     return CUBA_OK;
 }
 
+// ---- x-slab decomposition ---------------------------------------------------------
+// Collisions are cell-local and dt < cell edge, so the path shards by layers of
+// cells along x.  A rank owns the layers [layer_lo, layer_hi) and keeps, in the SAME global grid and
+// coordinates (no offset: every operation rounds as on one GPU), a copy of the two adjacent boundary layers
+// of its neighbours (ghosts).  One step = cuba_step(1) on the local store (S1-S4 on owned + ghost particles,
+// S5 on the owned cells only: ClassTable range) -- the particles that enter an owned cell from a ghost cell
+// are placed by the same stable sort as on one GPU, because the ghost cells hold exactly what the neighbour
+// holds, in the same order -- then the halo exchange: every rank packs its two owned boundary layers after
+// the collisions (contiguous ranges of the cell-sorted store: cuba_slab_pack), the neighbours rebuild their
+// store as [ghost from below][owned cells][ghost from above] (cuba_slab_unpack).  What a rank streamed out of
+// its owned layers is dropped there and reappears at the neighbour, which streamed its ghost copy of the same
+// particles.  The concatenation of the ranks' owned ranges is the one-GPU store bit for bit.
+static int slab_read_owned(cuba_ctx *ctx)
+{
+    if (ctx->own_valid) return CUBA_OK;
+    const uint32_t *cs = ctx->at<uint32_t>(ctx->lay.cell_start);
+    const uint32_t nyz = (uint32_t)(ctx->g.nc[1] * ctx->g.nc[2]);
+    const uint32_t at[4] = {ctx->own_lo, ctx->own_lo + nyz, ctx->own_hi - nyz, ctx->own_hi};
+    for (int k = 0; k < 4; ++k)
+        CU(cudaMemcpyAsync(ctx->h_u32 + k, cs + at[k], 4, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    for (int k = 0; k < 4; ++k) ctx->own_cs[k] = ctx->h_u32[k];
+    ctx->own_valid = true;
+    return CUBA_OK;
+}
+
+__global__ void __launch_bounds__(256)
+k_slab_pack_counts(const uint32_t *__restrict__ cell_start, uint32_t c0, uint32_t nyz, unsigned long long count,
+                   unsigned long long *__restrict__ header, uint32_t *__restrict__ counts)
+{
+    const uint32_t i = blockIdx.x * 256u + threadIdx.x;
+    if (i == 0) { header[0] = count; header[1] = nyz; }
+    if (i < nyz) counts[i] = cell_start[c0 + i + 1] - cell_start[c0 + i];
+}
+
+// population of every cell of the rebuilt store + per-block sums for the scan
+__global__ void __launch_bounds__(256)
+k_slab_counts(uint32_t ncells, const uint32_t *__restrict__ cell_start_old, uint32_t own_lo, uint32_t own_hi, uint32_t nyz,
+              const uint32_t *__restrict__ lo_counts, const uint32_t *__restrict__ hi_counts,
+              uint32_t *__restrict__ count_new, uint32_t *__restrict__ block_sum)
+{
+    __shared__ uint32_t s_warp[8];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const uint32_t c = blockIdx.x * 256u + threadIdx.x;
+    uint32_t v = 0;
+    if (c < ncells) {
+        if (c >= own_lo && c < own_hi) v = cell_start_old[c + 1] - cell_start_old[c];
+        else if (lo_counts && c + nyz >= own_lo && c < own_lo) v = lo_counts[c + nyz - own_lo];
+        else if (hi_counts && c >= own_hi && c < own_hi + nyz) v = hi_counts[c - own_hi];
+        count_new[c] = v;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+    if (lane == 0) s_warp[wid] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t t = 0;
+        for (int w = 0; w < 8; ++w) t += s_warp[w];
+        block_sum[blockIdx.x] = t;
+    }
+}
+
+size_t cuba_slab_buffer_bytes(int64_t count, const int ncell[3])
+{
+    if (!ncell || count < 0) return 0;
+    return 16 + (size_t)count * 52 + (size_t)ncell[1] * ncell[2] * 4;
+}
+
+int cuba_slab_owned(cuba_ctx *ctx, int64_t out[4])
+{
+    if (!ctx || !out) return CUBA_ERR_NULL;
+    if (!ctx->slab) return CUBA_ERR_VALUE;
+    const int rc = slab_read_owned(ctx);
+    if (rc != CUBA_OK) return rc;
+    out[0] = ctx->own_cs[0]; out[1] = (int64_t)ctx->own_cs[3] - ctx->own_cs[0]; out[2] = ctx->n; out[3] = ctx->cap;
+    return CUBA_OK;
+}
+
+int cuba_slab_count(cuba_ctx *ctx, int side, int64_t *count)
+{
+    if (!ctx || !count) return CUBA_ERR_NULL;
+    if (!ctx->slab || (side != 0 && side != 1)) return CUBA_ERR_VALUE;
+    const int rc = slab_read_owned(ctx);
+    if (rc != CUBA_OK) return rc;
+    *count = side == 0 ? (int64_t)ctx->own_cs[1] - ctx->own_cs[0] : (int64_t)ctx->own_cs[3] - ctx->own_cs[2];
+    return CUBA_OK;
+}
+
+int cuba_slab_pack(cuba_ctx *ctx, int side, void *buffer, size_t buffer_bytes)
+{
+    if (!ctx || !buffer) return CUBA_ERR_NULL;
+    if (!ctx->slab || (side != 0 && side != 1)) return CUBA_ERR_VALUE;
+    if (reinterpret_cast<uintptr_t>(buffer) & 15u) return CUBA_ERR_WORKSPACE;
+    int rc = slab_read_owned(ctx);
+    if (rc != CUBA_OK) return rc;
+    const uint32_t nyz = (uint32_t)(ctx->g.nc[1] * ctx->g.nc[2]);
+    const uint32_t first = side == 0 ? ctx->own_cs[0] : ctx->own_cs[2];
+    const uint32_t count = (side == 0 ? ctx->own_cs[1] : ctx->own_cs[3]) - first;
+    const uint32_t c0 = side == 0 ? ctx->own_lo : ctx->own_hi - nyz;
+    if (buffer_bytes < cuba_slab_buffer_bytes(count, ctx->g.nc)) return CUBA_ERR_SIZE;
+    unsigned char *b = static_cast<unsigned char *>(buffer);
+    cudaStream_t st = ctx->stream;
+    const Soa &c = ctx->set[ctx->cur];
+    const double *arr[6] = {c.x, c.y, c.z, c.px, c.py, c.pz};
+    for (int k = 0; k < 6; ++k)
+        if (count) CU(cudaMemcpyAsync(b + 16 + (size_t)k * count * 8, arr[k] + first, (size_t)count * 8, cudaMemcpyDeviceToDevice, st));
+    if (count) CU(cudaMemcpyAsync(b + 16 + (size_t)count * 48, c.pid + first, (size_t)count * 4, cudaMemcpyDeviceToDevice, st));
+    k_slab_pack_counts<<<(nyz + 255u) / 256u, 256, 0, st>>>(ctx->at<uint32_t>(ctx->lay.cell_start), c0, nyz, count,
+                                                            reinterpret_cast<unsigned long long *>(b),
+                                                            reinterpret_cast<uint32_t *>(b + 16 + (size_t)count * 52));
+    LAUNCHED();
+    return CUBA_OK;
+}
+
+int cuba_slab_unpack(cuba_ctx *ctx, const void *lo_buffer, int64_t lo_count, const void *hi_buffer, int64_t hi_count)
+{
+    if (!ctx) return CUBA_ERR_NULL;
+    if (!ctx->slab || lo_count < 0 || hi_count < 0) return CUBA_ERR_VALUE;
+    if ((lo_buffer == nullptr) != (ctx->layer_lo == 0) || (hi_buffer == nullptr) != (ctx->layer_hi == ctx->g.nc[0])) return CUBA_ERR_VALUE;
+    if (!lo_buffer) lo_count = 0;
+    if (!hi_buffer) hi_count = 0;
+    int rc = slab_read_owned(ctx);
+    if (rc != CUBA_OK) return rc;
+    const Layout &lay = ctx->lay;
+    const uint32_t own_first = ctx->own_cs[0];
+    const int64_t own_count = (int64_t)ctx->own_cs[3] - own_first;
+    const int64_t n_new = lo_count + own_count + hi_count;
+    if (n_new < 1 || n_new > ctx->cap) return CUBA_ERR_SIZE;
+    cudaStream_t st = ctx->stream;
+    const Soa &from = ctx->set[ctx->cur], &to = ctx->set[1 - ctx->cur];
+    const double *src[6] = {from.x, from.y, from.z, from.px, from.py, from.pz};
+    double *dst[6] = {to.x, to.y, to.z, to.px, to.py, to.pz};
+    const unsigned char *lb = static_cast<const unsigned char *>(lo_buffer), *hb = static_cast<const unsigned char *>(hi_buffer);
+    for (int k = 0; k < 6; ++k) {
+        if (lo_count) CU(cudaMemcpyAsync(dst[k], lb + 16 + (size_t)k * lo_count * 8, (size_t)lo_count * 8, cudaMemcpyDeviceToDevice, st));
+        if (own_count) CU(cudaMemcpyAsync(dst[k] + lo_count, src[k] + own_first, (size_t)own_count * 8, cudaMemcpyDeviceToDevice, st));
+        if (hi_count) CU(cudaMemcpyAsync(dst[k] + lo_count + own_count, hb + 16 + (size_t)k * hi_count * 8, (size_t)hi_count * 8, cudaMemcpyDeviceToDevice, st));
+    }
+    if (lo_count) CU(cudaMemcpyAsync(to.pid, lb + 16 + (size_t)lo_count * 48, (size_t)lo_count * 4, cudaMemcpyDeviceToDevice, st));
+    if (own_count) CU(cudaMemcpyAsync(to.pid + lo_count, from.pid + own_first, (size_t)own_count * 4, cudaMemcpyDeviceToDevice, st));
+    if (hi_count) CU(cudaMemcpyAsync(to.pid + lo_count + own_count, hb + 16 + (size_t)hi_count * 48, (size_t)hi_count * 4, cudaMemcpyDeviceToDevice, st));
+    // cell table of the rebuilt store
+    const uint32_t ncells = ctx->g.ncells, nyz = (uint32_t)(ctx->g.nc[1] * ctx->g.nc[2]);
+    uint32_t *zero = ctx->at<uint32_t>(lay.zero);
+    // the old table is read while the new one is written by a later kernel: counts first, into count_new
+    k_slab_counts<<<(unsigned)lay.nblocks_cells, 256, 0, st>>>(ncells, ctx->at<uint32_t>(lay.cell_start), ctx->own_lo, ctx->own_hi, nyz,
+                                                               lb ? reinterpret_cast<const uint32_t *>(lb + 16 + (size_t)lo_count * 52) : nullptr,
+                                                               hb ? reinterpret_cast<const uint32_t *>(hb + 16 + (size_t)hi_count * 52) : nullptr,
+                                                               ctx->at<uint32_t>(lay.count_new), ctx->at<uint32_t>(lay.block_sum));
+    LAUNCHED();
+    k_scan_blocks<<<1, 1024, 0, st>>>(ctx->at<uint32_t>(lay.block_sum), (int)lay.nblocks_cells, zero, kZeroWords);
+    LAUNCHED();
+    ClassTable ct{};
+#define CUBA_CAP(K, T, I, C, MB) ct.max_n[K] = C;
+    CUBA_FOR_EACH_CLASS(CUBA_CAP)
+#undef CUBA_CAP
+    ct.max_n[kSmemClasses] = 0xFFFFFFFFu;
+    ct.c_lo = ctx->own_lo; ct.c_hi = ctx->own_hi;
+    k_cell_start<<<(unsigned)lay.nblocks_cells, 256, 0, st>>>(ncells, ctx->at<uint32_t>(lay.count_new), ctx->at<uint32_t>(lay.block_sum),
+                                                              ctx->at<uint32_t>(lay.cell_start), ct, zero, ctx->at<uint4>(lay.class_list),
+                                                              ctx->at<unsigned long long>(lay.max_occ), zero + kStepMaxWord);
+    LAUNCHED();
+    ctx->cur = 1 - ctx->cur;
+    ctx->n = n_new;
+    ctx->pre_dt = 0.0; ctx->nmax_valid = false; ctx->own_valid = false;
+    return CUBA_OK;
+}
+
 int cuba_slot_stats(cuba_ctx *ctx, uint64_t out[2])
 {
     if (!ctx || !out) return CUBA_ERR_NULL;
@@ -1124,7 +1342,15 @@ int cuba_observables(cuba_ctx *ctx, double total[4], int nslab, double *edens)
     if (nslab < 1 || nslab > kObsMaxSlabs) return CUBA_ERR_SIZE;
     { const int rs = settle(ctx); if (rs != CUBA_OK) return rs; }
     const Layout &lay = ctx->lay;
-    const Soa &cur = ctx->set[ctx->cur];
+    Soa cur = ctx->set[ctx->cur];
+    int64_t n_obs = ctx->n;
+    if (ctx->slab) {           // a slab reports its owned particles only (the caller adds the slabs up)
+        const int ro = slab_read_owned(ctx);
+        if (ro != CUBA_OK) return ro;
+        const size_t f = ctx->own_cs[0];
+        cur.x += f; cur.px += f; cur.py += f; cur.pz += f;
+        n_obs = (int64_t)ctx->own_cs[3] - ctx->own_cs[0];
+    }
     cudaStream_t st = ctx->stream;
     const double inv_w = (double)nslab / ctx->box[0];
     const double vol = ((ctx->n_test * (ctx->box[0] / (double)nslab)) * ctx->box[1]) * ctx->box[2];
@@ -1134,9 +1360,9 @@ int cuba_observables(cuba_ctx *ctx, double total[4], int nslab, double *edens)
     if (nslab > 2 * ctx->g.nc[0]) {
         const int window = per_layer < kObsWindowMax ? per_layer : kObsWindowMax;
         k_observe_partial<false, true><<<kObsGrid, kObsThreads, (size_t)kObsWarps * (nslab + window * 32) * 8, st>>>(
-            ctx->n, cur.x, cur.px, cur.py, cur.pz, inv_w, nslab, window, partial);
+            n_obs, cur.x, cur.px, cur.py, cur.pz, inv_w, nslab, window, partial);
     } else {
-        k_observe_partial<false, false><<<kObsGrid, kObsThreads, (size_t)kObsWarps * nslab * 8, st>>>(ctx->n, cur.x, cur.px, cur.py, cur.pz,
+        k_observe_partial<false, false><<<kObsGrid, kObsThreads, (size_t)kObsWarps * nslab * 8, st>>>(n_obs, cur.x, cur.px, cur.py, cur.pz,
                                                                                                  inv_w, nslab, 2, partial);
     }
     LAUNCHED();
@@ -1156,7 +1382,15 @@ int cuba_observables_lrf(cuba_ctx *ctx, int nslab, double *T, double *lrf)
     if (nslab < 1 || nslab > kLrfMaxSlabs) return CUBA_ERR_SIZE;
     { const int rs = settle(ctx); if (rs != CUBA_OK) return rs; }
     const Layout &lay = ctx->lay;
-    const Soa &cur = ctx->set[ctx->cur];
+    Soa cur = ctx->set[ctx->cur];
+    int64_t n_obs = ctx->n;
+    if (ctx->slab) {           // a slab reports its owned particles only (the caller adds the slabs up)
+        const int ro = slab_read_owned(ctx);
+        if (ro != CUBA_OK) return ro;
+        const size_t f = ctx->own_cs[0];
+        cur.x += f; cur.px += f; cur.py += f; cur.pz += f;
+        n_obs = (int64_t)ctx->own_cs[3] - ctx->own_cs[0];
+    }
     cudaStream_t st = ctx->stream;
     const double inv_w = (double)nslab / ctx->box[0];
     const double vol = ((ctx->n_test * (ctx->box[0] / (double)nslab)) * ctx->box[1]) * ctx->box[2];
@@ -1167,9 +1401,9 @@ int cuba_observables_lrf(cuba_ctx *ctx, int nslab, double *T, double *lrf)
     if (nslab > 2 * ctx->g.nc[0]) {
         const int window = per_layer < kLrfWindowMax ? per_layer : kLrfWindowMax;
         k_observe_partial<true, true><<<grid, kObsThreads, (size_t)kObsWarps * kLrfComp * (nslab + window * 32) * 8, st>>>(
-            ctx->n, cur.x, cur.px, cur.py, cur.pz, inv_w, nslab, window, partial);
+            n_obs, cur.x, cur.px, cur.py, cur.pz, inv_w, nslab, window, partial);
     } else {
-        k_observe_partial<true, false><<<grid, kObsThreads, (size_t)kObsWarps * kLrfComp * nslab * 8, st>>>(ctx->n, cur.x, cur.px, cur.py, cur.pz,
+        k_observe_partial<true, false><<<grid, kObsThreads, (size_t)kObsWarps * kLrfComp * nslab * 8, st>>>(n_obs, cur.x, cur.px, cur.py, cur.pz,
                                                                                                          inv_w, nslab, 2, partial);
     }
     LAUNCHED();

@@ -169,6 +169,14 @@ k_gather_perm(int64_t n, const uint32_t *__restrict__ perm, Soa in, Soa out)
     out.pid[k] = s;
 }
 
+// x-slab decomposition: the particles of a slab carry their index in the whole problem
+__global__ void __launch_bounds__(256)
+k_map_pid(int64_t n, uint32_t *__restrict__ pid, const uint32_t *__restrict__ pid_global)
+{
+    const int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.x;
+    if (k < n) pid[k] = pid_global[pid[k]];
+}
+
 // cell_start from the sorted keys: slot k opens every cell in (key[k-1], key[k]]
 __global__ void __launch_bounds__(256)
 k_starts_from_sorted(int64_t n, uint32_t ncells, const uint32_t *__restrict__ keys, uint32_t *__restrict__ cell_start)

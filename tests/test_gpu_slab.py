@@ -1,0 +1,88 @@
+"""x-slab decomposition on the GPU: several ranks' contexts stepped in one process on
+one device (LocalSlabGroup: the calls of a multi-GPU job in the same order, buffers handed over directly).  The
+owned parts concatenated in rank order must be the one-GPU store and the oracle's BIT FOR BIT -- array order,
+pids, positions, momenta -- after every step; counters add up; observables add up to 1e-12."""
+import numpy as np
+import pytest
+
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def cuba():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1208_0961_b200 import build
+    build.build()
+    import paper_1208_0961_b200 as c
+    return c
+
+
+@pytest.fixture(scope="module")
+def oracle_mod():
+    import oracle
+    oracle.build()
+    return oracle
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_slab_ranks_reproduce_the_one_gpu_run_bit_for_bit(cuba, oracle_mod, world):
+    w = workloads.riemann_small(seed=51)
+    one = cuba.Cuba.from_workload(w)
+    o = oracle_mod.Oracle.from_workload(w)
+    grp = cuba.LocalSlabGroup(w, world)
+    assert [hi - lo for lo, hi in grp.layers] == ([4, 4] if world == 2 else [3, 3, 2])
+    for a, b in zip(grp.particles(), one.particles()):          # the initial binning (A19)
+        assert np.array_equal(a, b)
+    for k in (1, 2, 4):
+        grp.step(k, w.dt, w.sigma)
+        one.step(k, w.dt, w.sigma)
+        o.step(k, w.dt, w.sigma)
+        for a, b, c in zip(grp.particles(), one.particles(), o.particles()):
+            assert np.array_equal(a, b) and np.array_equal(a, c)
+    cg, c1, co = grp.counters(), one.counters(), o.counters()
+    assert (cg["pairs"], cg["collisions"], cg["rounds"]) == (c1.pairs, c1.collisions, c1.rounds) == \
+           (co["pairs"], co["collisions"], co["rounds"])
+    gt, ge = grp.observables(w.nslab)
+    ot, oe = o.observables(w.nslab)
+    assert np.allclose(ge, oe, rtol=1e-12, atol=0) and np.allclose(gt, ot, rtol=1e-12, atol=1e-9)
+    assert all(r.counters().device_flags == 0 for r in grp.ranks)
+    assert sum(r.owned()[1] for r in grp.ranks) == w.n         # every particle is owned exactly once
+    grp.close()
+
+
+def test_slab_with_many_rounds_walls_and_thin_layers(cuba, oracle_mod):
+    """Dense, strongly interacting gas (several rounds per cell), one-layer slabs at both walls, dt at 90 % of the
+    cell edge (every second particle changes cell), 12 steps."""
+    w = workloads.riemann(L=(6.0, 2.0, 2.0), ncell=(6, 2, 2), r_test=40.0, sigma_gev2=60.0, dt=0.9, seed=52)
+    o = oracle_mod.Oracle.from_workload(w)
+    grp = cuba.LocalSlabGroup(w, 6, capacity=w.n)
+    for _ in range(3):
+        grp.step(4, w.dt, w.sigma)
+        o.step(4, w.dt, w.sigma)
+        for a, c in zip(grp.particles(), o.particles()):
+            assert np.array_equal(a, c)
+    cg, co = grp.counters(), o.counters()
+    assert (cg["pairs"], cg["collisions"], cg["rounds"]) == (co["pairs"], co["collisions"], co["rounds"])
+    grp.close()
+
+
+def test_slab_argument_errors(cuba):
+    w = workloads.riemann_small(seed=53)
+    r = cuba.SlabRank(w, 2, 5)
+    with pytest.raises(cuba.CubaError):
+        r.step(2, w.dt, w.sigma)                 # a halo exchange belongs between two steps
+    with pytest.raises(cuba.CubaError):
+        r.unpack(None, None)                     # both neighbours exist
+    r.step(1, w.dt, w.sigma)
+    first, cnt, n, cap = r.owned()
+    assert 0 < first and first + cnt < n <= cap
+    assert r.count(0) > 0 and r.count(1) > 0
+    with pytest.raises(cuba.CubaError):
+        cuba.SlabRank(w, 5, 5)
+    with pytest.raises(cuba.CubaError):
+        cuba.SlabRank(w, 0, 4, capacity=10)
+    r.close()

@@ -154,6 +154,8 @@ CONFIGS: dict = {
     3: lambda: riemann(ncell=(64, 32, 32), r_test=40.0, sigma_gev2=50.0, dt=0.05, steps=200,
                        seed=4, name="configs[3] Riemann fine cells sigma=50"),
     4: lambda: skewed(r_test=100.0, seed=5, steps=50, name="configs[4] skewed occupancy r_test=100"),
+    # the ~100M-particle variant of configs[4] (BASELINE.json says "~100M"; r_test = 100 gives 53.9M)
+    5: lambda: skewed(r_test=185.5, seed=5, steps=50, name="configs[4] skewed occupancy r_test=185.5 (~100M)"),
 }
 
 
