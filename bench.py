@@ -276,6 +276,86 @@ def workloads_name(config):
             5: "configs[4] at ~100M particles: skewed occupancy 64x32x32 fm^3, r_test=185.5 (100.0M particles)"}[config]
 
 
+def run_slab(args, rank, world, local):
+    """--decomp slab: ONE problem (configs[C]) sharded by x-layers of cells over the ranks (strong scaling), halo
+    exchange by torch.distributed point-to-point after every step (paper_1208_0961_b200/slab.py).  With
+    --slab-emulate R on one GPU the R ranks' contexts are stepped one after the other in one process: the
+    per-rank device times project the step of an R-GPU run (max over ranks; transfers not included)."""
+    import torch
+    import torch.distributed as dist
+    import paper_1208_0961_b200 as cuba
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    w = workloads.CONFIGS[args.config]()
+    emul = args.slab_emulate
+    if emul:
+        grp = cuba.LocalSlabGroup(w, emul, device=dev, balance=True)
+        grp.step(args.warmup, w.dt, w.sigma)
+        per_rank = [0.0] * emul
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(6)] for _ in range(emul)]
+        torch.cuda.synchronize()
+        for _ in range(args.steps):
+            for k, r in enumerate(grp.ranks):
+                evs[k][0].record(); r.step(1, w.dt, w.sigma); evs[k][1].record()
+            sent = []
+            for k, r in enumerate(grp.ranks):
+                lo, hi = cuba.neighbours(k, emul)
+                evs[k][2].record()
+                sent.append((r.pack(0) if lo is not None else None, r.pack(1) if hi is not None else None))
+                evs[k][3].record()
+            for k, r in enumerate(grp.ranks):
+                lo, hi = cuba.neighbours(k, emul)
+                evs[k][4].record()
+                r.unpack(sent[lo][1] if lo is not None else None, sent[hi][0] if hi is not None else None)
+                evs[k][5].record()
+            torch.cuda.synchronize()
+            for k in range(emul):
+                per_rank[k] += sum(evs[k][2 * q].elapsed_time(evs[k][2 * q + 1]) for q in range(3))
+        ms = max(per_rank) / args.steps
+        halo = [sum(r.count(s) for s in (0, 1) if cuba.neighbours(k, emul)[s] is not None) for k, r in enumerate(grp.ranks)]
+        print(json.dumps({"metric": METRIC, "unit": UNIT, "value": w.n / (ms * 1e-3), "n_gpus": 1, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "dtype": "f64",
+                          "data": "synthetic", "vs_baseline": None,
+                          "config": {"workload": workloads_name(args.config), "decomposition": "x-slabs of whole cell layers, cuts balanced by particles per layer",
+                                     "emulated_ranks": emul, "layers": grp.layers,
+                                     "note": "PROJECTION: %d ranks stepped one after the other on ONE GPU; ms_per_step = slowest rank's "
+                                             "device time (step + pack + unpack), NVLink transfers not included" % emul},
+                          "per_rank_ms": [round(v / args.steps, 4) for v in per_rank],
+                          "halo_particles_sent_per_rank": halo, "halo_bytes_sent_per_rank": [52 * h for h in halo]}), flush=True)
+        return
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+    lo, hi = cuba.slab_layers(int(w.ncell[0]), world, cuba.layer_weights(w.x, float(w.box[0]), int(w.ncell[0])))[rank]
+    ctx = cuba.SlabRank(w, lo, hi, device=dev)
+    for _ in range(args.warmup):
+        cuba.slab_step(ctx, dist, rank, world, w.dt, w.sigma)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        cuba.slab_step(ctx, dist, rank, world, w.dt, w.sigma)
+    ev1.record()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t = torch.tensor([ev0.elapsed_time(ev1)], device=dev, dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t[0]) / args.steps
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "unit": UNIT, "value": w.n / (ms * 1e-3), "n_gpus": world, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "dtype": "f64",
+                          "data": "synthetic", "vs_baseline": None,
+                          "config": {"workload": workloads_name(args.config), "decomposition": "x-slabs of whole cell layers",
+                                     "parallelism": "slab x%d, halo exchange by NCCL point-to-point" % world}}), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -283,6 +363,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json:configs")
     ap.add_argument("--impl", default="cuba", choices=["cuba", "reference"])
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent replicas (default, weak scaling) or ONE problem in x-slabs (strong scaling)")
+    ap.add_argument("--slab-emulate", type=int, default=0, help="diagnostic: R slab ranks stepped in turn on one GPU (projection)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-fuse", action="store_true", help="run the separate k_stream_hist pass every step (A/B diagnostic)")
@@ -301,6 +384,9 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank, world)
+        return
+    if args.decomp == "slab" or args.slab_emulate:
+        run_slab(args, rank, world, local)
         return
 
     import torch

@@ -19,17 +19,40 @@ import numpy as np
 from .binding import Cuba, CubaError, _c3d, _c3i, _check, lib, workspace_bytes
 
 
-def slab_layers(nx: int, world: int):
-    """[(layer_lo, layer_hi)] per rank: contiguous, whole layers, sizes differing by at most one."""
+def slab_layers(nx: int, world: int, weights=None):
+    """[(layer_lo, layer_hi)] per rank: contiguous, whole layers.  Without weights the sizes differ by at most
+    one layer; with weights (work per layer, e.g. particles: `layer_weights`) the cuts are put where the running
+    sum of the weights crosses k/world of the total, every rank keeping at least one layer."""
     if world < 1 or nx < world:
         raise ValueError("need 1 <= world <= number of cell layers along x")
-    q, r = divmod(nx, world)
-    out, lo = [], 0
-    for k in range(world):
-        hi = lo + q + (1 if k < r else 0)
-        out.append((lo, hi))
-        lo = hi
-    return out
+    if weights is None:
+        q, r = divmod(nx, world)
+        out, lo = [], 0
+        for k in range(world):
+            hi = lo + q + (1 if k < r else 0)
+            out.append((lo, hi))
+            lo = hi
+        return out
+    wts = np.asarray(weights, dtype=np.float64)
+    if wts.shape != (nx,) or np.any(wts < 0) or not np.isfinite(wts).all():
+        raise ValueError("one finite non-negative weight per layer")
+    cum = np.concatenate([[0.0], np.cumsum(wts)])
+    cuts = [0]
+    for k in range(1, world):
+        target = cum[-1] * k / world
+        c = int(np.argmin(np.abs(cum - target)))                 # the layer boundary nearest to the target
+        c = max(c, cuts[-1] + 1)                                 # at least one layer for the rank below ...
+        c = min(c, nx - (world - k))                             # ... and for every rank above
+        cuts.append(c)
+    cuts.append(nx)
+    return [(cuts[k], cuts[k + 1]) for k in range(world)]
+
+
+def layer_weights(x: np.ndarray, box_x: float, nx: int) -> np.ndarray:
+    """Particles per cell layer along x (the S3 layer index of the library)."""
+    inv_d = 1.0 / (box_x / float(nx))
+    layer = np.clip((x * inv_d).astype(np.int64), 0, nx - 1)
+    return np.bincount(layer, minlength=nx).astype(np.float64)
 
 
 def initial_selection(x: np.ndarray, box_x: float, nx: int, layer_lo: int, layer_hi: int) -> np.ndarray:
@@ -102,7 +125,10 @@ class SlabRank:
         import torch
         cnt = self.count(side)
         nbytes = int(lib().cuba_slab_buffer_bytes(cnt, _c3i(self.ncell)))
-        buf = torch.empty(nbytes + 16, dtype=torch.uint8, device=self.device)
+        bufs = self.__dict__.setdefault("_halo", [None, None])      # one buffer per side, grown when needed
+        if bufs[side] is None or bufs[side].numel() < nbytes + 16:
+            bufs[side] = torch.empty(int(1.25 * nbytes) + 4096, dtype=torch.uint8, device=self.device)
+        buf = bufs[side]
         off = (-buf.data_ptr()) % 16
         view = buf[off:off + nbytes]
         _check(lib().cuba_slab_pack(self._h, int(side), c_void_p(view.data_ptr()), nbytes))
@@ -177,9 +203,10 @@ class LocalSlabGroup:
     """All ranks of a decomposition in ONE process on one device, stepped one after the other: the test vehicle
     where fewer GPUs than ranks are at hand (the calls and their order are those of `slab_step`)."""
 
-    def __init__(self, w, world, device="cuda:0", capacity=None):
+    def __init__(self, w, world, device="cuda:0", capacity=None, balance=False):
         self.world = int(world)
-        self.layers = slab_layers(int(w.ncell[0]), self.world)
+        nx = int(w.ncell[0])
+        self.layers = slab_layers(nx, self.world, layer_weights(w.x, float(w.box[0]), nx) if balance else None)
         self.ranks = [SlabRank(w, lo, hi, device=device, capacity=capacity) for lo, hi in self.layers]
 
     def step(self, nsteps, dt, sigma):

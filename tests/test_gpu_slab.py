@@ -70,6 +70,19 @@ def test_slab_with_many_rounds_walls_and_thin_layers(cuba, oracle_mod):
     grp.close()
 
 
+def test_slab_cuts_balanced_by_particles(cuba, oracle_mod):
+    """The cuts follow the particles per layer (the hot half of the Riemann problem gets more ranks); same bits."""
+    w = workloads.riemann_small(seed=54)
+    o = oracle_mod.Oracle.from_workload(w)
+    grp = cuba.LocalSlabGroup(w, 3, balance=True)
+    assert grp.layers[0][1] < 3 and grp.layers[-1][1] == 8          # the first rank takes fewer (hot) layers than 8/3
+    grp.step(5, w.dt, w.sigma)
+    o.step(5, w.dt, w.sigma)
+    for a, c in zip(grp.particles(), o.particles()):
+        assert np.array_equal(a, c)
+    grp.close()
+
+
 def test_slab_argument_errors(cuba):
     w = workloads.riemann_small(seed=53)
     r = cuba.SlabRank(w, 2, 5)

@@ -26,6 +26,15 @@ def test_slab_layers_cover_the_grid_in_whole_layers():
             assert min(sizes) >= 1 and max(sizes) - min(sizes) <= 1
     with pytest.raises(ValueError):
         slab_layers(4, 5)
+    # weighted cuts: a hot half that holds 8x the particles gets most of the ranks; every rank keeps a layer
+    wts = np.array([8.0] * 4 + [1.0] * 4)
+    assert slab_layers(8, 2, wts) == [(0, 2), (2, 8)]
+    parts = slab_layers(8, 4, wts)
+    assert parts[0][0] == 0 and parts[-1][1] == 8 and all(a[1] == b[0] and a[1] > a[0] for a, b in zip(parts, parts[1:]))
+    assert max(wts[lo:hi].sum() for lo, hi in parts) <= 16.0
+    assert slab_layers(3, 3, np.array([100.0, 0.0, 0.0])) == [(0, 1), (1, 2), (2, 3)]
+    with pytest.raises(ValueError):
+        slab_layers(8, 2, np.ones(7))
     assert neighbours(0, 1) == (None, None)
     assert neighbours(0, 3) == (None, 1) and neighbours(1, 3) == (0, 2) and neighbours(2, 3) == (1, None)
 
