@@ -22,6 +22,23 @@ namespace cuba {
 #define CUBA_FORCE_SLOW_PATHS 0
 #endif
 
+// Phase clocks (diagnostic builds only, -DCUBA_PHASE_CLOCKS): thread 0 of every CTA of the 256-thread class adds
+// the cycles between consecutive marks to a per-phase total; mark k closes phase k (its barrier wait included).
+#ifdef CUBA_PHASE_CLOCKS
+__device__ unsigned long long g_phase[16];
+__device__ __forceinline__ void phase_mark(long long &last, int k)
+{
+    if (threadIdx.x == 0 && blockDim.x == 256) {
+        const long long t = clock64();
+        atomicAdd(&g_phase[k], (unsigned long long)(t - last));
+        last = t;
+    }
+}
+#define CUBA_MARK(k) phase_mark(g_last, k)
+#else
+#define CUBA_MARK(k)
+#endif
+
 struct CollideParams {
     uint64_t seed;
     uint32_t rk[20];      // Philox round keys: rk[2r] = seed_lo + r*0x9E3779B9, rk[2r+1] = seed_hi + r*0xBB67AE85
@@ -781,7 +798,11 @@ __device__ __forceinline__ void rank_dirty(const CollideParams &P, const CtaStat
 // keepE: the caller needs the energies of the final momenta in sE afterwards.
 template <int THREADS, int ITEMS, int G, int CAP, int LCAP, bool TRACE>
 __device__ __forceinline__ void run_sweeps(const CollideParams &P, uint32_t c, uint32_t n, int R, uint32_t tcur,
-                                               bool hist, uint32_t *s_warp, CtaStats *stats)
+                                               bool hist, uint32_t *s_warp, CtaStats *stats
+#ifdef CUBA_PHASE_CLOCKS
+                                               , long long &g_last
+#endif
+                                               )
 {
     using S = CellSmem<CAP, LCAP>;
     constexpr int NG = ITEMS / G;
@@ -840,6 +861,7 @@ __device__ __forceinline__ void run_sweeps(const CollideParams &P, uint32_t c, u
             }
         }
         __syncthreads();
+        CUBA_MARK(1);
         // (B) per word: elements = popc + duplicates, both rounds packed in one word; exclusive scan
         {
             const uint32_t chunk = ((n + THREADS - 1) / THREADS) | 1u;
@@ -867,6 +889,7 @@ __device__ __forceinline__ void run_sweeps(const CollideParams &P, uint32_t c, u
             }
         }
         __syncthreads();
+        CUBA_MARK(2);
         // (C1) rank = prefix of the word + occupied bits below mine; elements of dirty words go onto a list
 #pragma unroll
         for (int it = 0; it < ITEMS; ++it) {
@@ -876,13 +899,15 @@ __device__ __forceinline__ void run_sweeps(const CollideParams &P, uint32_t c, u
             if (two) rank_clean<S, LCAP, 1>(P, stats, keyB[it], j, n, M, tcur, rho0 + 1);
         }
         __syncthreads();
+        CUBA_MARK(3);
         // (C2) the listed elements, one thread each
         rank_dirty<S, LCAP, THREADS>(P, stats, n, M, tcur, rho0, two);
         __syncthreads();
+        CUBA_MARK(4);
         // pair phases of the two rounds; energies appear in the first one
 #pragma unroll 1
         for (int sl = 0; sl < (two ? 2 : 1); ++sl) {
-            if (sl) __syncthreads();
+            if (sl) { __syncthreads(); CUBA_MARK(5); }
             pair_phase<S, THREADS, PITEMS, TRACE>(P, c, n, tcur, rho0 + sl, sl, sl == 0, sl == 0 ? (two || hist) : hist, stats);
         }
     }
@@ -892,7 +917,11 @@ template <int THREADS, int ITEMS, int G, int CAP, int LCAP, bool TRACE, bool LOC
 __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32_t c, uint32_t lo, uint32_t n,
                                                   uint32_t *s_warp, CtaStats *stats,
                                                   uint32_t *s_seg, long long *s_esum,
-                                                  uint32_t lo_next, uint32_t n_next)
+                                                  uint32_t lo_next, uint32_t n_next
+#ifdef CUBA_PHASE_CLOCKS
+                                                  , long long &g_last
+#endif
+                                                  )
 {
     static_assert(ITEMS % G == 0, "items are processed in groups of G");
     constexpr int NG = ITEMS / G;
@@ -955,6 +984,7 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
         for (uint32_t e = tid; e < ((lo + n - 1u) / kTile - lo / kTile + 1u) * kDirs; e += THREADS) s_seg[e] = 0;
     if (local) block_sum_ll_post<THREADS>(esum, s_esum);
     __syncthreads();
+    CUBA_MARK(0);
     if (local) {
         base = local_base(block_sum_ll_read<THREADS>(s_esum), n, P.dt, P.etas);
         const double pmax = (2.0 * cn) * base;
@@ -974,12 +1004,17 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
         if (hist) { prefetch_l2(P.x + e); prefetch_l2(P.y + e); prefetch_l2(P.z + e); }
     }
 
+#ifdef CUBA_PHASE_CLOCKS
+    run_sweeps<THREADS, ITEMS, G, CAP, LCAP, TRACE>(P, c, n, R, tcur, hist, s_warp, stats, g_last);
+#else
     run_sweeps<THREADS, ITEMS, G, CAP, LCAP, TRACE>(P, c, n, R, tcur, hist, s_warp, stats);
+#endif
     if (R == 0 && hist && tid == 0) {     // a lone particle: no pair phase has computed its energy
         const double2 xy = S::pxy()[0];
         sE[0] = energy(xy.x, xy.y, S::pz()[0]);
     }
     __syncthreads();
+    CUBA_MARK(6);
     const uint32_t lo_w = *reinterpret_cast<volatile uint32_t *>(&stats->lo);
     constexpr int HB = (ITEMS % 2 == 0) ? 2 : 1;
 #pragma unroll 1
@@ -990,17 +1025,28 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
     if (tid == 0) { stats->pairs += (unsigned long long)R * (n >> 1); stats->rounds += (unsigned long long)R; }
 
     // ---- fused histogram of the next step (S1-S3 of step t+1 on the final momenta) ----------
+    // The positions of group g + 1 are in flight while group g is worked on (the loads hit L2: the cell was
+    // prefetched while the previous one was processed; their latency is what this phase used to wait for).
     if (hist) {
         const uint32_t T0 = lo_w / kTile;
         const HistCell &hc = stats->h;
+        constexpr int NGH = ITEMS / HB;
+        double xx[HB], yy[HB], zz[HB];
+#pragma unroll
+        for (int i = 0; i < HB; ++i) {
+            const uint32_t jc = lo_w + min((uint32_t)(tid + i * THREADS), last);
+            xx[i] = P.x[jc]; yy[i] = P.y[jc]; zz[i] = P.z[jc];
+        }
 #pragma unroll 1
-        for (int g = 0; g < ITEMS / HB; ++g) {
+        for (int g = 0; g < NGH; ++g) {
             if ((uint32_t)(g * HB * THREADS) >= n) break;
-            double xx[HB], yy[HB], zz[HB];
+            double xn[HB], yn[HB], zn[HB];
+            const bool more = g + 1 < NGH && (uint32_t)((g + 1) * HB * THREADS) < n;
 #pragma unroll
             for (int i = 0; i < HB; ++i) {
-                const uint32_t jc = lo_w + min((uint32_t)(tid + (g * HB + i) * THREADS), last);
-                xx[i] = P.x[jc]; yy[i] = P.y[jc]; zz[i] = P.z[jc];
+                const uint32_t jc = lo_w + min((uint32_t)(tid + ((g + 1) * HB + i) * THREADS), last);
+                xn[i] = xx[i]; yn[i] = yy[i]; zn[i] = zz[i];
+                if (more) { xn[i] = P.x[jc]; yn[i] = P.y[jc]; zn[i] = P.z[jc]; }
             }
 #pragma unroll
             for (int i = 0; i < HB; ++i) {
@@ -1012,8 +1058,11 @@ __device__ __forceinline__ void collide_cell_smem(const CollideParams &P, uint32
                     atomicAdd(&s_seg[((lo_w + j) / kTile - T0) * kDirs + (uint32_t)max(d, 0)], 1u);
                 }
             }
+#pragma unroll
+            for (int i = 0; i < HB; ++i) { xx[i] = xn[i]; yy[i] = yn[i]; zz[i] = zn[i]; }
         }
         __syncthreads();
+        CUBA_MARK(7);
         hist_fill_stay<THREADS>(lo_w, n, s_seg);
         __syncthreads();
         hist_publish<THREADS>(P, c, lo_w, n, s_seg);
@@ -1096,15 +1145,25 @@ k_collide(CollideParams P)
     uint32_t item = s_item[0];
     uint4 cur = make_uint4(0u, 0u, 0u, 0u);
     if (item < nlist) cur = P.list[item];
+#ifdef CUBA_PHASE_CLOCKS
+    long long g_last = clock64();
+#endif
     for (int it = 0; item < nlist; ++it) {
         if (threadIdx.x == 0) s_item[(it + 1) & 1] = atomicAdd(P.work, 1u);
         __syncthreads();
+        CUBA_MARK(9);
         item = s_item[(it + 1) & 1];
         uint4 nxt = make_uint4(0u, 0u, 0u, 0u);
         if (item < nlist) nxt = P.list[item];   // first used after the staging barrier
+#ifdef CUBA_PHASE_CLOCKS
+        collide_cell_smem<THREADS, ITEMS, G, CAP, LCAP, TRACE, LOCAL, GRAPH>(P, cur.x, cur.y, cur.z, s_warp, &s_stats, s_seg, s_esum,
+                                                                        nxt.y, nxt.z, g_last);
+#else
         collide_cell_smem<THREADS, ITEMS, G, CAP, LCAP, TRACE, LOCAL, GRAPH>(P, cur.x, cur.y, cur.z, s_warp, &s_stats, s_seg, s_esum,
                                                                         nxt.y, nxt.z);
+#endif
         __syncthreads();
+        CUBA_MARK(8);
         cur = nxt;
     }
     if (threadIdx.x == 0) {       // the loop ends with a block barrier

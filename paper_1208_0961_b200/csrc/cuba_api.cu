@@ -1328,6 +1328,16 @@ int cuba_slab_unpack(cuba_ctx *ctx, const void *lo_buffer, int64_t lo_count, con
     return CUBA_OK;
 }
 
+#ifdef CUBA_PHASE_CLOCKS
+extern "C" int cuba_debug_phase(unsigned long long out[16], int reset)
+{
+    if (cudaDeviceSynchronize() != cudaSuccess) return CUBA_ERR_CUDA;
+    if (cudaMemcpyFromSymbol(out, g_phase, sizeof(unsigned long long) * 16) != cudaSuccess) return CUBA_ERR_CUDA;
+    if (reset) { unsigned long long z[16] = {}; cudaMemcpyToSymbol(g_phase, z, sizeof(z)); }
+    return CUBA_OK;
+}
+#endif
+
 int cuba_slot_stats(cuba_ctx *ctx, uint64_t out[2])
 {
     if (!ctx || !out) return CUBA_ERR_NULL;

@@ -254,7 +254,12 @@ __device__ __forceinline__ void step_cell_slots(const CollideParams &P, const Sl
         }
     }
     if (COLLIDE) {
+#ifdef CUBA_PHASE_CLOCKS
+        long long g_last = 0;
+        run_sweeps<THREADS, ITEMS, G, CAP, LCAP, false>(P, c, n, R, tcur, STREAM, s_warp, stats, g_last);
+#else
         run_sweeps<THREADS, ITEMS, G, CAP, LCAP, false>(P, c, n, R, tcur, STREAM, s_warp, stats);
+#endif
         if (STREAM && R == 0 && tid == 0) {     // a lone particle: no pair phase has computed its energy
             const double2 xy = S::pxy()[0];
             sE[0] = energy(xy.x, xy.y, S::pz()[0]);
