@@ -54,12 +54,18 @@ bool cuda_ok(cudaError_t e, const char *what)
 #ifndef CUBA_C0_MB
 #define CUBA_C0_MB 16
 #endif
+#ifndef CUBA_C2_MB
+#define CUBA_C2_MB 8
+#endif
+#ifndef CUBA_C3_MB
+#define CUBA_C3_MB 4
+#endif
 #define CUBA_FOR_EACH_CLASS(X) \
     X(6, 1024, 5, 4544, 1)     \
     X(5, 512, 4, 2048, 2)      \
     X(4, CUBA_C4_T, CUBA_C4_I, CUBA_C4_CAP, CUBA_C4_MB) \
-    X(3, 224, 4, 896, 4)       \
-    X(2, 128, 4, 512, 8)       \
+    X(3, 224, 4, 896, CUBA_C3_MB) \
+    X(2, 128, 4, 512, CUBA_C2_MB) \
     X(1, 64, 4, 256, CUBA_C1_MB) \
     X(0, 32, 4, 128, CUBA_C0_MB)
 constexpr int kSmemClasses = 7;
