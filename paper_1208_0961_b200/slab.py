@@ -69,8 +69,10 @@ def neighbours(rank: int, world: int):
     return (rank - 1 if rank > 0 else None, rank + 1 if rank + 1 < world else None)
 
 
-class SlabRank:
-    """One rank's context: cuba_slab_init and the per-step calls."""
+class SlabRank(Cuba):
+    """One rank's context: cuba_slab_init and the per-step calls.  The calls of `Cuba` apply to a slab context as
+    include/cuba.h says: step (one step at a time), step_local_sigma, counters and the observables (owned
+    particles only) work; step_traced and step_adaptive raise CubaError."""
 
     def __init__(self, w, layer_lo, layer_hi, device="cuda:0", capacity=None, stream=None):
         import torch
@@ -99,15 +101,12 @@ class SlabRank:
                                     float(w.n_test), int(w.seed), c_void_p(ws_ptr), wsb,
                                     c_void_p(self._stream.cuda_stream), self.layer_lo, self.layer_hi))
         self._h = h
+        self.ncells = self.ncell[0] * self.ncell[1] * self.ncell[2]
 
-    # the calls of Cuba that apply unchanged to a slab context
-    step = Cuba.step
-    observables = Cuba.observables
-    observables_lrf = Cuba.observables_lrf
-    counters = Cuba.counters
-    step_local_sigma = Cuba.step_local_sigma
-    close = Cuba.close
-    __del__ = Cuba.__del__
+    @property
+    def n(self):
+        """Particles in the local store (owned + ghosts); changes with every halo exchange."""
+        return self.owned()[2]
 
     def owned(self):
         """(first slot, count) of the owned part of the store, particles in the store, capacity."""
@@ -151,11 +150,8 @@ class SlabRank:
 
     def owned_particles(self):
         """(pid, x, y, z, px, py, pz) of the owned part as host numpy arrays, in array order."""
-        first, cnt, n, _ = self.owned()
-        pid = np.zeros(n, dtype=np.uint32)
-        a = [np.zeros(n) for _ in range(6)]
-        _check(lib().cuba_get_particles(self._h, pid.ctypes.data_as(c_void_p), *[v.ctypes.data_as(c_void_p) for v in a]))
-        return tuple(v[first:first + cnt] for v in (pid, *a))
+        first, cnt, _, _ = self.owned()
+        return tuple(v[first:first + cnt] for v in self.particles())
 
 
 def exchange_halos(dist, rank, world, send_lo, send_hi, device):
@@ -188,9 +184,13 @@ def exchange_halos(dist, rank, world, send_lo, send_hi, device):
     return recv[0], recv[1]
 
 
-def slab_step(ctx: SlabRank, dist, rank, world, dt, sigma):
-    """One step of one rank of a torch.distributed job: step, pack, exchange, unpack."""
-    ctx.step(1, dt, sigma)
+def slab_step(ctx: SlabRank, dist, rank, world, dt, sigma, eta_over_s=None):
+    """One step of one rank of a torch.distributed job: step, pack, exchange, unpack.  eta_over_s: the per-cell
+    cross section of cuba_step_local_sigma instead of sigma."""
+    if eta_over_s is None:
+        ctx.step(1, dt, sigma)
+    else:
+        ctx.step_local_sigma(1, dt, eta_over_s)
     lo, hi = neighbours(rank, world)
     send_lo = ctx.pack(0) if lo is not None else None
     send_hi = ctx.pack(1) if hi is not None else None
@@ -209,10 +209,13 @@ class LocalSlabGroup:
         self.layers = slab_layers(nx, self.world, layer_weights(w.x, float(w.box[0]), nx) if balance else None)
         self.ranks = [SlabRank(w, lo, hi, device=device, capacity=capacity) for lo, hi in self.layers]
 
-    def step(self, nsteps, dt, sigma):
+    def step(self, nsteps, dt, sigma, eta_over_s=None):
         for _ in range(int(nsteps)):
             for r in self.ranks:
-                r.step(1, dt, sigma)
+                if eta_over_s is None:
+                    r.step(1, dt, sigma)
+                else:
+                    r.step_local_sigma(1, dt, eta_over_s)
             sent = []
             for k, r in enumerate(self.ranks):
                 lo, hi = neighbours(k, self.world)

@@ -70,6 +70,27 @@ def test_slab_with_many_rounds_walls_and_thin_layers(cuba, oracle_mod):
     grp.close()
 
 
+def test_slab_with_the_local_cross_section(cuba, oracle_mod):
+    """cuba_step_local_sigma (constant eta/s, A24) in a slab context: the per-cell factor needs the cell's own
+    particles only, so the decomposition stays exact; mixed with constant-sigma steps."""
+    w = workloads.riemann_small(seed=55)
+    o = oracle_mod.Oracle.from_workload(w)
+    grp = cuba.LocalSlabGroup(w, 3)
+    grp.step(3, w.dt, w.sigma, eta_over_s=0.1)
+    o.step_etas(3, w.dt, 0.1)
+    grp.step(1, w.dt, w.sigma)
+    o.step(1, w.dt, w.sigma)
+    grp.step(2, w.dt, w.sigma, eta_over_s=0.02)
+    o.step_etas(2, w.dt, 0.02)
+    for a, c in zip(grp.particles(), o.particles()):
+        assert np.array_equal(a, c)
+    cg, co = grp.counters(), o.counters()
+    assert (cg["pairs"], cg["collisions"], cg["rounds"]) == (co["pairs"], co["collisions"], co["rounds"])
+    with pytest.raises(cuba.CubaError):
+        grp.ranks[0].step_adaptive(1, w.dt, w.sigma)
+    grp.close()
+
+
 def test_slab_cuts_balanced_by_particles(cuba, oracle_mod):
     """The cuts follow the particles per layer (the hot half of the Riemann problem gets more ranks); same bits."""
     w = workloads.riemann_small(seed=54)
