@@ -1201,6 +1201,42 @@ k_slab_pack_counts(const uint32_t *__restrict__ cell_start, uint32_t c0, uint32_
     if (i < nyz) counts[i] = cell_start[c0 + i + 1] - cell_start[c0 + i];
 }
 
+// Copies up to three runs of particles (seven arrays each) into dst[0 .. n0 + n1 + n2): one launch instead of 21
+// copies.  A run is (source arrays, first slot, count); a halo buffer is a source whose arrays are its sections.
+struct SlabRun { const double *a[6]; const uint32_t *pid; uint32_t first, count; };
+
+__global__ void __launch_bounds__(256)
+k_slab_gather(SlabRun r0, SlabRun r1, SlabRun r2, Soa dst, uint32_t dst_first)
+{
+    const uint32_t total = r0.count + r1.count + r2.count;
+    for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < total; i += gridDim.x * 256u) {
+        const SlabRun &r = i < r0.count ? r0 : (i < r0.count + r1.count ? r1 : r2);
+        const uint32_t k = r.first + (i < r0.count ? i : (i < r0.count + r1.count ? i - r0.count : i - r0.count - r1.count));
+        const uint32_t o = dst_first + i;
+        dst.x[o] = r.a[0][k]; dst.y[o] = r.a[1][k]; dst.z[o] = r.a[2][k];
+        dst.px[o] = r.a[3][k]; dst.py[o] = r.a[4][k]; dst.pz[o] = r.a[5][k];
+        dst.pid[o] = r.pid[k];
+    }
+}
+
+static SlabRun slab_run_of_store(const Soa &s, uint32_t first, uint32_t count)
+{
+    SlabRun r{};
+    r.a[0] = s.x; r.a[1] = s.y; r.a[2] = s.z; r.a[3] = s.px; r.a[4] = s.py; r.a[5] = s.pz;
+    r.pid = s.pid; r.first = first; r.count = count;
+    return r;
+}
+
+static SlabRun slab_run_of_buffer(const unsigned char *b, uint32_t count)
+{
+    SlabRun r{};
+    if (b)
+        for (int k = 0; k < 6; ++k) r.a[k] = reinterpret_cast<const double *>(b + 16 + (size_t)k * count * 8);
+    r.pid = b ? reinterpret_cast<const uint32_t *>(b + 16 + (size_t)count * 48) : nullptr;
+    r.first = 0; r.count = b ? count : 0u;
+    return r;
+}
+
 // population of every cell of the rebuilt store + per-block sums for the scan
 __global__ void __launch_bounds__(256)
 k_slab_counts(uint32_t ncells, const uint32_t *__restrict__ cell_start_old, uint32_t own_lo, uint32_t own_hi, uint32_t nyz,
@@ -1268,11 +1304,15 @@ int cuba_slab_pack(cuba_ctx *ctx, int side, void *buffer, size_t buffer_bytes)
     if (buffer_bytes < cuba_slab_buffer_bytes(count, ctx->g.nc)) return CUBA_ERR_SIZE;
     unsigned char *b = static_cast<unsigned char *>(buffer);
     cudaStream_t st = ctx->stream;
-    const Soa &c = ctx->set[ctx->cur];
-    const double *arr[6] = {c.x, c.y, c.z, c.px, c.py, c.pz};
-    for (int k = 0; k < 6; ++k)
-        if (count) CU(cudaMemcpyAsync(b + 16 + (size_t)k * count * 8, arr[k] + first, (size_t)count * 8, cudaMemcpyDeviceToDevice, st));
-    if (count) CU(cudaMemcpyAsync(b + 16 + (size_t)count * 48, c.pid + first, (size_t)count * 4, cudaMemcpyDeviceToDevice, st));
+    if (count) {
+        Soa dst{};
+        double **d6[6] = {&dst.x, &dst.y, &dst.z, &dst.px, &dst.py, &dst.pz};
+        for (int k = 0; k < 6; ++k) *d6[k] = reinterpret_cast<double *>(b + 16 + (size_t)k * count * 8);
+        dst.pid = reinterpret_cast<uint32_t *>(b + 16 + (size_t)count * 48);
+        const SlabRun none{};
+        k_slab_gather<<<std::min<unsigned>((count + 255u) / 256u, 148u * 8u), 256, 0, st>>>(slab_run_of_store(ctx->set[ctx->cur], first, count), none, none, dst, 0u);
+        LAUNCHED();
+    }
     k_slab_pack_counts<<<(nyz + 255u) / 256u, 256, 0, st>>>(ctx->at<uint32_t>(ctx->lay.cell_start), c0, nyz, count,
                                                             reinterpret_cast<unsigned long long *>(b),
                                                             reinterpret_cast<uint32_t *>(b + 16 + (size_t)count * 52));
@@ -1296,17 +1336,11 @@ int cuba_slab_unpack(cuba_ctx *ctx, const void *lo_buffer, int64_t lo_count, con
     if (n_new < 1 || n_new > ctx->cap) return CUBA_ERR_SIZE;
     cudaStream_t st = ctx->stream;
     const Soa &from = ctx->set[ctx->cur], &to = ctx->set[1 - ctx->cur];
-    const double *src[6] = {from.x, from.y, from.z, from.px, from.py, from.pz};
-    double *dst[6] = {to.x, to.y, to.z, to.px, to.py, to.pz};
     const unsigned char *lb = static_cast<const unsigned char *>(lo_buffer), *hb = static_cast<const unsigned char *>(hi_buffer);
-    for (int k = 0; k < 6; ++k) {
-        if (lo_count) CU(cudaMemcpyAsync(dst[k], lb + 16 + (size_t)k * lo_count * 8, (size_t)lo_count * 8, cudaMemcpyDeviceToDevice, st));
-        if (own_count) CU(cudaMemcpyAsync(dst[k] + lo_count, src[k] + own_first, (size_t)own_count * 8, cudaMemcpyDeviceToDevice, st));
-        if (hi_count) CU(cudaMemcpyAsync(dst[k] + lo_count + own_count, hb + 16 + (size_t)k * hi_count * 8, (size_t)hi_count * 8, cudaMemcpyDeviceToDevice, st));
-    }
-    if (lo_count) CU(cudaMemcpyAsync(to.pid, lb + 16 + (size_t)lo_count * 48, (size_t)lo_count * 4, cudaMemcpyDeviceToDevice, st));
-    if (own_count) CU(cudaMemcpyAsync(to.pid + lo_count, from.pid + own_first, (size_t)own_count * 4, cudaMemcpyDeviceToDevice, st));
-    if (hi_count) CU(cudaMemcpyAsync(to.pid + lo_count + own_count, hb + 16 + (size_t)hi_count * 48, (size_t)hi_count * 4, cudaMemcpyDeviceToDevice, st));
+    k_slab_gather<<<std::min<unsigned>((unsigned)((n_new + 255) / 256), 148u * 8u), 256, 0, st>>>(
+        slab_run_of_buffer(lb, (uint32_t)lo_count), slab_run_of_store(from, own_first, (uint32_t)own_count),
+        slab_run_of_buffer(hb, (uint32_t)hi_count), to, 0u);
+    LAUNCHED();
     // cell table of the rebuilt store
     const uint32_t ncells = ctx->g.ncells, nyz = (uint32_t)(ctx->g.nc[1] * ctx->g.nc[2]);
     uint32_t *zero = ctx->at<uint32_t>(lay.zero);
