@@ -739,29 +739,40 @@ __device__ __forceinline__ void pair_phase(const CollideParams &P, uint32_t c, u
 
 // Phase C1 for one element and one of the two rounds of a sweep (slot 0 / 1): the rank of an element of
 // a clean word; an element of a dirty word goes onto the round's list, chained by word mod kChains.
-template <typename S, int LCAP, int SLOT>
-__device__ __forceinline__ void rank_clean(const CollideParams &P, CtaStats *stats,
-                                           uint32_t k, uint32_t j, uint32_t n, uint32_t M,
-                                           uint32_t tcur, int rho)
+// Clean part, straight-line: rank of the element if its word holds no duplicate, stored right away; returns true
+// for an element of a dirty word, which rank_listed handles.
+template <typename S, int SLOT>
+__device__ __forceinline__ bool rank_clean(uint32_t k, uint32_t j, bool valid, uint32_t n, uint32_t M)
 {
     const uint32_t b = __umulhi(k, M), word = b >> 5, below = (1u << (b & 31u)) - 1u;
     const uint32_t cw = S::cnt()[word];
     const uint32_t pw = SLOT ? (cw >> 16) : (cw & 0xFFFFu);
-    uint32_t rank = (pw >> 1) + __popc((S::bm() + SLOT * n)[word] & below);
-    if (j < n) {
-        if (CUBA_FORCE_SLOW_PATHS || (pw & 1u)) {
-            const uint32_t at = atomicAdd(&stats->nlist[SLOT], 1u);
-            if (at < (uint32_t)LCAP) {
-                const uint32_t next = atomicExch(&stats->head[SLOT][word % kChains], at);
-                S::lkey(SLOT)[at] = k;
-                S::lwj(SLOT)[at] = (word << 13) | j;
-                S::lpn(SLOT)[at] = (pw >> 1) | (next << 16);
-                return;
-            }
-            rank = (pw >> 1) + brute_rank(P.seed, tcur, S::pid(), n, M, word, k, S::pid()[j], rho);   // the list is full
-        }
-        S::ord(SLOT)[rank] = (uint16_t)j;
+    const uint32_t rank = (pw >> 1) + __popc((S::bm() + SLOT * n)[word] & below);
+    const bool dirty = CUBA_FORCE_SLOW_PATHS || (pw & 1u);
+    if (valid && !dirty) S::ord(SLOT)[rank] = (uint16_t)j;
+    return valid && dirty;
+}
+
+// An element of a dirty word goes onto the round's list, chained by word mod kChains (phase C2 ranks it).
+// slot is a run-time value here: the few listed elements of a thread are handled one after the other.
+template <typename S, int LCAP>
+__device__ __forceinline__ void rank_listed(const CollideParams &P, CtaStats *stats, int slot,
+                                            uint32_t k, uint32_t j, uint32_t n, uint32_t M,
+                                            uint32_t tcur, int rho)
+{
+    const uint32_t b = __umulhi(k, M), word = b >> 5;
+    const uint32_t cw = S::cnt()[word];
+    const uint32_t pw = slot ? (cw >> 16) : (cw & 0xFFFFu);
+    const uint32_t at = atomicAdd(&stats->nlist[slot], 1u);
+    if (at < (uint32_t)LCAP) {
+        const uint32_t next = atomicExch(&stats->head[slot][word % kChains], at);
+        S::lkey(slot)[at] = k;
+        S::lwj(slot)[at] = (word << 13) | j;
+        S::lpn(slot)[at] = (pw >> 1) | (next << 16);
+        return;
     }
+    const uint32_t rank = (pw >> 1) + brute_rank(P.seed, tcur, S::pid(), n, M, word, k, S::pid()[j], rho);   // the list is full
+    S::ord(slot)[rank] = (uint16_t)j;
 }
 
 // Phase C2, one thread per list entry (the two lists side by side, each on its own half of the CTA): rank
@@ -890,13 +901,26 @@ __device__ __forceinline__ void run_sweeps(const CollideParams &P, uint32_t c, u
         }
         __syncthreads();
         CUBA_MARK(2);
-        // (C1) rank = prefix of the word + occupied bits below mine; elements of dirty words go onto a list
+        // (C1) rank = prefix of the word + occupied bits below mine, all items of the thread in one straight-line
+        // block; then every thread lists its elements of dirty words one after the other (about 5 % of the
+        // elements: a warp loops two or three times instead of branching once per item and round)
+        uint32_t listed = 0;
 #pragma unroll
         for (int it = 0; it < ITEMS; ++it) {
-            if (it >= nit) break;
             const uint32_t j = tid + it * THREADS;
-            rank_clean<S, LCAP, 0>(P, stats, keyA[it], j, n, M, tcur, rho0);
-            if (two) rank_clean<S, LCAP, 1>(P, stats, keyB[it], j, n, M, tcur, rho0 + 1);
+            const bool valid = it < nit && j < n;
+            listed |= (rank_clean<S, 0>(keyA[it], j, valid, n, M) ? 1u : 0u) << (2 * it);
+            if (two) listed |= (rank_clean<S, 1>(keyB[it], j, valid, n, M) ? 2u : 0u) << (2 * it);
+        }
+        while (__any_sync(0xFFFFFFFFu, listed != 0u)) {
+            if (listed) {
+                const int e = __ffs(listed) - 1, it = e >> 1, sl = e & 1;
+                listed &= listed - 1u;
+                uint32_t k = 0;
+#pragma unroll
+                for (int q = 0; q < ITEMS; ++q) k = (q == it) ? (sl ? keyB[q] : keyA[q]) : k;
+                rank_listed<S, LCAP>(P, stats, sl, k, tid + it * THREADS, n, M, tcur, rho0 + sl);
+            }
         }
         __syncthreads();
         CUBA_MARK(3);
