@@ -1164,21 +1164,22 @@ k_collide(CollideParams P)
     const uint32_t nlist = *P.list_count;
     if (threadIdx.x == 0) { s_stats.near = 0; s_stats.hits = 0; s_stats.pairs = 0; s_stats.rounds = 0; }
     __shared__ uint32_t s_item[2];
-    if (threadIdx.x == 0) s_item[0] = atomicAdd(P.work, 1u);
+    if (threadIdx.x == 0) { s_item[0] = atomicAdd(P.work, 1u); s_item[1] = 0xFFFFFFFFu; }
     __syncthreads();
     uint32_t item = s_item[0];
     uint4 cur = make_uint4(0u, 0u, 0u, 0u);
     if (item < nlist) cur = P.list[item];
+    if (threadIdx.x == 0 && item < nlist) s_item[1] = atomicAdd(P.work, 1u);
+    __syncthreads();
 #ifdef CUBA_PHASE_CLOCKS
     long long g_last = clock64();
 #endif
+    // One block barrier per cell: thread 0 claims the cell after the next one at the END of a cell, so that the
+    // barrier that frees the shared memory for the next cell also publishes the claim.
     for (int it = 0; item < nlist; ++it) {
-        if (threadIdx.x == 0) s_item[(it + 1) & 1] = atomicAdd(P.work, 1u);
-        __syncthreads();
-        CUBA_MARK(9);
-        item = s_item[(it + 1) & 1];
+        const uint32_t item_next = s_item[(it + 1) & 1];
         uint4 nxt = make_uint4(0u, 0u, 0u, 0u);
-        if (item < nlist) nxt = P.list[item];   // first used after the staging barrier
+        if (item_next < nlist) nxt = P.list[item_next];   // first used after the staging barrier
 #ifdef CUBA_PHASE_CLOCKS
         collide_cell_smem<THREADS, ITEMS, G, CAP, LCAP, TRACE, LOCAL, GRAPH>(P, cur.x, cur.y, cur.z, s_warp, &s_stats, s_seg, s_esum,
                                                                         nxt.y, nxt.z, g_last);
@@ -1186,9 +1187,11 @@ k_collide(CollideParams P)
         collide_cell_smem<THREADS, ITEMS, G, CAP, LCAP, TRACE, LOCAL, GRAPH>(P, cur.x, cur.y, cur.z, s_warp, &s_stats, s_seg, s_esum,
                                                                         nxt.y, nxt.z);
 #endif
+        if (threadIdx.x == 0) s_item[it & 1] = item_next < nlist ? atomicAdd(P.work, 1u) : 0xFFFFFFFFu;
         __syncthreads();
         CUBA_MARK(8);
         cur = nxt;
+        item = item_next;
     }
     if (threadIdx.x == 0) {       // the loop ends with a block barrier
         if (s_stats.hits) atomicAdd(&P.counters[1], (unsigned long long)s_stats.hits);
