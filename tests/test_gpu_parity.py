@@ -676,3 +676,12 @@ def test_short_trace_capacity_completes_the_step(cuba, oracle_mod):
     g.step(3, w.dt, w.sigma)
     o.step(3, w.dt, w.sigma)
     assert_state_equal(g.particles(), o.particles())
+
+
+def test_fp64_probe_reports_a_plausible_peak(cuba):
+    """cuba_probe_fp64 (the measured fp64 leg of the roofline): a B200 does tens of TFLOP/s in fp64; argument errors."""
+    rate = cuba.probe_fp64(repeats=2)
+    assert 2e12 < rate < 4e13                       # thread-level DFMA per second (x 2 = FLOP/s)
+    with pytest.raises(cuba.CubaError):
+        cuba.probe_fp64(repeats=0)
+

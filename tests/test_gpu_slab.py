@@ -91,6 +91,21 @@ def test_slab_with_the_local_cross_section(cuba, oracle_mod):
     grp.close()
 
 
+def test_slab_tensor_observables_add_up(cuba, oracle_mod):
+    """cuba_observables_lrf in a slab context covers the owned particles: the five tensor components per slab are
+    sums over particles, so the ranks' results add up to the oracle's (1e-12); the Landau-matched quantities are
+    not additive and are formed from the summed tensor by the caller."""
+    w = workloads.riemann_small(seed=56)
+    o = oracle_mod.Oracle.from_workload(w)
+    grp = cuba.LocalSlabGroup(w, 2)
+    grp.step(3, w.dt, w.sigma)
+    o.step(3, w.dt, w.sigma)
+    T = sum(r.observables_lrf(16)[0] for r in grp.ranks)
+    To, _ = o.observables_lrf(16)
+    assert np.allclose(T, To, rtol=1e-12, atol=1e-300)
+    grp.close()
+
+
 def test_slab_cuts_balanced_by_particles(cuba, oracle_mod):
     """The cuts follow the particles per layer (the hot half of the Riemann problem gets more ranks); same bits."""
     w = workloads.riemann_small(seed=54)
