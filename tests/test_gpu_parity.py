@@ -4,6 +4,7 @@
      counted -- there are none), state within 1e-12 relative (in fact identical bits);
  (ii) many steps: state still identical, energy-density profiles within 1e-12."""
 import math
+import os
 
 import numpy as np
 import pytest
@@ -513,7 +514,7 @@ def test_stress_geometries_match_oracle(cuba, oracle_mod, case):
             assert oc["collisions"] > 100
 
 
-@pytest.mark.parametrize("seed", range(16))
+@pytest.mark.parametrize("seed", range(int(os.environ.get("CUBA_FUZZ_SEEDS", "16"))))
 def test_random_configurations_match_oracle(cuba, oracle_mod, seed):
     """Seeded fuzz over the parameter space: box shape, grid, density, cross section (from no
     collisions to several rounds), dt up to the CFL limit, step mix (fixed / traced / adaptive /
@@ -540,6 +541,7 @@ def test_random_configurations_match_oracle(cuba, oracle_mod, seed):
     g = cuba.Cuba.from_workload(w, stream=stream)
     g.set_option(1, int(rng.integers(0, 2)))
     g.set_option(2, int(rng.integers(0, 2)))
+    g.set_option(3, int(np.random.default_rng(7000 + seed).integers(0, 3)))      # compact or slotted schedule
     o = oracle_mod.Oracle.from_workload(w)
 
     def check():
