@@ -456,7 +456,9 @@ __device__ __forceinline__ void hist_publish(const CollideParams &P, uint32_t c,
 //     duplicates, both rounds packed into one 32-bit scan.  Phase C: rank = prefix of the word +
 //     popc(bits below mine) -- two loads and a popc, no parked keys, no comparisons.  The ~5 % of the
 //     elements whose word holds a duplicate ("dirty" words) put (key, word, index) on a short list
-//     in phase B and rank themselves inside the word by scanning that list, with the pid deciding
+//     at the end of phase C (every thread lists its own, one per loop trip: a branch taken once per
+//     item and round would be executed by almost every warp for one or two lanes) and rank themselves
+//     inside the word by scanning that list, with the pid deciding
 //     between equal 32-bit keys (A7); if the list overflows (never with uniform keys; forced in the
 //     slow-paths test build) a brute-force count over recomputed keys takes over.  The result depends
 //     on keys and pids only, never on the order in which threads arrived.
@@ -469,7 +471,9 @@ __device__ __forceinline__ void hist_publish(const CollideParams &P, uint32_t c,
 //     Hits are compacted per warp and a warp scatters its own hits right away (pairs are disjoint).
 //
 // Shared memory: 44 B per particle (p_x,p_y as one 16-byte element, p_z, pid, two bitmaps | E,
-// packed duplicate counters | prefixes, two 16-bit orders).  Block barriers per sweep of two rounds: 7.
+// packed duplicate counters | prefixes, two 16-bit orders).  Block barriers per sweep of two rounds: 7;
+// per cell otherwise: staging, end of the rounds, fused histogram (2), end of the cell (which also publishes the
+// claim of the cell after next).
 
 // 53-bit uniform from two Philox words, same value as u53(): both halves are exact integers
 // below 2^27 placed in the mantissa of 2^52, so every operation below is exact.
