@@ -156,7 +156,7 @@ int cuba_step_adaptive(cuba_ctx *ctx, int nsteps, double dt_max, double sigma, d
  * 2: every call does.  The slotted store is device memory allocated BY THE LIBRARY on first use (two
  * copies of ncells * slots-per-cell * 52 bytes, 7 GB at 25M particles) and freed by cuba_destroy -- the
  * one exception to "the caller owns all device memory", which is why it is opt-in; if the allocation
- * fails the compact schedule runs.  Measured at 25M particles: 1.64 vs 1.65 ms per step.  Results are
+ * fails the compact schedule runs.  Measured at 25M particles: 1.57 vs 1.61 ms per step.  Results are
  * bit-identical for every setting. */
 #define CUBA_OPT_SLOTS 3
 /* CUBA_OPT_SLOT_MARGIN (default 100): per cent by which the segment capacities of the slotted store
