@@ -275,7 +275,8 @@ static int occupancy_grid(K kernel, int threads, size_t smem, int sms, int *grid
 static int init_impl(cuba_ctx **out, const double box[3], const int ncell[3], int64_t cap, int64_t n,
                      double *x, double *y, double *z, double *px, double *py, double *pz,
                      double n_test, uint64_t seed, void *workspace, size_t workspace_bytes,
-                     void *cuda_stream, const uint32_t *pid_global, int layer_lo, int layer_hi, bool slab)
+                     void *cuda_stream, const uint32_t *pid_global, int layer_lo, int layer_hi, bool slab,
+                     cudaEvent_t momenta_ready = nullptr)   // non-null: px, py, pz are being written on another stream until this event
 {
     if (!out || !box || !ncell || !x || !y || !z || !px || !py || !pz || !workspace) return CUBA_ERR_NULL;
     *out = nullptr;
@@ -399,7 +400,8 @@ static int init_impl(cuba_ctx **out, const double box[3], const int ncell[3], in
             LAUNCHED();
             src = 1 - src;
         }
-        k_gather_perm<<<gb, 256, 0, st>>>(n, vals[src], ctx->set[0], ctx->set[1]);
+        if (momenta_ready) CU(cudaStreamWaitEvent(st, momenta_ready, 0));
+        k_gather_perm<<<gb, 256, 0, st>>>(n, vals[src], ctx->set[0], ctx->set[1], ctx->at<uint32_t>(lay.flags));
         LAUNCHED();
         if (pid_global) {
             k_map_pid<<<gb, 256, 0, st>>>(n, ctx->set[1].pid, pid_global);
@@ -1638,7 +1640,8 @@ int cuba_run_host(const double box[3], const int ncell[3], int64_t n,
     double *dev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     void *ws = nullptr;
     cuba_ctx *ctx = nullptr;
-    cudaStream_t st = nullptr;
+    cudaStream_t st = nullptr, st2 = nullptr;
+    cudaEvent_t ev_alloc = nullptr, ev_mom = nullptr;
     auto body = [&]() -> int {
         CU(cudaStreamCreate(&st));
         // stream-ordered allocations from a pool owned by the library, which keeps what it has been
@@ -1651,8 +1654,19 @@ int cuba_run_host(const double box[3], const int ncell[3], int64_t n,
         if (rp != CUBA_OK) return rp;
         for (int k = 0; k < 6; ++k) CU(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&dev[k]), (size_t)n * 8, pool, st));
         CU(cudaMallocFromPoolAsync(&ws, wsb, pool, st));
-        for (int k = 0; k < 6; ++k) CU(cudaMemcpyAsync(dev[k], host[k], (size_t)n * 8, cudaMemcpyHostToDevice, st));
-        int r = cuba_init(&ctx, box, ncell, n, dev[0], dev[1], dev[2], dev[3], dev[4], dev[5], n_test, seed, ws, wsb, st);
+        // positions on the main stream, momenta on a second one: the binning of the initial state needs the
+        // positions only until it gathers the sorted store, so the sort of the keys overlaps the second half of the upload
+        CU(cudaStreamCreateWithFlags(&st2, cudaStreamNonBlocking));
+        CU(cudaEventCreateWithFlags(&ev_alloc, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&ev_mom, cudaEventDisableTiming));
+        CU(cudaEventRecord(ev_alloc, st));
+        CU(cudaStreamWaitEvent(st2, ev_alloc, 0));
+        for (int k = 0; k < 3; ++k) CU(cudaMemcpyAsync(dev[k], host[k], (size_t)n * 8, cudaMemcpyHostToDevice, st));
+        for (int k = 3; k < 6; ++k) CU(cudaMemcpyAsync(dev[k], host[k], (size_t)n * 8, cudaMemcpyHostToDevice, st2));
+        CU(cudaEventRecord(ev_mom, st2));
+        if (!ncell) return CUBA_ERR_NULL;
+        int r = init_impl(&ctx, box, ncell, n, n, dev[0], dev[1], dev[2], dev[3], dev[4], dev[5], n_test, seed, ws, wsb, st,
+                          nullptr, 0, ncell[0] > 0 ? ncell[0] : 1, false, ev_mom);
         if (r != CUBA_OK) return r;
         r = cuba_step(ctx, nsteps, dt, sigma);
         if (r != CUBA_OK) return r;
@@ -1669,12 +1683,15 @@ int cuba_run_host(const double box[3], const int ncell[3], int64_t n,
     };
     const int rc = body();
     if (ctx) cuba_destroy(ctx);
+    if (st2) { cudaStreamSynchronize(st2); cudaStreamDestroy(st2); }     // (an early error may have left the copy running)
     if (st) {
         for (int k = 0; k < 6; ++k) if (dev[k]) cudaFreeAsync(dev[k], st);
         if (ws) cudaFreeAsync(ws, st);
         cudaStreamSynchronize(st);
         cudaStreamDestroy(st);
     }
+    if (ev_alloc) cudaEventDestroy(ev_alloc);
+    if (ev_mom) cudaEventDestroy(ev_mom);
     return rc;
 }
 

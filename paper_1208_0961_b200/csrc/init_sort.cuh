@@ -16,12 +16,12 @@ __global__ void __launch_bounds__(256)
 k_init_keys(Geom g, int64_t n, Soa in, uint32_t *__restrict__ keys, uint32_t *__restrict__ vals,
             uint32_t *__restrict__ flags)
 {
+    // positions only: the momenta are validated where they are first read (k_gather_perm), so that a caller
+    // who uploads them on a second stream can overlap that copy with the sort of the keys (cuba_run_host)
     const int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
     if (i >= n) return;
     const double x = in.x[i], y = in.y[i], z = in.z[i];
-    const double E = energy(in.px[i], in.py[i], in.pz[i]);
-    const bool ok = (x >= 0.0 && x <= g.L[0] && y >= 0.0 && y <= g.L[1] && z >= 0.0 && z <= g.L[2]) &&
-                    (E > 0.0) && isfinite(E);
+    const bool ok = (x >= 0.0 && x <= g.L[0] && y >= 0.0 && y <= g.L[1] && z >= 0.0 && z <= g.L[2]);
     if (!ok) atomicOr(flags, kFlagState);
     keys[i] = ok ? cell_linear(g, axis_index(x, g.inv_d[0], g.nc[0]), axis_index(y, g.inv_d[1], g.nc[1]),
                                axis_index(z, g.inv_d[2], g.nc[2])) : 0u;
@@ -159,13 +159,16 @@ k_rs_scatter(const uint32_t *__restrict__ keys, const uint32_t *__restrict__ val
 
 // out[k] = in[perm[k]] for the six fp64 arrays; pid[k] = perm[k] (ids are the original indices)
 __global__ void __launch_bounds__(256)
-k_gather_perm(int64_t n, const uint32_t *__restrict__ perm, Soa in, Soa out)
+k_gather_perm(int64_t n, const uint32_t *__restrict__ perm, Soa in, Soa out, uint32_t *__restrict__ flags)
 {
     const int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.x;
     if (k >= n) return;
     const uint32_t s = perm[k];
     out.x[k] = in.x[s]; out.y[k] = in.y[s]; out.z[k] = in.z[s];
-    out.px[k] = in.px[s]; out.py[k] = in.py[s]; out.pz[k] = in.pz[s];
+    const double px = in.px[s], py = in.py[s], pz = in.pz[s];
+    const double E = energy(px, py, pz);
+    if (!(E > 0.0) || !isfinite(E)) atomicOr(flags, kFlagState);       // finite momenta, |p| > 0 (A21)
+    out.px[k] = px; out.py[k] = py; out.pz[k] = pz;
     out.pid[k] = s;
 }
 
