@@ -188,6 +188,45 @@ int cuba_observables(cuba_ctx *ctx, double total[4], int nslab, double *edens);
  * 1 <= nslab <= 256 (CUBA_ERR_SIZE otherwise).  Synchronises; reports pending device errors. */
 int cuba_observables_lrf(cuba_ctx *ctx, int nslab, double *T, double *lrf);
 
+/* The totals and the energy density per x-slab of cuba_observables (Fig. 2), for
+ * callers that are not allowed to allocate GPU memory or to wait for the GPU: code that runs inside somebody
+ * else's memory budget (a plug-in of a host application that owns the allocator, a process sharing the GPU
+ * under a fixed memory reservation), an in-situ analysis hook called between steps of a running loop, where an
+ * allocation or a free can stall every stream of the device, or a service that pre-allocates everything at start-up and
+ * treats a later allocation as a fault.  cuba_observables needs a context (cuba_init allocates pinned host
+ * memory, streams and events) and keeps its per-block partial sums in the workspace; this call needs neither.
+ * It takes no context, calls no cudaMalloc / cudaFree / cudaMallocHost and no library routine that allocates,
+ * does not synchronise and copies nothing to the host: it enqueues two kernels on `cuda_stream` and returns.
+ *
+ *   n                      particles, 1 <= n < 2^32
+ *   x, px, py, pz          DEVICE, n doubles each (8-byte aligned), read only, owned by the caller; any order
+ *                          works, a cell-sorted store (cuba_state) is what the kernel is fast on
+ *   box[3], n_test         HOST: box edges in fm and the testparticle multiplier, as given to cuba_init
+ *   nslab                  1 .. CUBA_NOALLOC_MAX_SLABS equal slabs along x
+ *   result                 DEVICE, 4 + nslab doubles, owned by the caller, written in stream order:
+ *                          sum E, sum px, sum py, sum pz, then edens[nslab] = slab energy / (n_test V_slab)
+ *   cuda_stream            a cudaStream_t (NULL = default stream)
+ *
+ * Where the partial sums go: a fixed array inside the library image (static __device__, 592 x (4 +
+ * CUBA_NOALLOC_MAX_SLABS) doubles = 625,152 bytes).  Every GPU on which the library is loaded holds that array
+ * until the process exits, used or not -- which is why the limit on nslab is modest.  Consequences:
+ *   - nslab > CUBA_NOALLOC_MAX_SLABS returns CUBA_ERR_SIZE and launches nothing (use cuba_observables, whose
+ *     limit is 1024, if you can afford a context);
+ *   - the FIRST call on each device looks up the array's device address (cudaGetSymbolAddress with that device
+ *     current; the result is remembered per device).  Make that first call during set-up, outside any stream
+ *     capture; the call uses whatever device is current and `cuda_stream` must belong to it;
+ *   - all calls on a device share the one array.  Nothing in it has to be zero beforehand (every block
+ *     overwrites its whole row before the second kernel reads it, so the previous call's contents do not
+ *     matter), but two calls whose kernels can overlap on the GPU -- different streams without an ordering
+ *     between them, or two host threads -- race on it and give wrong sums.  Calls on one stream are safe.
+ * The arithmetic, grid and summation order are those of cuba_observables for nslab <= 2 nx: same bits there,
+ * within 1e-12 relative elsewhere.  Errors: CUBA_ERR_NULL, CUBA_ERR_SIZE (n, nslab), CUBA_ERR_VALUE (box,
+ * n_test, more than 64 devices), CUBA_ERR_WORKSPACE (misaligned pointer), CUBA_ERR_CUDA (no device; launch
+ * failed).  Device-side problems in the inputs (non-finite values) are not checked: the sums carry them. */
+#define CUBA_NOALLOC_MAX_SLABS 128
+int cuba_observables_noalloc(int64_t n, const double *x, const double *px, const double *py, const double *pz,
+                             const double box[3], double n_test, int nslab, double *result, void *cuda_stream);
+
 /* Where the current state lives (DEVICE pointers, valid until the next cuba_step). */
 int cuba_state(cuba_ctx *ctx, cuba_soa *out);
 

@@ -7,6 +7,7 @@ compute call needs the built library and a CUDA device and fails loudly otherwis
 """
 from .binding import (Cuba, CubaError, Counters, Trace, lib, lib_path, run_host,  # noqa: F401
                       workspace_bytes, launch_count, probe_fp64, strerror, EXPORTS,
+                      observables_noalloc, NOALLOC_MAX_SLABS,
                       OPT_FUSE_HIST, OPT_GRAPH, OPT_SLOTS, OPT_SLOT_MARGIN)
 
 from .slab import (SlabRank, LocalSlabGroup, slab_layers, layer_weights, initial_selection, neighbours,  # noqa: F401,E402
@@ -14,5 +15,5 @@ from .slab import (SlabRank, LocalSlabGroup, slab_layers, layer_weights, initial
 
 __all__ = ["SlabRank", "LocalSlabGroup", "slab_layers", "layer_weights", "initial_selection", "neighbours", "exchange_halos", "slab_step",
            "Cuba", "CubaError", "Counters", "Trace", "lib", "lib_path", "run_host",
-           "workspace_bytes", "launch_count", "probe_fp64", "strerror", "EXPORTS",
+           "workspace_bytes", "launch_count", "probe_fp64", "strerror", "EXPORTS", "observables_noalloc", "NOALLOC_MAX_SLABS",
            "OPT_FUSE_HIST", "OPT_GRAPH", "OPT_SLOTS", "OPT_SLOT_MARGIN"]

@@ -16,12 +16,14 @@ EXPORTS = ("cuba_workspace_bytes", "cuba_init", "cuba_step", "cuba_observables",
            "cuba_strerror", "cuba_last_cuda_error", "cuba_launch_count", "cuba_profile_enable",
            "cuba_profile_read", "cuba_profile_name", "cuba_set_option", "cuba_observables_lrf",
            "cuba_step_adaptive", "cuba_step_local_sigma", "cuba_probe_fp64", "cuba_slot_stats",
-           "cuba_slab_init", "cuba_slab_owned", "cuba_slab_count", "cuba_slab_buffer_bytes", "cuba_slab_pack", "cuba_slab_unpack")
+           "cuba_slab_init", "cuba_slab_owned", "cuba_slab_count", "cuba_slab_buffer_bytes", "cuba_slab_pack", "cuba_slab_unpack",
+           "cuba_observables_noalloc")
 
 
 # cuba_set_option
 OPT_FUSE_HIST, OPT_GRAPH, OPT_SLOTS, OPT_SLOT_MARGIN = 1, 2, 3, 4
 PROFILE_GROUPS = 21   # CUBA_PROFILE_GROUPS
+NOALLOC_MAX_SLABS = 128   # CUBA_NOALLOC_MAX_SLABS
 
 
 class CubaError(RuntimeError):
@@ -125,6 +127,7 @@ def lib():
         L.cuba_slab_buffer_bytes.restype = c_size_t
         L.cuba_slab_pack.argtypes = [c_void_p, c_int, c_void_p, c_size_t]
         L.cuba_slab_unpack.argtypes = [c_void_p, c_void_p, c_int64, c_void_p, c_int64]
+        L.cuba_observables_noalloc.argtypes = [c_int64] + [c_void_p] * 4 + [dp, c_double, c_int, c_void_p, c_void_p]
         L.cuba_profile_name.argtypes = [c_int]
         L.cuba_profile_name.restype = c_char_p
         _lib = L
@@ -165,6 +168,31 @@ def probe_fp64(stream=None, repeats=5) -> float:
     v = c_double(0.0)
     _check(lib().cuba_probe_fp64(c_void_p(stream) if stream else None, int(repeats), ctypes.byref(v)))
     return float(v.value)
+
+
+def observables_noalloc(x, px, py, pz, box, n_test, nslab, result, stream=None):
+    """cuba_observables_noalloc: sum E, sum p and the energy density per x-slab for a caller that may not
+    allocate GPU memory (a plug-in inside another program's memory budget, a hook between the steps of a
+    running loop, a service that allocates only at start-up).  Everything is the caller's: x, px, py, pz are
+    1-D float64 CUDA tensors of equal length, `result` a float64 CUDA tensor of 4 + nslab entries that
+    receives (sum E, sum px, sum py, sum pz, edens[nslab]) in stream order -- nothing is allocated, copied to
+    the host or waited for here.  nslab <= NOALLOC_MAX_SLABS (the partial sums live in a fixed array inside
+    the library; beyond it CubaError(-2)).  Calls share that array: keep them on one stream, or order them.
+    `stream`: a torch.cuda.Stream (default: the current one)."""
+    import torch
+    for a in (x, px, py, pz, result):
+        if not (a.is_cuda and a.dtype == torch.float64 and a.is_contiguous() and a.dim() == 1):
+            raise ValueError("x, px, py, pz and result must be contiguous 1-D float64 CUDA tensors")
+    n = int(x.shape[0])
+    if not (px.shape[0] == n and py.shape[0] == n and pz.shape[0] == n):
+        raise ValueError("x, px, py, pz must have the same length")
+    if result.shape[0] < 4 + int(nslab):
+        raise ValueError("result needs 4 + nslab entries")
+    st = stream if stream is not None else torch.cuda.current_stream(x.device)
+    with torch.cuda.device(x.device):
+        _check(lib().cuba_observables_noalloc(n, *[c_void_p(a.data_ptr()) for a in (x, px, py, pz)], _c3d(box),
+                                              float(n_test), int(nslab), c_void_p(result.data_ptr()),
+                                              c_void_p(st.cuda_stream)))
 
 
 def _np_ptr(a):

@@ -1469,6 +1469,65 @@ int cuba_observables_lrf(cuba_ctx *ctx, int nslab, double *T, double *lrf)
     return CUBA_OK;
 }
 
+// ---- cuba_observables_noalloc: the observables pass for callers that must not allocate -------------------
+// The per-CTA partial sums that cuba_observables keeps in the caller's workspace live here in a
+// fixed array that is part of the loaded library image instead: kObsGrid rows of 4 totals +
+// CUBA_NOALLOC_MAX_SLABS slab energies (592 x 132 doubles = 625,152 bytes on every GPU that loads
+// the library, until the process exits).
+static __device__ __align__(256) double g_noalloc_partial[(size_t)kObsGrid * (4 + CUBA_NOALLOC_MAX_SLABS)];
+
+namespace {
+constexpr int kNoallocMaxDevices = 64;
+std::mutex g_noalloc_mutex;
+double *g_noalloc_ptr[kNoallocMaxDevices] = {};   // device address of g_noalloc_partial on each device, once looked up
+}  // namespace
+
+// In host code the name g_noalloc_partial is only a handle for the runtime, not a device address: the
+// address a kernel can use has to be asked for, per device, with that device current.  Done on the first
+// call on each device and remembered; later calls on that device touch no CUDA API but the launches.
+static int noalloc_scratch(double **out)
+{
+    int dev = -1;
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kNoallocMaxDevices) return CUBA_ERR_VALUE;
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+        void *p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_noalloc_partial));
+        if (!p) return CUBA_ERR_CUDA;
+        g_noalloc_ptr[dev] = static_cast<double *>(p);
+    }
+    *out = g_noalloc_ptr[dev];
+    return CUBA_OK;
+}
+
+int cuba_observables_noalloc(int64_t n, const double *x, const double *px, const double *py, const double *pz,
+                             const double box[3], double n_test, int nslab, double *result, void *cuda_stream)
+{
+    if (!x || !px || !py || !pz || !box || !result) return CUBA_ERR_NULL;
+    if (n < 1 || n >= ((int64_t)1 << 32)) return CUBA_ERR_SIZE;
+    if (nslab < 1 || nslab > CUBA_NOALLOC_MAX_SLABS) return CUBA_ERR_SIZE;   // the fixed array has no room for more
+    for (int k = 0; k < 3; ++k) if (!(box[k] > 0.0) || !std::isfinite(box[k])) return CUBA_ERR_VALUE;
+    if (!(n_test > 0.0) || !std::isfinite(n_test)) return CUBA_ERR_VALUE;
+    for (const double *a : {x, px, py, pz, (const double *)result})
+        if (reinterpret_cast<uintptr_t>(a) & 7u) return CUBA_ERR_WORKSPACE;
+    double *partial = nullptr;
+    const int rc = noalloc_scratch(&partial);
+    if (rc != CUBA_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    // the same two kernels, grid, operation order and constants as cuba_observables with nslab <= 2 nx, so
+    // the sums come out with the same bits; every CTA writes its whole row of `partial` before the second
+    // kernel reads it, so what the previous call left in the array is never read and nothing needs clearing
+    const double inv_w = (double)nslab / box[0];
+    const double vol = ((n_test * (box[0] / (double)nslab)) * box[1]) * box[2];
+    k_observe_partial<false, false><<<kObsGrid, kObsThreads, (size_t)kObsWarps * nslab * 8, st>>>(n, x, px, py, pz, inv_w, nslab, 2,
+                                                                                             partial);
+    LAUNCHED();
+    k_observe_final<<<(4 + nslab + 7) / 8, 256, 0, st>>>(kObsGrid, nslab, partial, vol, result);
+    LAUNCHED();
+    return CUBA_OK;
+}
+
 int cuba_state(cuba_ctx *ctx, cuba_soa *out)
 {
     if (!ctx || !out) return CUBA_ERR_NULL;
