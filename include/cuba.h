@@ -49,6 +49,7 @@ extern "C" {
 #define CUBA_ERR_MOVED (-8)       /* device check: a particle crossed more than one cell      */
 #define CUBA_ERR_ROUNDS (-9)      /* a cell needs more than CUBA_MAX_ROUNDS rounds (A6)       */
 #define CUBA_ERR_TRACE (-10)      /* trace capacity too small                                 */
+#define CUBA_ERR_HALO (-11)       /* device check: a halo buffer's header is not the count given */
 
 #define CUBA_MAX_ROUNDS 64
 
@@ -142,7 +143,9 @@ int cuba_step_adaptive(cuba_ctx *ctx, int nsteps, double dt_max, double sigma, d
  * (cell, direction) histogram of the counting sort, so that consecutive steps with the same
  * dt skip the separate streaming/histogram pass; a step whose dt differs from the previous
  * one (or that follows cuba_init / cuba_step_traced) runs that pass.  value 0 always runs the
- * separate pass.  Errors: CUBA_ERR_NULL, CUBA_ERR_VALUE (unknown option or value). */
+ * separate pass.  Errors: CUBA_ERR_NULL, CUBA_ERR_VALUE (unknown option or value; in a slab context
+ * (cuba_slab_init) a non-zero value for CUBA_OPT_FUSE_HIST, CUBA_OPT_GRAPH or CUBA_OPT_SLOTS: those
+ * schedules are not available there and stay off). */
 #define CUBA_OPT_FUSE_HIST 1
 /* CUBA_OPT_GRAPH (default 1): for problems of up to 2^20 particles, whose step is bound by the host
  * cost of its launches, cuba_step replays a CUDA graph of two steps (captured on first use for the
@@ -310,7 +313,9 @@ int cuba_slab_pack(cuba_ctx *ctx, int side, void *buffer, size_t buffer_bytes);
  * buffers are what the lower / upper neighbour packed for its side 1 / side 0 (DEVICE; null exactly where there
  * is no neighbour), the counts those of cuba_slab_count there.  Stream-ordered after one synchronisation.
  * CUBA_ERR_SIZE if the capacity is exceeded, CUBA_ERR_VALUE for a buffer where no neighbour is (or none where
- * one is). */
+ * one is).  The header {count, cells per layer} that cuba_slab_pack wrote into each buffer is compared on the
+ * device with the count given here and with this grid; a mismatch (a buffer paired with the wrong count, a
+ * truncated transfer) surfaces as CUBA_ERR_HALO at the next synchronising call -- the store is then invalid. */
 int cuba_slab_unpack(cuba_ctx *ctx, const void *lo_buffer, int64_t lo_count, const void *hi_buffer, int64_t hi_count);
 
 /* fp64 leg of the roofline (fp64-pipe utilisation against a measured peak; no passage of

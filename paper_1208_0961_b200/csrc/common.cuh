@@ -22,6 +22,7 @@ constexpr uint32_t kFlagMoved = 1u;    // a particle crossed more than one cell 
 constexpr uint32_t kFlagRounds = 2u;   // a cell needed more than CUBA_MAX_ROUNDS rounds
 constexpr uint32_t kFlagState = 4u;    // invalid particle at init
 constexpr uint32_t kFlagTrace = 8u;    // trace capacity exceeded
+constexpr uint32_t kFlagHalo = 32u;    // cuba_slab_unpack: a halo buffer's header disagrees with the count it was given (16 = kFlagSlots)
 
 constexpr uint32_t kTagShuf = 0u, kTagDec = 1u, kTagDir = 2u;
 

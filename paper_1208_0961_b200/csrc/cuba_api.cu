@@ -160,6 +160,7 @@ struct cuba_ctx {
     int slot_mode = 0;            // CUBA_OPT_SLOTS: 0 never (default), 1 for calls of >= kSlotMinSteps steps, 2 for every call
     double slot_margin = 1.0;     // CUBA_OPT_SLOT_MARGIN (percent): scales the segment capacities (tests force overflows)
     double slot_boost = 1.0;      // grows after an overflow so that the next geometry is roomier
+    double slot_margin_built = 0.0;   // slot_margin * slot_boost the current store was laid out with
     unsigned char *slot_mem = nullptr;   // library-owned device memory: two slotted copies + the counter backup
     size_t slot_bytes = 0;
     SlotGeom slot_geom{};
@@ -201,6 +202,7 @@ const char *cuba_strerror(int code)
     case CUBA_ERR_MOVED: return "a particle crossed more than one cell in a step";
     case CUBA_ERR_ROUNDS: return "a cell needs more than 64 collision rounds";
     case CUBA_ERR_TRACE: return "trace capacity too small";
+    case CUBA_ERR_HALO: return "halo buffer does not hold the number of particles given to cuba_slab_unpack";
     default: return "unknown error";
     }
 }
@@ -232,6 +234,7 @@ static int device_flags_to_error(uint32_t f)
     if (f & kFlagMoved) return CUBA_ERR_MOVED;
     if (f & kFlagRounds) return CUBA_ERR_ROUNDS;
     if (f & kFlagTrace) return CUBA_ERR_TRACE;
+    if (f & kFlagHalo) return CUBA_ERR_HALO;
     return CUBA_OK;
 }
 
@@ -352,8 +355,10 @@ static int init_impl(cuba_ctx **out, const double box[3], const int ncell[3], in
     if (rc == CUBA_OK) rc = occupancy_grid(k_scatter<true>, kTileThreads, 2 * sizeof(TileStage<7>), sms, &ctx->grid_scat);
     if (rc == CUBA_OK) rc = occupancy_grid(k_scatter<false>, kTileThreads, 2 * sizeof(TileStage<7>), sms, &ctx->grid_scat);
     if (rc != CUBA_OK) return fail(rc);
-    if (const char *e = getenv("CUBA_DEBUG_GRID_C4")) ctx->grid_cls[4] = atoi(e) * sms;      // experiments only
-    if (const char *e = getenv("CUBA_DEBUG_GRID_SCAT")) ctx->grid_scat = atoi(e) * sms;
+#ifdef CUBA_DEBUG_KNOBS   // experiment builds only (-DCUBA_DEBUG_KNOBS): resident CTAs per SM of class 4 / of the scatter
+    if (const char *e = getenv("CUBA_DEBUG_GRID_C4")) ctx->grid_cls[4] = std::max(1, atoi(e)) * sms;
+    if (const char *e = getenv("CUBA_DEBUG_GRID_SCAT")) ctx->grid_scat = std::max(1, atoi(e)) * sms;
+#endif
     ctx->grid_o = sms;
     if (!cuda_ok(cudaFuncSetAttribute(k_observe_partial<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                       kObsWarps * kObsMaxSlabs * 8), "cudaFuncSetAttribute")) return fail(CUBA_ERR_CUDA);
@@ -724,7 +729,7 @@ static SlotGeom slot_geometry(const cuba_ctx *ctx, uint32_t nmax, double dt, dou
 static void slot_release(cuba_ctx *ctx)
 {
     if (ctx->slot_mem) cudaFree(ctx->slot_mem);
-    ctx->slot_mem = nullptr; ctx->slot_bytes = 0; ctx->slot_nmax = 0; ctx->slot_dt = 0.0;
+    ctx->slot_mem = nullptr; ctx->slot_bytes = 0; ctx->slot_nmax = 0; ctx->slot_dt = 0.0; ctx->slot_margin_built = 0.0;
 }
 
 // Make sure a slotted store fit for (nmax, dt) exists.  Returns false (and leaves the compact path in
@@ -733,7 +738,9 @@ static bool slot_prepare(cuba_ctx *ctx, uint32_t nmax, double dt)
 {
     if (ctx->slot_unavailable) return false;
     const double margin = ctx->slot_margin * ctx->slot_boost;
-    if (ctx->slot_mem && nmax <= ctx->slot_nmax && dt <= ctx->slot_dt) return true;
+    // reuse the store only if it was laid out with at least the margin asked for now: after a run outgrew a
+    // segment settle() raises slot_boost, and the next call must get the roomier geometry, not the old one
+    if (ctx->slot_mem && nmax <= ctx->slot_nmax && dt <= ctx->slot_dt && margin <= ctx->slot_margin_built) return true;
     slot_release(ctx);
     const uint32_t size_n = nmax + nmax / 16u;             // a little head room so that small fluctuations do not reallocate
     const SlotGeom sg = slot_geometry(ctx, size_n, dt, margin);
@@ -765,6 +772,7 @@ static bool slot_prepare(cuba_ctx *ctx, uint32_t nmax, double dt)
     ctx->slot_geom = sg;
     ctx->slot_nmax = size_n;
     ctx->slot_dt = dt;
+    ctx->slot_margin_built = margin;
     return true;
 }
 
@@ -1148,6 +1156,11 @@ int cuba_step_traced(cuba_ctx *ctx, double dt, double sigma, cuba_trace *out)
 int cuba_set_option(cuba_ctx *ctx, int option, int value)
 {
     if (!ctx) return CUBA_ERR_NULL;
+    // a slab context steps on the plain compact schedule only (cuba_slab_init): the slotted store and the graph
+    // would collide the ghost cells too, a fused histogram would cover the owned cells only -- switching one
+    // on is refused, switching it off (what it already is) is accepted
+    if (ctx->slab && value != 0 && (option == CUBA_OPT_SLOTS || option == CUBA_OPT_FUSE_HIST || option == CUBA_OPT_GRAPH))
+        return CUBA_ERR_VALUE;
     if (option == CUBA_OPT_SLOTS) {
         if (value < 0 || value > 2) return CUBA_ERR_VALUE;
         ctx->slot_mode = value;
@@ -1243,11 +1256,18 @@ static SlabRun slab_run_of_buffer(const unsigned char *b, uint32_t count)
 __global__ void __launch_bounds__(256)
 k_slab_counts(uint32_t ncells, const uint32_t *__restrict__ cell_start_old, uint32_t own_lo, uint32_t own_hi, uint32_t nyz,
               const uint32_t *__restrict__ lo_counts, const uint32_t *__restrict__ hi_counts,
-              uint32_t *__restrict__ count_new, uint32_t *__restrict__ block_sum)
+              uint32_t *__restrict__ count_new, uint32_t *__restrict__ block_sum,
+              const unsigned long long *__restrict__ lo_header, unsigned long long lo_count,
+              const unsigned long long *__restrict__ hi_header, unsigned long long hi_count, uint32_t *__restrict__ flags)
 {
     __shared__ uint32_t s_warp[8];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const uint32_t c = blockIdx.x * 256u + threadIdx.x;
+    // the header {particles, cells per layer} that cuba_slab_pack wrote must be the count the caller passed on:
+    // the sections of the buffer were addressed with that count
+    if (c == 0 && ((lo_header && (lo_header[0] != lo_count || lo_header[1] != nyz)) ||
+                   (hi_header && (hi_header[0] != hi_count || hi_header[1] != nyz))))
+        atomicOr(flags, kFlagHalo);
     uint32_t v = 0;
     if (c < ncells) {
         if (c >= own_lo && c < own_hi) v = cell_start_old[c + 1] - cell_start_old[c];
@@ -1350,7 +1370,10 @@ int cuba_slab_unpack(cuba_ctx *ctx, const void *lo_buffer, int64_t lo_count, con
     k_slab_counts<<<(unsigned)lay.nblocks_cells, 256, 0, st>>>(ncells, ctx->at<uint32_t>(lay.cell_start), ctx->own_lo, ctx->own_hi, nyz,
                                                                lb ? reinterpret_cast<const uint32_t *>(lb + 16 + (size_t)lo_count * 52) : nullptr,
                                                                hb ? reinterpret_cast<const uint32_t *>(hb + 16 + (size_t)hi_count * 52) : nullptr,
-                                                               ctx->at<uint32_t>(lay.count_new), ctx->at<uint32_t>(lay.block_sum));
+                                                               ctx->at<uint32_t>(lay.count_new), ctx->at<uint32_t>(lay.block_sum),
+                                                               reinterpret_cast<const unsigned long long *>(lb), (unsigned long long)lo_count,
+                                                               reinterpret_cast<const unsigned long long *>(hb), (unsigned long long)hi_count,
+                                                               ctx->at<uint32_t>(lay.flags));
     LAUNCHED();
     k_scan_blocks<<<1, 1024, 0, st>>>(ctx->at<uint32_t>(lay.block_sum), (int)lay.nblocks_cells, zero, kZeroWords);
     LAUNCHED();

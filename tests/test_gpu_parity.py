@@ -422,6 +422,31 @@ def test_slotted_run_that_outgrows_a_segment_is_redone_on_the_compact_schedule(c
     assert cg.device_flags == 0
 
 
+def test_slotted_store_grows_after_an_overflow(cuba, oracle_mod):
+    """after a run outgrew a segment the next call must lay the slotted store out with a larger
+    margin (x 1.5 per overflow) instead of reusing the undersized one and being redone on the compact schedule
+    every time.  From 20 % of the usual capacities at most a handful of calls are redone; after that the
+    slotted store runs without replays, and the state equals the oracle's all along."""
+    w = workloads.riemann(L=(6.0, 3.0, 2.0), ncell=(12, 3, 2), r_test=90.0, sigma_gev2=50.0, dt=0.05, seed=33)
+    g = cuba.Cuba.from_workload(w)
+    g.set_option(3, 2)
+    g.set_option(4, 20)
+    o = oracle_mod.Oracle.from_workload(w)
+    history = []
+    for _ in range(9):
+        g.step(3, w.dt, w.sigma)
+        o.step(3, w.dt, w.sigma)
+        history.append(g.slot_stats())
+    for a, c in zip(g.particles(), o.particles()):
+        assert np.array_equal(a, c)
+    runs, replays = zip(*history)
+    assert replays[0] >= 1, "20 % of the capacities was meant to overflow"
+    assert replays[-1] == replays[-2] == replays[-3], history       # the last calls were not redone ...
+    assert runs[-1] == runs[-3] + 2, history                        # ... and did run on the slotted store
+    assert replays[-1] <= 6, history                                # 0.2 * 1.5^k passes 1 at k = 4
+    assert g.counters().device_flags == 0
+
+
 @pytest.mark.parametrize("n", [129, 513, 897, 1537, 2049, 4545])
 def test_slotted_schedule_in_every_size_class(cuba, oracle_mod, n):
     """CUBA_OPT_SLOTS with one cell of n particles next to a thin one, particles spread over the whole cells so

@@ -130,8 +130,41 @@ def test_slab_argument_errors(cuba):
     first, cnt, n, cap = r.owned()
     assert 0 < first and first + cnt < n <= cap
     assert r.count(0) > 0 and r.count(1) > 0
+    # the schedules that are off in a slab context cannot be switched on afterwards (they would
+    # collide the ghost cells / bin with a histogram of the owned cells only); switching them off is a no-op
+    for opt, val in ((cuba.OPT_SLOTS, 2), (cuba.OPT_SLOTS, 1), (cuba.OPT_FUSE_HIST, 1), (cuba.OPT_GRAPH, 1)):
+        with pytest.raises(cuba.CubaError) as e:
+            r.set_option(opt, val)
+        assert e.value.code == -3                # CUBA_ERR_VALUE
+    for opt in (cuba.OPT_SLOTS, cuba.OPT_FUSE_HIST, cuba.OPT_GRAPH):
+        r.set_option(opt, 0)
+    before = r.counters()
+    r.step(1, w.dt, w.sigma)                     # still the compact schedule on the owned cells
+    assert r.counters().steps == before.steps + 1 and r.slot_stats() == (0, 0)
     with pytest.raises(cuba.CubaError):
         cuba.SlabRank(w, 5, 5)
     with pytest.raises(cuba.CubaError):
         cuba.SlabRank(w, 0, 4, capacity=10)
     r.close()
+
+
+def test_slab_unpack_checks_the_buffer_header(cuba):
+    """cuba_slab_unpack addresses the sections of a halo buffer with the count the caller passes on.
+    The header {count, cells per layer} that cuba_slab_pack wrote is compared with it on the device: a buffer
+    paired with the wrong count raises CUBA_ERR_HALO at the next synchronising call, the right pairing does not."""
+    w = workloads.riemann_small(seed=54)
+    lo, hi = cuba.SlabRank(w, 0, 4), cuba.SlabRank(w, 4, 8)
+    for r in (lo, hi):
+        r.step(1, w.dt, w.sigma)
+    up, down = lo.pack(1), hi.pack(0)             # (buffer, count) for the upper / lower neighbour
+    hi.unpack(up, None)
+    assert hi.counters().device_flags == 0        # matching header: clean
+    lo.unpack(None, (down[0], down[1] - 1))       # one particle short of what the header says
+    assert lo.counters().device_flags & 32        # kFlagHalo, sticky
+    with pytest.raises(cuba.CubaError) as e:
+        lo.observables(4)                         # the next call that synchronises and reports device errors
+    assert e.value.code == -11                    # CUBA_ERR_HALO
+    assert "halo" in cuba.strerror(-11)
+    lo.close()
+    hi.close()
+
