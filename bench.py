@@ -11,8 +11,9 @@ max over ranks.  The state (1.3 GB per copy) is far larger than the 126 MB L2, s
 flush is needed between steps.  N > 1 GPUs run N independent replicas (different seeds),
 no collective on the data path ("replicas only", scaling "weak").
 
-`--impl reference` times the CPU oracle, as it stands, on a bounded sample of the same
-workload (a transverse slice of the box: same densities, cells, dt, sigma).
+`--impl reference` times the CPU oracle, as it stands, on the same inputs (the configuration
+itself, every particle) for as many of the K steps as fit into about a minute of one host
+core; --quick (and the 54M / 100M-particle variants) use a transverse slice of the box instead.
 """
 from __future__ import annotations
 
@@ -204,21 +205,34 @@ class ClockSampler(threading.Thread):
                 "reasons": reasons, "samples": len(self.samples)}
 
 
-def oracle_sample_workload(config):
-    """The bounded sample of configs[config] the CPU oracle is timed on: same densities,
-    cell size, dt and sigma, a quarter of the transverse extent in y and z."""
+def oracle_sample_workload(config, quick=False, w_full=None):
+    """(workload, description, same_inputs) the CPU oracle is timed on.  Default: configs[config] ITSELF, every
+    particle (the same inputs, fewer steps) -- the bounded sample is then a few steps of it.  Only the
+    ~54M / ~100M-particle configs[4] variants, and --quick, fall back to a transverse slice of the box (same
+    densities, cell size, dt and sigma, a quarter of the extent in y and z)."""
+    if not quick and config in (0, 1, 2, 3):
+        w = w_full if w_full is not None else workloads.make(config)
+        return w, "configs[%d] itself, all %d particles" % (config, w.n), True
     if config in (1, 2):
         r = 10.0 if config == 1 else 100.0
         w = workloads.riemann(L=(32.0, 8.0, 8.0), ncell=(32, 8, 8), r_test=r, seed=config + 1)
-        return w, "configs[%d] restricted to a 32x8x8 fm^3 transverse slice (same T, r_test, cells, dt, sigma)" % config
+        return w, "configs[%d] restricted to a 32x8x8 fm^3 transverse slice (same T, r_test, cells, dt, sigma)" % config, False
     if config == 3:
         w = workloads.riemann(L=(32.0, 8.0, 8.0), ncell=(64, 8, 8), r_test=40.0, sigma_gev2=50.0, dt=0.05, seed=4)
-        return w, "configs[3] restricted to a 32x8x8 fm^3 transverse slice"
+        return w, "configs[3] restricted to a 32x8x8 fm^3 transverse slice", False
     if config in (4, 5):
         w = workloads.skewed(L=(64.0, 8.0, 8.0), ncell=(64, 8, 8), r_test=100.0 if config == 4 else 185.5, seed=5)
-        return w, "configs[4] restricted to a 64x8x8 fm^3 transverse slice"
+        return w, "configs[4] restricted to a 64x8x8 fm^3 transverse slice", False
     w = workloads.make(0)
-    return w, "configs[0] whole"
+    return w, "configs[0] whole", True
+
+
+def oracle_step_budget(n, steps, warmup, seconds):
+    """(timed steps, warm-up steps) of the oracle that fit into about `seconds` of one host core, assuming the
+    ~2.5 M particle-updates/s it reaches on stores far larger than the caches; never more than asked for."""
+    per_step = max(n, 1) / 2.5e6
+    timed = max(2, min(steps, int(seconds / per_step)))
+    return timed, (min(warmup, 1) if timed < steps else warmup)
 
 
 def time_oracle(w, steps, warmup):
@@ -238,15 +252,17 @@ def run_reference(args, rank, world):
     """--impl reference: the CPU oracle as it stands, host cores, rank 0 only."""
     if rank != 0:
         return
-    w, sample = oracle_sample_workload(args.config)
-    dt, c = time_oracle(w, args.steps, args.warmup)
-    value = w.n * args.steps / dt
+    w, sample, same = oracle_sample_workload(args.config, args.quick)
+    steps, warmup = oracle_step_budget(w.n, args.steps, args.warmup, 60.0)
+    dt, c = time_oracle(w, steps, warmup)
+    value = w.n * steps / dt
     full = workloads_name(args.config)
+    sample = "%s, %d timed steps after %d warm-up (asked: %d / %d), %.1f s" % (sample, steps, warmup, args.steps, args.warmup, dt)
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "steps": args.steps, "warmup": args.warmup, "steps_timed": steps, "warmup_run": warmup, "ms_per_step": 1e3 * dt / steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": full, "sample": sample, "n_particles": w.n},
+        "config": {"workload": full, "sample": sample, "n_particles": w.n, "same_inputs": same},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -367,6 +383,7 @@ def main():
                     help="N > 1: independent replicas (default, weak scaling) or ONE problem in x-slabs (strong scaling)")
     ap.add_argument("--slab-emulate", type=int, default=0, help="diagnostic: R slab ranks stepped in turn on one GPU (projection)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--quick", action="store_true", help="time the oracle on a transverse slice of the box instead of the configuration itself")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-fuse", action="store_true", help="run the separate k_stream_hist pass every step (A/B diagnostic)")
     ap.add_argument("--slots", type=int, default=-1, help="CUBA_OPT_SLOTS: 0 compact schedule, 1/2 slotted schedule; -1 library default (A/B diagnostic)")
@@ -588,12 +605,12 @@ def main():
                            "cold_value": n_total * e2e["steps"] / e2e["cold_s"], "cold_seconds": e2e["cold_s"],
                            "note": "value: second call (the library's memory pool already mapped); cold_value: first call of the process"}
         if not args.no_cpu_baseline:
-            ow, sample = oracle_sample_workload(args.config)
-            osteps = max(2, min(60, int(60e6 // max(ow.n, 1)) + 1))   # about 10-30 s of one host core
+            ow, sample, same = oracle_sample_workload(args.config, args.quick, w_full=w)
+            osteps = max(2, min(60, int(40e6 // max(ow.n, 1)) + 1))   # about 10-30 s of one host core
             odt, oc = time_oracle(ow, osteps, 0)
             line["cpu_baseline"] = {"value": ow.n * osteps / odt, "unit": UNIT, "cores": 1, "kind": "oracle",
                                     "sample": "%s, N=%d, %d steps, %.1f s" % (sample, ow.n, osteps, odt),
-                                    "host_cores_available": os.cpu_count()}
+                                    "same_inputs": same, "host_cores_available": os.cpu_count()}
         line["paper_context"] = ("CuBA 58.09 s vs BAMPS 756 s (~13x), GPU and CPU models not named in the paper "
                                  "(Fermi-era CUDA 4.1), run size not stated (PAPER.md:92)")
         print(json.dumps(line), flush=True)

@@ -298,6 +298,13 @@ int cuba_slab_init(cuba_ctx **out, const double box[3], const int ncell[3], int6
                    double *x, double *y, double *z, double *px, double *py, double *pz, const uint32_t *pid,
                    double n_test, uint64_t seed, void *workspace, size_t workspace_bytes, void *cuda_stream,
                    int layer_lo, int layer_hi);
+/* The cell layer along x of every particle, exactly as S3 computes it on the device (the cells the
+ * particles are sorted into; the same inline function as the kernels, compiled for the host: trunc(x * (1 /
+ * (box_x / nx))) clamped to [0, nx - 1]).  HOST in, HOST out, no device needed: x (n doubles), layer (n int32).
+ * This is what decides which rank is given a particle at the start (cuba_slab_init wants the particles of the
+ * layers [layer_lo - 1, layer_hi + 1)) and what the cuts are balanced with; a particle on a layer face goes where
+ * the device would bin it.  Errors: CUBA_ERR_NULL, CUBA_ERR_SIZE (n < 0, nx < 1), CUBA_ERR_VALUE (box_x). */
+int cuba_slab_layer_index(double box_x, int nx, int64_t n, const double *x, int32_t *layer);
 /* HOST out[4] = first slot of the owned part of the current store, its length, particles in the store, capacity.
  * Synchronises (reads four words back) once after a step. */
 int cuba_slab_owned(cuba_ctx *ctx, int64_t out[4]);

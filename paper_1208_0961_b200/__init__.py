@@ -10,10 +10,10 @@ from .binding import (Cuba, CubaError, Counters, Trace, lib, lib_path, run_host,
                       observables_noalloc, NOALLOC_MAX_SLABS,
                       OPT_FUSE_HIST, OPT_GRAPH, OPT_SLOTS, OPT_SLOT_MARGIN)
 
-from .slab import (SlabRank, LocalSlabGroup, slab_layers, layer_weights, initial_selection, neighbours,  # noqa: F401,E402
+from .slab import (SlabRank, LocalSlabGroup, slab_layers, layer_index, layer_weights, initial_selection, neighbours,  # noqa: F401,E402
                    exchange_halos, slab_step)
 
-__all__ = ["SlabRank", "LocalSlabGroup", "slab_layers", "layer_weights", "initial_selection", "neighbours", "exchange_halos", "slab_step",
+__all__ = ["SlabRank", "LocalSlabGroup", "slab_layers", "layer_index", "layer_weights", "initial_selection", "neighbours", "exchange_halos", "slab_step",
            "Cuba", "CubaError", "Counters", "Trace", "lib", "lib_path", "run_host",
            "workspace_bytes", "launch_count", "probe_fp64", "strerror", "EXPORTS", "observables_noalloc", "NOALLOC_MAX_SLABS",
            "OPT_FUSE_HIST", "OPT_GRAPH", "OPT_SLOTS", "OPT_SLOT_MARGIN"]

@@ -17,7 +17,7 @@ EXPORTS = ("cuba_workspace_bytes", "cuba_init", "cuba_step", "cuba_observables",
            "cuba_profile_read", "cuba_profile_name", "cuba_set_option", "cuba_observables_lrf",
            "cuba_step_adaptive", "cuba_step_local_sigma", "cuba_probe_fp64", "cuba_slot_stats",
            "cuba_slab_init", "cuba_slab_owned", "cuba_slab_count", "cuba_slab_buffer_bytes", "cuba_slab_pack", "cuba_slab_unpack",
-           "cuba_observables_noalloc")
+           "cuba_observables_noalloc", "cuba_slab_layer_index")
 
 
 # cuba_set_option
@@ -128,6 +128,7 @@ def lib():
         L.cuba_slab_pack.argtypes = [c_void_p, c_int, c_void_p, c_size_t]
         L.cuba_slab_unpack.argtypes = [c_void_p, c_void_p, c_int64, c_void_p, c_int64]
         L.cuba_observables_noalloc.argtypes = [c_int64] + [c_void_p] * 4 + [dp, c_double, c_int, c_void_p, c_void_p]
+        L.cuba_slab_layer_index.argtypes = [c_double, c_int, c_int64, c_void_p, c_void_p]
         L.cuba_profile_name.argtypes = [c_int]
         L.cuba_profile_name.restype = c_char_p
         _lib = L

@@ -87,9 +87,17 @@ __device__ __forceinline__ void stream_reflect(const Geom &g, double dt, double 
     reflect_axis(z, pz, g.L[2]);
 }
 
-__device__ __forceinline__ int axis_index(double x, double inv_d, int nc)
+// Also compiled for the host (cuba_slab_layer_index): there the conversion spells out what cvt.rzi.s32.f64 does
+// (truncation, saturation, NaN -> 0); the product rounds the same (IEEE fp64, no contraction on either side).
+__host__ __device__ __forceinline__ int axis_index(double x, double inv_d, int nc)
 {
+#ifdef __CUDA_ARCH__
     int i = __double2int_rz(x * inv_d);
+#else
+    const double v = x * inv_d;
+    int i = (v != v) ? 0 : (v >= 2147483647.0 ? 2147483647 : (v <= -2147483648.0 ? (-2147483647 - 1) : (int)v));
+    using std::min; using std::max;
+#endif
     i = min(i, nc - 1);                              // x == L lands in the last cell (A12)
     return max(i, 0);
 }

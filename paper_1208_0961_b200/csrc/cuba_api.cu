@@ -1286,6 +1286,16 @@ k_slab_counts(uint32_t ncells, const uint32_t *__restrict__ cell_start_old, uint
     }
 }
 
+int cuba_slab_layer_index(double box_x, int nx, int64_t n, const double *x, int32_t *layer)
+{
+    if (!x || !layer) return CUBA_ERR_NULL;
+    if (n < 0 || nx < 1) return CUBA_ERR_SIZE;
+    if (!(box_x > 0.0) || !std::isfinite(box_x)) return CUBA_ERR_VALUE;
+    const double inv_d = 1.0 / (box_x / (double)nx);       // as Geom::inv_d in init_impl
+    for (int64_t i = 0; i < n; ++i) layer[i] = axis_index(x[i], inv_d, nx);
+    return CUBA_OK;
+}
+
 size_t cuba_slab_buffer_bytes(int64_t count, const int ncell[3])
 {
     if (!ncell || count < 0) return 0;

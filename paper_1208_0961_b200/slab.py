@@ -48,19 +48,25 @@ def slab_layers(nx: int, world: int, weights=None):
     return [(cuts[k], cuts[k + 1]) for k in range(world)]
 
 
+def layer_index(x: np.ndarray, box_x: float, nx: int) -> np.ndarray:
+    """cuba_slab_layer_index: the S3 cell layer along x of every particle, computed by the library with the very
+    function its kernels bin with (HOST arrays, no device needed).  int32, one per particle."""
+    xs = np.ascontiguousarray(x, dtype=np.float64)
+    out = np.empty(xs.shape[0], dtype=np.int32)
+    _check(lib().cuba_slab_layer_index(float(box_x), int(nx), int(xs.shape[0]), c_void_p(xs.ctypes.data),
+                                       c_void_p(out.ctypes.data)))
+    return out
+
+
 def layer_weights(x: np.ndarray, box_x: float, nx: int) -> np.ndarray:
-    """Particles per cell layer along x (the S3 layer index of the library)."""
-    inv_d = 1.0 / (box_x / float(nx))
-    layer = np.clip((x * inv_d).astype(np.int64), 0, nx - 1)
-    return np.bincount(layer, minlength=nx).astype(np.float64)
+    """Particles per cell layer along x (counts of `layer_index`), to balance the cuts with."""
+    return np.bincount(layer_index(x, box_x, nx), minlength=nx).astype(np.float64)
 
 
 def initial_selection(x: np.ndarray, box_x: float, nx: int, layer_lo: int, layer_hi: int) -> np.ndarray:
     """Ascending global indices of the particles a rank is given at the start: those whose cell layer
-    (the S3 index of the library: trunc(x * (1 / (box_x / nx))), clamped) lies in [layer_lo - 1, layer_hi + 1)."""
-    inv_d = 1.0 / (box_x / float(nx))
-    layer = np.minimum((x * inv_d).astype(np.int64), nx - 1)
-    layer = np.maximum(layer, 0)
+    (`layer_index`, the library's S3 index) lies in [layer_lo - 1, layer_hi + 1)."""
+    layer = layer_index(x, box_x, nx)
     return np.nonzero((layer >= layer_lo - 1) & (layer < layer_hi + 1))[0]
 
 

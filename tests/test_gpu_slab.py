@@ -168,3 +168,28 @@ def test_slab_unpack_checks_the_buffer_header(cuba):
     lo.close()
     hi.close()
 
+
+
+def test_layer_index_agrees_with_the_device_binning(cuba):
+    """cuba_slab_layer_index (host) against S3 on the device (cuba_init's binning) for particles exactly on the
+    layer faces, one ulp to either side, at the walls, and in between -- on a grid whose cell edge (3.3 / 7) is
+    not a binary fraction: a particle goes to the ranks that the device will bin it for."""
+    nx, ny, nz, Lx = 7, 2, 2, 3.3
+    d = Lx / nx
+    rng = np.random.default_rng(9)
+    xs = np.concatenate([[k * d for k in range(nx + 1)], np.nextafter([k * d for k in range(1, nx + 1)], -np.inf),
+                         np.nextafter([k * d for k in range(nx)], np.inf), [Lx, np.nextafter(Lx, 0.0), 0.0],
+                         rng.uniform(0, Lx, 3000)])
+    xs = np.minimum(xs, Lx)
+    n = xs.size
+    base = workloads.thermal_box(L=(Lx, 1.0, 1.0), ncell=(nx, ny, nz), count=n, seed=77)
+    w = workloads.Workload("faces", (Lx, 1.0, 1.0), (nx, ny, nz), 2.0, 0.1, 0.05, 1, 77, 4,
+                           xs.copy(), base.y, base.z, base.px, base.py, base.pz)
+    g = cuba.Cuba.from_workload(w)
+    pid = g.particles()[0]
+    start = g.cell_start()
+    cell_of_slot = np.repeat(np.arange(nx * ny * nz), np.diff(start.astype(np.int64)))
+    dev_layer = np.empty(n, dtype=np.int64)
+    dev_layer[pid] = cell_of_slot // (ny * nz)
+    assert np.array_equal(cuba.layer_index(xs, Lx, nx), dev_layer)
+    g.close()

@@ -39,6 +39,45 @@ def test_slab_layers_cover_the_grid_in_whole_layers():
     assert neighbours(0, 3) == (None, 1) and neighbours(1, 3) == (0, 2) and neighbours(2, 3) == (1, None)
 
 
+@pytest.fixture(scope="module", autouse=True)
+def built_library():
+    from paper_1208_0961_b200 import build
+    build.build()          # layer_index goes through the C ABI (host function, no device needed)
+
+
+def test_layer_index_comes_from_the_library_and_handles_the_faces():
+    """the layer index that hands particles to ranks is the library's own S3 function
+    (cuba_slab_layer_index), not a numpy copy of it.  Faces: a particle exactly on the face between
+    layers k-1 and k belongs to k, one ulp below to k-1; x == L and beyond clamp to the last layer, x < 0 and NaN
+    to the first (what cvt.rzi does on the device)."""
+    from paper_1208_0961_b200.slab import layer_index, layer_weights
+    import paper_1208_0961_b200 as c
+    nx, Lx = 8, 8.0                                     # faces at the integers: x * 1.0 is exact
+    faces = np.arange(0, nx + 1, dtype=np.float64)
+    assert list(layer_index(faces, Lx, nx)) == [0, 1, 2, 3, 4, 5, 6, 7, 7]
+    assert list(layer_index(np.nextafter(faces[1:], -np.inf), Lx, nx)) == [0, 1, 2, 3, 4, 5, 6, 7]
+    assert list(layer_index(np.array([-0.0, -1e-300, -3.0, 1e300, np.inf, -np.inf, np.nan]), Lx, nx)) == [0, 0, 0, 7, 7, 0, 0]
+    # a cell edge that is not a binary fraction: the index is trunc(fl(x * fl(1 / fl(L / nx)))) -- checked in exact
+    # rational arithmetic on the three roundings, not by repeating the float expression
+    from fractions import Fraction
+    nx, Lx = 7, 3.3
+    d = Lx / nx
+    inv_d = 1.0 / d
+    xs = np.concatenate([[k * d for k in range(nx + 1)], np.nextafter([k * d for k in range(1, nx + 1)], -np.inf),
+                         np.nextafter([k * d for k in range(nx)], np.inf), np.random.default_rng(5).uniform(0, Lx, 200)])
+    got = layer_index(xs, Lx, nx)
+    for x, g in zip(xs, got):
+        prod = Fraction(float(x)) * Fraction(inv_d)     # exact product of the two doubles
+        fl = float(prod)                                # one correct rounding (Fraction -> float rounds to nearest even)
+        assert g == min(max(int(fl), 0), nx - 1)
+    assert layer_weights(xs, Lx, nx).sum() == xs.size
+    assert c.lib().cuba_slab_layer_index(8.0, 0, 1, None, None) == -1          # CUBA_ERR_NULL
+    one = np.zeros(1)
+    out = np.zeros(1, dtype=np.int32)
+    assert c.lib().cuba_slab_layer_index(8.0, 0, 1, one.ctypes.data, out.ctypes.data) == -2   # nx < 1
+    assert c.lib().cuba_slab_layer_index(0.0, 4, 1, one.ctypes.data, out.ctypes.data) == -3   # box
+
+
 def test_initial_selection_is_owned_plus_one_ghost_layer_in_global_order():
     import workloads
     from paper_1208_0961_b200.slab import initial_selection, slab_layers
