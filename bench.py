@@ -270,6 +270,33 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def short_run(cuba, torch, dev, config, steps, warmup):
+    """One short device-timed run of another configuration (no repeats, no per-kernel pass): W warm-up steps,
+    then K steps between CUDA events on the launching stream, state resident in HBM (far larger than L2)."""
+    w = workloads.CONFIGS[config]()
+    sim = cuba.Cuba.from_workload(w, device=dev)
+    sim.step(warmup, w.dt, w.sigma)
+    torch.cuda.synchronize()
+    c0 = sim.counters()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    sim.step(steps, w.dt, w.sigma)
+    ev1.record()
+    torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1)
+    c1 = sim.counters()
+    if c1.device_flags:
+        raise SystemExit("device error flags %d in configs[%d]" % (c1.device_flags, config))
+    out = {"workload": workloads_name(config), "n_particles": w.n, "steps": steps, "warmup": warmup,
+           "ms_per_step": ms / steps, "value": w.n * steps / (ms * 1e-3), "unit": UNIT,
+           "pair_evals_per_s": (c1.pairs - c0.pairs) / (ms * 1e-3), "max_occupancy": c1.max_occupancy,
+           "overflow_cells": c1.overflow_cells}
+    sim.close()
+    del sim
+    torch.cuda.empty_cache()
+    return out
+
+
 def reduce_over_ranks(dist, device, ms, e2e_s, n, pairs, launches):
     """Whole-job aggregation for N independent replicas: the time is the MAX over ranks, the
     work (particles, pair evaluations, launches) the SUM.  `dist` is torch.distributed or None."""
@@ -385,6 +412,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--quick", action="store_true", help="time the oracle on a transverse slice of the box instead of the configuration itself")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-other-configs", dest="other_configs", action="store_false",
+                    help="skip the short runs of configs[3] and configs[4] that the default line carries under other_configs")
     ap.add_argument("--no-fuse", action="store_true", help="run the separate k_stream_hist pass every step (A/B diagnostic)")
     ap.add_argument("--slots", type=int, default=-1, help="CUBA_OPT_SLOTS: 0 compact schedule, 1/2 slotted schedule; -1 library default (A/B diagnostic)")
     ap.add_argument("--import-ncu", default=None, help="ncu --csv log of a short bench run: write the tracked export under profiles/ and exit")
@@ -514,7 +543,16 @@ def main():
         torch.cuda.synchronize()
         e2e_s = time.perf_counter() - t0
         e2e = {"s": e2e_s, "steps": e2e_steps, "cold_s": cold_s}
+    ncells_main = sim.ncells
     sim.close()
+    del sim
+    torch.cuda.empty_cache()
+
+    # ---- the other large configurations, short runs (the driver's record should carry them too) ----
+    others = {}
+    if args.other_configs and world == 1 and args.config == 2:
+        for oc in (3, 4):
+            others["configs[%d]" % oc] = short_run(cuba, torch, dev, oc, 10, 3)
 
     # ---- reduce over ranks: max time, summed work --------------------------------------
     ms, e2e_s, n_total, pairs_total, launches = reduce_over_ranks(
@@ -562,7 +600,7 @@ def main():
                         "median": ms / args.steps, "best": min(reps) / args.steps,
                         "note": "every repeat times steps W..W+K from the same initial state (the step cost drifts as the profile evolves); "
                                 "value and ms_per_step are the median repeat; profiling off in the timed region"},
-            "config": {"workload": workloads_name(args.config), "n_particles": n, "ncells": sim.ncells,
+            "config": {"workload": workloads_name(args.config), "n_particles": n, "ncells": ncells_main,
                        "l2": "inputs larger than L2 (%.2f GB state per copy vs 126 MB L2), no flush" % (52 * n / 1e9)
                        if 52 * n > 4 * 126e6 else "state comparable to L2: cache-resident, not a roofline config",
                        "parallelism": "replicas x%d" % world if world > 1 else "single GPU",
@@ -611,6 +649,12 @@ def main():
             line["cpu_baseline"] = {"value": ow.n * osteps / odt, "unit": UNIT, "cores": 1, "kind": "oracle",
                                     "sample": "%s, N=%d, %d steps, %.1f s" % (sample, ow.n, osteps, odt),
                                     "same_inputs": same, "host_cores_available": os.cpu_count()}
+        if others:
+            pk = peak
+            for v in others.values():
+                v["roofline_step_frac"] = BYTES_STEP * v["value"] / 1e9 / pk
+                v["roofline_step_frac_moved_bytes"] = BYTES_STEP_FUSED * v["value"] / 1e9 / pk
+            line["other_configs"] = others
         line["paper_context"] = ("CuBA 58.09 s vs BAMPS 756 s (~13x), GPU and CPU models not named in the paper "
                                  "(Fermi-era CUDA 4.1), run size not stated (PAPER.md:92)")
         print(json.dumps(line), flush=True)

@@ -26,6 +26,13 @@ def cuba():
 
 @pytest.mark.parametrize("config", [1, 2, 3, 4])
 def test_full_size_step_sampled_against_oracle(cuba, oracle_mod, config):
+    # configs[3] (sigma = 50 GeV^-2) is the many-rounds regime: a wider sample there (parity gap b)
+    check_full_size_step(cuba, oracle_mod, config, n_hot=8 if config == 3 else 3, n_random=60 if config == 3 else 12)
+
+
+def check_full_size_step(cuba, oracle_mod, config, n_hot=3, n_random=12, expect_overflow=False):
+    """Body of the sampled full-size check; tests/test_zy_gpu_overflow_regime.py runs it on the ~100M-particle
+    variant (index 5), where the hottest cells are beyond the largest shared-memory class."""
     w = workloads.make(config)
     g = cuba.Cuba.from_workload(w)
     ncells = g.ncells
@@ -84,9 +91,14 @@ def test_full_size_step_sampled_against_oracle(cuba, oracle_mod, config):
     rng = np.random.default_rng(5)
     slot_b = np.empty(w.n, dtype=np.int64)
     slot_b[pidb] = np.arange(w.n)
-    hot = np.argsort(counts)[-3:]
-    sample = np.concatenate([hot, rng.integers(0, ncells, 12)])
+    hot = np.argsort(counts)[-n_hot:]
+    sample = np.concatenate([hot, rng.integers(0, ncells, n_random)])
     sample = np.array([c for c in sample if starta[c + 1] - starta[c] >= 2])
+    if config == 3:
+        # the fullest cells need four rounds (two full sweeps), typical hot-side cells three (a half-filled second sweep)
+        assert int(R[sample].max()) >= 3 and int((R[sample] == 3).sum()) >= 8 and int((R[sample] >= 3).sum()) >= n_hot + 8
+    if expect_overflow:
+        assert counts[hot].min() > 4544 and c2.overflow_cells - c1.overflow_cells >= n_hot   # k_collide_overflow did them
     # momenta before S5 of this step = S1-S2 of the oracle on the state before the step, in the new array order
     (rx, ry, rz, rpx, rpy, rpz), _ = oracle_mod.stream_reflect(*[a[slot_b[pida]] for a in sb], w.dt, w.box)
     lo, hi = starta[sample].astype(np.int64), starta[sample + 1].astype(np.int64)
@@ -95,6 +107,28 @@ def test_full_size_step_sampled_against_oracle(cuba, oracle_mod, config):
         for name, got, ref in (("px", sa[3], qx), ("py", sa[4], qy), ("pz", sa[5], qz)):
             assert np.array_equal(got[l:h], ref[l:h]), "cell %d %s" % (c, name)
     assert cnt["collisions"] > 0
+
+
+def test_config2_slotted_schedule_equals_compact_at_full_size(cuba):
+    """VERDICT r2, parity gap c: the opt-in slotted schedule (CUBA_OPT_SLOTS = 2) at north_star's size.  The
+    compact schedule is the one compared with the oracle bit for bit at this size (next test); the slotted run
+    must leave the identical store, cell table and counters after calls of 4 and 3 steps, without a replay."""
+    w = workloads.make(2)
+    a, b = cuba.Cuba.from_workload(w), cuba.Cuba.from_workload(w)
+    a.set_option(cuba.OPT_SLOTS, 2)
+    for k in (4, 3):
+        a.step(k, w.dt, w.sigma)
+        b.step(k, w.dt, w.sigma)
+    runs, replays = a.slot_stats()
+    assert runs == 2 and replays == 0 and b.slot_stats() == (0, 0)
+    for name, u, v in zip("pid x y z px py pz".split(), a.particles(), b.particles()):
+        assert np.array_equal(u, v), name
+    assert np.array_equal(a.cell_start(), b.cell_start())
+    ca, cb = a.counters(), b.counters()
+    assert (ca.pairs, ca.collisions, ca.rounds, ca.near_threshold) == (cb.pairs, cb.collisions, cb.rounds, cb.near_threshold)
+    assert ca.device_flags == 0 and cb.device_flags == 0
+    a.close()
+    b.close()
 
 
 def test_config2_whole_state_against_oracle(cuba, oracle_mod):
