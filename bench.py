@@ -49,7 +49,7 @@ BYTES_STEP_FUSED = BYTES_SCATTER + BYTES_COLLIDE_FUSED           # 180: what the
 # number.  Metrics: dram__bytes_read.sum, dram__bytes_write.sum, smsp__inst_executed.sum,
 # sm__inst_executed_pipe_fp64.sum (warp-level), gpu__time_duration.sum, launch__registers_per_thread,
 # sm__warps_active.avg.pct_of_peak_sustained_active.
-NCU_EXPORT = os.path.join(ROOT, "profiles", "r02_ncu_step_c%d.csv")
+NCU_EXPORT = os.path.join(ROOT, "profiles", "r03_ncu_step_c%d.csv")
 ISSUE_SLOTS_PER_CLOCK = 148 * 4
 
 
@@ -106,7 +106,7 @@ def ncu_export(config):
 
 
 def import_ncu(raw_csv, config):
-    """`python bench.py --import-ncu <ncu --csv log> --config C`: writes the tracked export profiles/r02_ncu_step_cC.csv:
+    """`python bench.py --import-ncu <ncu --csv log> --config C`: writes the tracked export profiles/r03_ncu_step_cC.csv:
     the rows of the LAST launch of every kernel instantiation (one step), headed by the hash of the kernel
     sources they were measured on."""
     import csv

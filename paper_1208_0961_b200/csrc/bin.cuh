@@ -360,15 +360,18 @@ k_carry(int ntiles, const uint32_t *__restrict__ tile_rec, uint32_t *__restrict_
 // local index li = r*32 + lane = j*256 + tid.  prefix_d(li) = number of particles before li
 // in the tile that moved in direction d.  Stable rank inside (c_old, d) =
 // prefix_d(li) - prefix_d(first particle of c_old in the tile) [+ carry if that is li 0].
+#ifndef CUBA_SCAT_MB   // resident CTAs per SM asked for the scatter (build-time tunable; 4 needs <= 64 registers)
+#define CUBA_SCAT_MB 3
+#endif
 template <bool WITH_CELL_OF_PID>
-__global__ void __launch_bounds__(kTileThreads, 3)
+__global__ void __launch_bounds__(kTileThreads, CUBA_SCAT_MB)
 k_scatter(Geom g, double dt, int64_t n, int64_t ntiles, Soa in, Soa out, const uint32_t *__restrict__ dest_base,
           const uint32_t *__restrict__ carry, uint32_t *__restrict__ cell_of_pid)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     TileStage<7> *stage = reinterpret_cast<TileStage<7> *>(smem_raw);
     __shared__ __align__(8) uint64_t s_bar[2];
-    __shared__ uint32_t s_cold[kTile];
+    __shared__ uint32_t s_rowlast[kTileRows];   // old cell of the last particle of every row (its successor is lane 0 of the next row)
     __shared__ uint32_t s_ball[kTileRows][kDirs];
     __shared__ uint32_t s_pref[kTileRows][kDirs];
     __shared__ uint32_t s_head[kTileRows];
@@ -397,7 +400,7 @@ k_scatter(Geom g, double dt, int64_t n, int64_t ntiles, Soa in, Soa out, const u
             m[j].d = -1; m[j].c_old = 0xFFFFFFFFu;
             if (base + li < n)
                 m[j] = move_particle(g, dt, st.v[0][li], st.v[1][li], st.v[2][li], st.v[3][li], st.v[4][li], st.v[5][li]);
-            s_cold[li] = m[j].c_old;
+            if (lane == 31) s_rowlast[j * (kTileThreads / 32) + wid] = m[j].c_old;
             dbase[j] = (m[j].d >= 0) ? dest_base[(size_t)m[j].d * g.ncells + m[j].c_old] : 0u;
         }
         __syncthreads();
@@ -410,7 +413,11 @@ k_scatter(Geom g, double dt, int64_t n, int64_t ntiles, Soa in, Soa out, const u
             // one bit mask per direction present in the row (absent directions stay zero)
             const uint32_t peers = __match_any_sync(0xFFFFFFFFu, dd);
             if (dd >= 0 && (peers & lanemask_lt()) == 0) s_ball[r][dd] = peers;
-            const bool head = valid && (li == 0 || s_cold[li - 1] != m[j].c_old);
+            // the predecessor's old cell: the lane below, for lane 0 the last lane of the previous row (2 KB of
+            // shared memory less than a per-particle table: four CTAs fit an SM with it)
+            uint32_t prev = __shfl_up_sync(0xFFFFFFFFu, m[j].c_old, 1);
+            if (lane == 0) prev = r > 0 ? s_rowlast[r - 1] : 0xFFFFFFFFu;
+            const bool head = valid && (li == 0 || prev != m[j].c_old);
             const uint32_t hb = __ballot_sync(0xFFFFFFFFu, head);
             if (lane == 0) s_head[r] = hb;
         }
