@@ -297,6 +297,55 @@ def short_run(cuba, torch, dev, config, steps, warmup):
     return out
 
 
+def run_two_stream_probe(args):
+    """--two-stream-probe (diagnostic): how much do the kernels of two independent problems overlap on one GPU?
+    Two half-size copies of configs[2] (32x32x16 fm^3 each: the same cell populations, half the cells) are stepped
+    K times (a) one after the other and (b) on two streams with their step(1) calls interleaved; wall clock
+    between device synchronisations.  A proxy for running the scatter of some cell layers under the collisions of
+    others (round 3); no bench value."""
+    import torch
+    import paper_1208_0961_b200 as cuba
+    dev = torch.device("cuda", 0)
+    K = args.steps
+    ws = [workloads.riemann(L=(32.0, 32.0, 16.0), ncell=(32, 32, 16), r_test=100.0, seed=s) for s in (3, 4)]
+    streams = [torch.cuda.Stream(device=dev) for _ in ws]
+    ctx = []
+    for w, st in zip(ws, streams):
+        with torch.cuda.stream(st):
+            ctx.append(cuba.Cuba.from_workload(w, device=dev, stream=st))
+    for c, w in zip(ctx, ws):
+        c.step(max(args.warmup, 3), w.dt, w.sigma)
+
+    def timed(fn):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        fn()
+        torch.cuda.synchronize()
+        return 1e3 * (time.perf_counter() - t0)
+
+    def one_after_the_other():
+        for c, w in zip(ctx, ws):
+            c.step(K, w.dt, w.sigma)
+            torch.cuda.synchronize()
+
+    def interleaved():
+        for _ in range(K):
+            for c, w in zip(ctx, ws):
+                c.step(1, w.dt, w.sigma)
+
+    seq = [timed(one_after_the_other) for _ in range(2)]
+    con = [timed(interleaved) for _ in range(2)]
+    line = {"probe": "two half-size copies of configs[2] on two streams", "n_particles_each": ws[0].n, "steps": K,
+            "sequential_ms_per_step_of_both": min(seq) / K, "interleaved_ms_per_step_of_both": min(con) / K,
+            "gain": 1.0 - min(con) / min(seq), "lib": cuba.lib_path(),
+            "grid_c4_knob": os.environ.get("CUBA_DEBUG_GRID_C4"), "note": "diagnostic, not a bench value"}
+    for c in ctx:
+        if c.counters().device_flags:
+            raise SystemExit("device error flags")
+        c.close()
+    print(json.dumps(line), flush=True)
+
+
 def reduce_over_ranks(dist, device, ms, e2e_s, n, pairs, launches):
     """Whole-job aggregation for N independent replicas: the time is the MAX over ranks, the
     work (particles, pair evaluations, launches) the SUM.  `dist` is torch.distributed or None."""
@@ -409,6 +458,8 @@ def main():
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: independent replicas (default, weak scaling) or ONE problem in x-slabs (strong scaling)")
     ap.add_argument("--slab-emulate", type=int, default=0, help="diagnostic: R slab ranks stepped in turn on one GPU (projection)")
+    ap.add_argument("--two-stream-probe", action="store_true",
+                    help="diagnostic: two half-size copies of configs[2] stepped one after the other vs interleaved on two streams")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--quick", action="store_true", help="time the oracle on a transverse slice of the box instead of the configuration itself")
     ap.add_argument("--no-e2e", action="store_true")
@@ -430,6 +481,10 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank, world)
+        return
+    if args.two_stream_probe:
+        if rank == 0:
+            run_two_stream_probe(args)
         return
     if args.decomp == "slab" or args.slab_emulate:
         run_slab(args, rank, world, local)
